@@ -1,0 +1,139 @@
+/*
+ * sg.h — C-ABI of libsg_b200: the Monte Carlo hot path of arXiv:1403.4560 on one B200 (sm_100a).
+ *
+ * What the library computes (citations: PAPER.md:<line> of /root/reference/PAPER.md; R<n> = reading
+ * n in DESIGN.md §3, taken where the paper is silent):
+ *   - the 3D Edwards-Anderson Hamiltonian  H = -sum_<ij> J_ij S_i S_j - h sum_i S_i  on a periodic
+ *     L^3 simple-cubic lattice, J_ij = +-1 equiprobable (Eq. 1) or N(0,1) in fp32
+ *     (PAPER.md:120 mention; BASELINE.json config 4);
+ *   - checkerboard Metropolis sweeps ("spin flip attempt"; R2-R6) of n_samples disorder
+ *     samples x n_replicas replicas x n_temps temperature slots;
+ *   - parallel tempering between neighbouring temperatures (R12);
+ *   - the replica overlap q(k) = (1/N) sum_j S^a_j S^b_j exp(i k.r_j) (Eq. 2) at k = 0
+ *     and 12 small wave vectors (R8) for every replica pair, and running sums
+ *     of the moments entering Eqs. 3-6 (R9).
+ *
+ * Conventions
+ *   - every function returns SG_OK (0) or a negative sg_status; nothing is printed, nothing exits;
+ *     output arguments are untouched on failure; sg_last_error() gives a description.
+ *   - "host ptr" / "device ptr" is stated per argument.  The caller owns every buffer it passes.
+ *   - all GPU work is enqueued on the stream given to sg_create; calls that fill HOST buffers
+ *     synchronise that stream before returning, the others are asynchronous.
+ *   - a context is not thread-safe; one context = one GPU (the current device at sg_create).
+ *   - site index i = x + L*(y + L*z); sample index s = 32*w + lane for the packed +-J path;
+ *     replica pairs in the order (0,1),(0,2),(0,3),(1,2),(1,3),(2,3).
+ */
+#ifndef SG_B200_H
+#define SG_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sg_ctx sg_ctx; /* opaque */
+
+typedef enum sg_status {
+    SG_OK = 0,
+    SG_EINVAL = -1,       /* bad argument (see each function) */
+    SG_ENOMEM = -2,       /* host or device allocation failed / workspace too small */
+    SG_ECUDA = -3,        /* a CUDA call or kernel launch failed; sg_last_error has the CUDA string */
+    SG_EUNSUPPORTED = -4, /* valid request outside what the kernels support */
+    SG_ESTATE = -5        /* call not valid in the current state */
+} sg_status;
+
+enum { SG_PMJ = 0, SG_GAUSS = 1 }; /* coupling_kind */
+
+#define SG_NK 12   /* non-zero wave vectors per record (R8) */
+#define SG_REC 25  /* doubles per (sample, slot, pair) record: q(0), Re q(K0), Im q(K0), ... (R9) */
+#define SG_NMOM 66 /* accumulator doubles per (sample, slot) (R9) */
+
+/* Bytes of device workspace sg_create needs for these parameters (0 if they are invalid).
+ * The workspace must be 256-byte aligned. */
+size_t sg_workspace_bytes(int L, int n_samples, int n_replicas, int n_temps, int coupling_kind);
+
+/* Create a simulation: validates, builds the beta / threshold tables on the host in double (R4),
+ * and generates couplings and random initial spins on the device from Philox4x32-10 keyed by
+ * `seed` (R5, R6).
+ *   out           host ptr, receives the context
+ *   L             even, 4 <= L <= 64 (checkerboard needs even L; R3)
+ *   h             external field, any finite double
+ *   n_samples     >= 1 disorder samples; the +-J path packs 32 per uint32 (idle lanes are ignored)
+ *   n_replicas    2 or 4 replicas per (sample, temperature) (R9)
+ *   temps         host ptr, n_temps temperatures T > 0, non-decreasing (slot 0 coldest); copied
+ *   n_temps       1 <= n_temps <= 64
+ *   coupling_kind SG_PMJ or SG_GAUSS
+ *   workspace     device ptr, 256-byte aligned, >= sg_workspace_bytes(...) bytes, must outlive the
+ *                 context; or NULL: the library cudaMallocs (and frees in sg_destroy)
+ *   cuda_stream   a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL = default
+ * Errors: SG_EINVAL (any violated constraint, null out/temps, misaligned workspace), SG_ENOMEM
+ * (workspace too small, allocation failure), SG_ECUDA. */
+int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, const double *temps,
+              int n_temps, int coupling_kind, uint64_t seed, void *workspace, size_t workspace_bytes,
+              void *cuda_stream);
+
+/* Regenerate couplings and initial spins from the seed, zero the counters and the accumulators:
+ * the state right after sg_create, without reallocating.  Asynchronous. */
+int sg_reset(sg_ctx *ctx);
+
+/* n >= 0 full checkerboard Metropolis sweeps of every system, colour 0 then colour 1 (R2, R3),
+ * no exchange, no measurement.  Asynchronous. */
+int sg_sweep(sg_ctx *ctx, int n);
+
+/* One parallel-tempering exchange step: pairs (t, t+1) with t = e mod 2 for the e-th call (R12),
+ * decided per (sample, replica); accepted pairs trade configurations.  Asynchronous. */
+int sg_pt_exchange(sg_ctx *ctx);
+
+/* Measure the overlaps of all replica pairs at every slot (Eq. 2) and add their moments to the
+ * device accumulators (R9).
+ *   out  host ptr to [n_samples][n_temps][n_pairs][SG_REC] doubles, or NULL (then asynchronous). */
+int sg_measure(sg_ctx *ctx, double *out);
+
+/* Fused driver, bit-identical to the primitive sequence (R16):
+ *   for s in 1..n_sweeps: sweep; if pt_every>0 and sweeps_done % pt_every == 0: exchange;
+ *                                if meas_every>0 and sweeps_done % meas_every == 0: measure(NULL)
+ * (sweeps_done = global sweep counter).  Asynchronous. */
+int sg_run(sg_ctx *ctx, int n_sweeps, int pt_every, int meas_every);
+
+/* Block until all enqueued work of this context has finished. */
+int sg_synchronize(sg_ctx *ctx);
+
+/* Free the context and whatever the library allocated (never the caller's workspace). */
+int sg_destroy(sg_ctx *ctx);
+
+/* ---- introspection (canonical unpacked layouts, HOST pointers, synchronous) ---- */
+
+/* out: [n_samples][n_replicas][n_temps][N] int8, values +-1 */
+int sg_get_spins(sg_ctx *ctx, int8_t *out);
+/* in: same layout; any value > 0 means +1 */
+int sg_set_spins(sg_ctx *ctx, const int8_t *in);
+/* out: [n_samples][3][N] float; entry (d, i) is the bond i -> i+e_d; +-1.0f for SG_PMJ */
+int sg_get_couplings(sg_ctx *ctx, float *out);
+/* The same three for the samples [s0, s0+ns) only (buffers sized for ns samples): what the
+ * parity tests use at full BASELINE.json sizes.  SG_EINVAL if the range is empty or out of bounds. */
+int sg_get_spins_range(sg_ctx *ctx, int s0, int ns, int8_t *out);
+int sg_set_spins_range(sg_ctx *ctx, int s0, int ns, const int8_t *in);
+int sg_get_couplings_range(sg_ctx *ctx, int s0, int ns, float *out);
+/* U: [n_samples][n_replicas][n_temps] int64 — SG_PMJ: number of unsatisfied bonds (E = 2U - 3N - hM);
+ * SG_GAUSS: fixed-point E_fix = -sum trunc(J 2^32) S_i S_j (R14).  M: same shape int32, sum of spins.
+ * Either pointer may be NULL. */
+int sg_get_energies(sg_ctx *ctx, int64_t *U, int32_t *M);
+/* out: [n_temps][7][2] uint64 Metropolis thresholds thr[t][n_u][a] in [0, 2^32] (R4) */
+int sg_get_thresholds(sg_ctx *ctx, uint64_t *out);
+/* out: [n_samples][n_temps][SG_NMOM] doubles (may be NULL); n_meas: measurements so far (may be NULL) */
+int sg_get_moments(sg_ctx *ctx, double *out, int64_t *n_meas);
+/* global sweep / exchange counters (either may be NULL) */
+int sg_get_counters(sg_ctx *ctx, uint64_t *sweeps_done, uint64_t *exchanges_done);
+/* number of kernels this context has launched so far (for bench.py's gpu_launches) */
+int sg_get_launch_count(sg_ctx *ctx, uint64_t *launches);
+
+/* Description of the last error of this context (or of the last failed sg_create if ctx is NULL).
+ * The string is owned by the library and valid until the next call on the same context. */
+const char *sg_last_error(sg_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SG_B200_H */

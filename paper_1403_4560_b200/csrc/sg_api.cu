@@ -1,0 +1,451 @@
+// sg_api.cu — the C-ABI of libsg_b200 (include/sg.h): argument validation, workspace layout,
+// host-side tables (R4, R12, R13), and the call sequences that drive the kernels.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "sg_internal.h"
+
+using namespace sg;
+
+namespace {
+
+thread_local std::string g_create_err;
+
+constexpr size_t ALIGN = 256;
+constexpr size_t SCRATCH_CAP = (size_t)128 << 20;    // per scratch buffer
+constexpr int DEXP64_N = 5761, DEXP32_N = 1441;
+
+inline size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Layout {
+    size_t spins, J, tab, exp64, exp32, tw, U, M, swap, acc, hist, rec, stage, total;
+    int chunk_meas, chunk_stage, S_pad;
+};
+
+bool valid_args(int L, int n_samples, int R, int NT, int kind)
+{
+    if (L < 4 || L > 64 || (L & 1)) return false;
+    if (n_samples < 1 || n_samples > (1 << 24)) return false;
+    if (R != 2 && R != 4) return false;
+    if (NT < 1 || NT > MAX_NT) return false;
+    if (kind != SG_PMJ && kind != SG_GAUSS) return false;
+    return true;
+}
+
+Layout make_layout(int L, int n_samples, int R, int NT, int kind)
+{
+    Layout lo;
+    const size_t N = (size_t)L * L * L;
+    const int P = R * (R - 1) / 2;
+    const int W = (n_samples + 31) / 32;
+    lo.S_pad = kind == SG_PMJ ? W * 32 : n_samples;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += up(bytes); return o; };
+    if (kind == SG_PMJ) {
+        lo.spins = take((size_t)W * R * NT * N * 4);
+        lo.J = take((size_t)W * 3 * N * 4);
+    } else {
+        lo.spins = take((size_t)n_samples * R * NT * N);
+        lo.J = take((size_t)n_samples * 3 * N * 4);
+    }
+    lo.tab = take(sizeof(SlotTab) * NT);
+    lo.exp64 = take(sizeof(double) * DEXP64_N);
+    lo.exp32 = take(sizeof(float) * DEXP32_N);
+    lo.tw = take(sizeof(double) * 2 * L);
+    lo.U = take(sizeof(int64_t) * (size_t)lo.S_pad * R * NT);
+    lo.M = take(sizeof(int32_t) * (size_t)lo.S_pad * R * NT);
+    lo.swap = take(sizeof(uint32_t) * (size_t)lo.S_pad * R * (NT / 2 + 1));
+    lo.acc = take(sizeof(double) * (size_t)n_samples * NT * SG_NMOM);
+    // measurement scratch, chunked over samples (multiples of 32)
+    const size_t hist_per = (size_t)NT * P * N_HIST * L * sizeof(uint16_t);
+    const size_t rec_per = (size_t)NT * P * SG_REC * sizeof(double);
+    size_t cm = SCRATCH_CAP / std::max(hist_per, rec_per);
+    cm = std::max<size_t>(32, cm / 32 * 32);
+    cm = std::min<size_t>(cm, (size_t)(n_samples + 31) / 32 * 32);
+    lo.chunk_meas = (int)cm;
+    lo.hist = take(hist_per * cm);
+    lo.rec = take(rec_per * cm);
+    const size_t stage_per = std::max((size_t)R * NT * N, 12 * N);
+    size_t cs = std::max<size_t>(1, SCRATCH_CAP / stage_per);
+    cs = std::min<size_t>(cs, (size_t)n_samples);
+    lo.chunk_stage = (int)cs;
+    lo.stage = take(stage_per * cs);
+    lo.total = off;
+    return lo;
+}
+
+int fail(sg_ctx *c, int code, const std::string &msg)
+{
+    if (c) c->err = msg; else g_create_err = msg;
+    return code;
+}
+
+int check_cuda(sg_ctx *c, cudaError_t e, const char *what)
+{
+    if (e == cudaSuccess) return SG_OK;
+    return fail(c, SG_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+int check_launch(sg_ctx *c, const char *what)
+{
+    return check_cuda(c, cudaGetLastError(), what);
+}
+
+// host tables -> device (R4, R12, R13)
+int upload_tables(sg_ctx *c)
+{
+    const int NT = c->d.NT;
+    const double h = c->h;
+    std::vector<SlotTab> tabs(NT);
+    c->thr.assign((size_t)NT * 14, 0);
+    c->beta.resize(NT);
+    bool monotone = fabs(h) <= 1.0;
+    for (int t = 0; t < NT; ++t) {
+        const double beta = 1.0 / c->temps[t];
+        c->beta[t] = beta;
+        memset(&tabs[t], 0, sizeof(SlotTab));
+        tabs[t].beta = beta;
+        tabs[t].beta_f = (float)(1.0 / c->temps[t]);
+        for (int nu = 0; nu <= 6; ++nu)
+            for (int a = 0; a < 2; ++a) {
+                const double dE = (double)(12 - 4 * nu) + (a ? 2.0 * fabs(h) : -(2.0 * fabs(h)));
+                uint64_t th;
+                if (dE <= 0.0) th = 4294967296ULL;
+                else {
+                    const double p = floor(exp(-beta * dE) * 4294967296.0);
+                    th = p >= 4294967296.0 ? 4294967296ULL : (uint64_t)p;
+                }
+                c->thr[((size_t)t * 7 + nu) * 2 + a] = th;
+                const uint64_t neg = (uint64_t)0 - th;
+                tabs[t].c64g[nu][a] = make_uint2((uint32_t)neg, (uint32_t)(neg >> 32));
+            }
+        // comparator path: code c = 2 n_u + (1 - a); needs thr non-decreasing in c and thr = 2^32 for c >= 7
+        uint64_t prev = 0;
+        for (int code = 0; code < 14; ++code) {
+            const int nu = code >> 1, a = 1 - (code & 1);
+            const uint64_t th = c->thr[((size_t)t * 7 + nu) * 2 + a];
+            if (th < prev) monotone = false;
+            if (code >= 7 && th != 4294967296ULL) monotone = false;
+            prev = th;
+            if (code < 7) tabs[t].c64[code] = tabs[t].c64g[nu][a];
+        }
+    }
+    c->d.fast_accept = monotone ? 1 : 0;
+    std::vector<double> t64(DEXP64_N);
+    std::vector<float> t32(DEXP32_N);
+    for (int i = 0; i < DEXP64_N; ++i) t64[i] = exp(-(double)i / 256.0);
+    for (int i = 0; i < DEXP32_N; ++i) t32[i] = (float)exp(-(double)i / 64.0);
+    const int L = c->d.L;
+    std::vector<double> tw(2 * L);
+    for (int m = 0; m < L; ++m) {
+        const double ph = 2.0 * 3.14159265358979323846 * (double)m / (double)L;
+        tw[m] = cos(ph);
+        tw[L + m] = sin(ph);
+    }
+    int rc;
+    if ((rc = check_cuda(c, cudaMemcpyAsync(c->tab, tabs.data(), sizeof(SlotTab) * NT, cudaMemcpyHostToDevice, c->stream), "upload tab"))) return rc;
+    if ((rc = check_cuda(c, cudaMemcpyAsync(c->exp64_tab, t64.data(), sizeof(double) * DEXP64_N, cudaMemcpyHostToDevice, c->stream), "upload exp64"))) return rc;
+    if ((rc = check_cuda(c, cudaMemcpyAsync(c->exp32_tab, t32.data(), sizeof(float) * DEXP32_N, cudaMemcpyHostToDevice, c->stream), "upload exp32"))) return rc;
+    if ((rc = check_cuda(c, cudaMemcpyAsync(c->twiddle, tw.data(), sizeof(double) * 2 * L, cudaMemcpyHostToDevice, c->stream), "upload twiddle"))) return rc;
+    // the host vectors die at return: the copies above come from pageable memory, which
+    // cudaMemcpyAsync stages before returning, so this is safe; synchronise anyway (once per create).
+    return check_cuda(c, cudaStreamSynchronize(c->stream), "sync after table upload");
+}
+
+int do_reset(sg_ctx *c)
+{
+    const Dims &d = c->d;
+    int rc;
+    if ((rc = check_cuda(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * (size_t)d.n_samples * d.NT * SG_NMOM, c->stream), "zero acc"))) return rc;
+    c->launches += c->kind == SG_PMJ ? launch_init_pmj(c) : launch_init_gauss(c);
+    c->sweeps = c->exchanges = 0;
+    c->n_meas = 0;
+    return check_launch(c, "init kernels");
+}
+
+int do_exchange(sg_ctx *c)
+{
+    if (c->kind == SG_PMJ) {
+        c->launches += launch_energy_pmj(c);
+        c->launches += launch_pt_pmj(c, c->exchanges);
+    } else {
+        c->launches += launch_energy_gauss(c);
+        c->launches += launch_pt_gauss(c, c->exchanges);
+    }
+    c->exchanges += 1;
+    return check_launch(c, "pt kernels");
+}
+
+int do_measure(sg_ctx *c, double *out)
+{
+    const Dims &d = c->d;
+    for (int s0 = 0; s0 < d.n_samples; s0 += c->chunk_samples) {
+        const int ns = std::min(c->chunk_samples, d.n_samples - s0);
+        c->launches += c->kind == SG_PMJ ? launch_hist_pmj(c, s0, ns) : launch_hist_gauss(c, s0, ns);
+        c->launches += launch_finalize(c, s0, ns, out != nullptr);
+        int rc = check_launch(c, "measure kernels");
+        if (rc) return rc;
+        if (out) {
+            const size_t per = (size_t)d.NT * d.P * SG_REC;
+            rc = check_cuda(c, cudaMemcpyAsync(out + (size_t)s0 * per, c->rec, sizeof(double) * per * ns,
+                                               cudaMemcpyDeviceToHost, c->stream), "copy records");
+            if (rc) return rc;
+            rc = check_cuda(c, cudaStreamSynchronize(c->stream), "sync records");
+            if (rc) return rc;
+        }
+    }
+    c->n_meas += 1;
+    return SG_OK;
+}
+
+int do_sweep(sg_ctx *c)
+{
+    c->launches += c->kind == SG_PMJ ? launch_sweep_pmj(c, c->sweeps) : launch_sweep_gauss(c, c->sweeps);
+    c->sweeps += 1;
+    return SG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t sg_workspace_bytes(int L, int n_samples, int n_replicas, int n_temps, int coupling_kind)
+{
+    if (!valid_args(L, n_samples, n_replicas, n_temps, coupling_kind)) return 0;
+    return make_layout(L, n_samples, n_replicas, n_temps, coupling_kind).total;
+}
+
+int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, const double *temps, int n_temps,
+              int coupling_kind, uint64_t seed, void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!out) return fail(nullptr, SG_EINVAL, "sg_create: out is NULL");
+    if (!temps) return fail(nullptr, SG_EINVAL, "sg_create: temps is NULL");
+    if (!valid_args(L, n_samples, n_replicas, n_temps, coupling_kind))
+        return fail(nullptr, SG_EINVAL, "sg_create: need even 4<=L<=64, n_samples>=1, n_replicas in {2,4}, 1<=n_temps<=64, kind in {0,1}");
+    if (!(h == h) || fabs(h) > 1e300) return fail(nullptr, SG_EINVAL, "sg_create: h must be finite");
+    for (int t = 0; t < n_temps; ++t) {
+        if (!(temps[t] > 0.0) || !(temps[t] < 1e308)) return fail(nullptr, SG_EINVAL, "sg_create: temperatures must be finite and > 0");
+        if (t && temps[t] < temps[t - 1]) return fail(nullptr, SG_EINVAL, "sg_create: temperatures must be non-decreasing");
+    }
+    const Layout lo = make_layout(L, n_samples, n_replicas, n_temps, coupling_kind);
+    if (workspace) {
+        if (((uintptr_t)workspace) % ALIGN) return fail(nullptr, SG_EINVAL, "sg_create: workspace must be 256-byte aligned");
+        if (workspace_bytes < lo.total) return fail(nullptr, SG_ENOMEM, "sg_create: workspace smaller than sg_workspace_bytes()");
+    }
+    sg_ctx *c = new (std::nothrow) sg_ctx();
+    if (!c) return fail(nullptr, SG_ENOMEM, "sg_create: host allocation failed");
+    c->kind = coupling_kind;
+    c->h = h;
+    c->seed = seed;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->temps.assign(temps, temps + n_temps);
+    c->sweeps = c->exchanges = c->launches = 0;
+    c->n_meas = 0;
+    Dims &d = c->d;
+    d.L = L; d.Lh = L / 2; d.N = L * L * L; d.H = d.N / 2;
+    d.R = n_replicas; d.NT = n_temps; d.P = n_replicas * (n_replicas - 1) / 2;
+    d.n_samples = n_samples;
+    d.W = coupling_kind == SG_PMJ ? (n_samples + 31) / 32 : n_samples;
+    d.k0 = (uint32_t)seed; d.k1 = (uint32_t)(seed >> 32);
+    d.neg_h = h < 0.0 ? 1u : 0u;
+    d.fast_accept = 0;
+    c->own_ws = workspace == nullptr;
+    c->ws_bytes = lo.total;
+    if (workspace) c->ws = workspace;
+    else {
+        cudaError_t e = cudaMalloc(&c->ws, lo.total);
+        if (e != cudaSuccess) {
+            g_create_err = std::string("sg_create: cudaMalloc: ") + cudaGetErrorString(e);
+            delete c;
+            return SG_ENOMEM;
+        }
+    }
+    char *b = (char *)c->ws;
+    c->spins = (uint32_t *)(b + lo.spins);
+    c->spins8 = (int8_t *)(b + lo.spins);
+    c->J = (uint32_t *)(b + lo.J);
+    c->Jg = (float *)(b + lo.J);
+    c->tab = (SlotTab *)(b + lo.tab);
+    c->exp64_tab = (double *)(b + lo.exp64);
+    c->exp32_tab = (float *)(b + lo.exp32);
+    c->twiddle = (double *)(b + lo.tw);
+    c->U = (int64_t *)(b + lo.U);
+    c->M = (int32_t *)(b + lo.M);
+    c->swapmask = (uint32_t *)(b + lo.swap);
+    c->acc = (double *)(b + lo.acc);
+    c->hist = (uint16_t *)(b + lo.hist);
+    c->rec = (double *)(b + lo.rec);
+    c->stage8 = (int8_t *)(b + lo.stage);
+    c->chunk_samples = lo.chunk_meas;
+    int rc = upload_tables(c);
+    if (!rc) rc = do_reset(c);
+    if (rc) {
+        g_create_err = c->err;
+        if (c->own_ws) cudaFree(c->ws);
+        delete c;
+        return rc;
+    }
+    *out = c;
+    return SG_OK;
+}
+
+int sg_reset(sg_ctx *c)
+{
+    if (!c) return SG_EINVAL;
+    return do_reset(c);
+}
+
+int sg_sweep(sg_ctx *c, int n)
+{
+    if (!c) return SG_EINVAL;
+    if (n < 0) return fail(c, SG_EINVAL, "sg_sweep: n < 0");
+    for (int k = 0; k < n; ++k) do_sweep(c);
+    return check_launch(c, "sweep kernels");
+}
+
+int sg_pt_exchange(sg_ctx *c)
+{
+    if (!c) return SG_EINVAL;
+    return do_exchange(c);
+}
+
+int sg_measure(sg_ctx *c, double *out)
+{
+    if (!c) return SG_EINVAL;
+    return do_measure(c, out);
+}
+
+int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
+{
+    if (!c) return SG_EINVAL;
+    if (n_sweeps < 0 || pt_every < 0 || meas_every < 0) return fail(c, SG_EINVAL, "sg_run: negative argument");
+    for (int k = 0; k < n_sweeps; ++k) {
+        do_sweep(c);
+        int rc;
+        if (pt_every > 0 && c->sweeps % (uint64_t)pt_every == 0)
+            if ((rc = do_exchange(c))) return rc;
+        if (meas_every > 0 && c->sweeps % (uint64_t)meas_every == 0)
+            if ((rc = do_measure(c, nullptr))) return rc;
+    }
+    return check_launch(c, "run kernels");
+}
+
+int sg_synchronize(sg_ctx *c)
+{
+    if (!c) return SG_EINVAL;
+    return check_cuda(c, cudaStreamSynchronize(c->stream), "sg_synchronize");
+}
+
+int sg_destroy(sg_ctx *c)
+{
+    if (!c) return SG_EINVAL;
+    cudaStreamSynchronize(c->stream);
+    if (c->own_ws) cudaFree(c->ws);
+    delete c;
+    return SG_OK;
+}
+
+static int spins_range(sg_ctx *c, int s0, int ns, int8_t *out, const int8_t *in)
+{
+    if (!c) return SG_EINVAL;
+    if ((!out && !in) || ns < 1 || s0 < 0 || s0 + ns > c->d.n_samples) return fail(c, SG_EINVAL, "spins range: bad range or NULL buffer");
+    const Dims &d = c->d;
+    const size_t per = (size_t)d.R * d.NT * d.N;
+    const Layout lo = make_layout(d.L, d.n_samples, d.R, d.NT, c->kind);
+    for (int a = s0; a < s0 + ns; a += lo.chunk_stage) {
+        const int n = std::min(lo.chunk_stage, s0 + ns - a);
+        int rc;
+        if (out) {
+            c->launches += c->kind == SG_PMJ ? launch_unpack_pmj(c, a, n) : launch_unpack_gauss(c, a, n);
+            if ((rc = check_launch(c, "unpack kernel"))) return rc;
+            if ((rc = check_cuda(c, cudaMemcpyAsync(out + (size_t)(a - s0) * per, c->stage8, per * n, cudaMemcpyDeviceToHost, c->stream), "copy spins"))) return rc;
+        } else {
+            if ((rc = check_cuda(c, cudaMemcpyAsync(c->stage8, in + (size_t)(a - s0) * per, per * n, cudaMemcpyHostToDevice, c->stream), "copy spins"))) return rc;
+            c->launches += c->kind == SG_PMJ ? launch_pack_pmj(c, a, n) : launch_pack_gauss(c, a, n);
+            if ((rc = check_launch(c, "pack kernel"))) return rc;
+        }
+        if ((rc = check_cuda(c, cudaStreamSynchronize(c->stream), "sync spins"))) return rc;
+    }
+    return SG_OK;
+}
+
+int sg_get_spins_range(sg_ctx *c, int s0, int ns, int8_t *out) { return out ? spins_range(c, s0, ns, out, nullptr) : SG_EINVAL; }
+int sg_set_spins_range(sg_ctx *c, int s0, int ns, const int8_t *in) { return in ? spins_range(c, s0, ns, nullptr, in) : SG_EINVAL; }
+int sg_get_spins(sg_ctx *c, int8_t *out) { return c ? sg_get_spins_range(c, 0, c->d.n_samples, out) : SG_EINVAL; }
+int sg_set_spins(sg_ctx *c, const int8_t *in) { return c ? sg_set_spins_range(c, 0, c->d.n_samples, in) : SG_EINVAL; }
+
+int sg_get_couplings_range(sg_ctx *c, int s0, int ns, float *out)
+{
+    if (!c) return SG_EINVAL;
+    if (!out || ns < 1 || s0 < 0 || s0 + ns > c->d.n_samples) return fail(c, SG_EINVAL, "couplings range: bad range or NULL buffer");
+    const Dims &d = c->d;
+    const size_t per = (size_t)3 * d.N;
+    const Layout lo = make_layout(d.L, d.n_samples, d.R, d.NT, c->kind);
+    for (int a = s0; a < s0 + ns; a += lo.chunk_stage) {
+        const int n = std::min(lo.chunk_stage, s0 + ns - a);
+        float *dev = (float *)c->stage8;
+        c->launches += c->kind == SG_PMJ ? launch_couplings_pmj(c, a, n, dev) : launch_couplings_gauss(c, a, n, dev);
+        int rc;
+        if ((rc = check_launch(c, "couplings kernel"))) return rc;
+        if ((rc = check_cuda(c, cudaMemcpyAsync(out + (size_t)(a - s0) * per, dev, sizeof(float) * per * n, cudaMemcpyDeviceToHost, c->stream), "copy couplings"))) return rc;
+        if ((rc = check_cuda(c, cudaStreamSynchronize(c->stream), "sync couplings"))) return rc;
+    }
+    return SG_OK;
+}
+
+int sg_get_couplings(sg_ctx *c, float *out) { return c ? sg_get_couplings_range(c, 0, c->d.n_samples, out) : SG_EINVAL; }
+
+int sg_get_energies(sg_ctx *c, int64_t *U, int32_t *M)
+{
+    if (!c) return SG_EINVAL;
+    c->launches += c->kind == SG_PMJ ? launch_energy_pmj(c) : launch_energy_gauss(c);
+    int rc;
+    if ((rc = check_launch(c, "energy kernel"))) return rc;
+    const size_t n = (size_t)c->d.n_samples * c->d.R * c->d.NT;
+    if (U && (rc = check_cuda(c, cudaMemcpyAsync(U, c->U, sizeof(int64_t) * n, cudaMemcpyDeviceToHost, c->stream), "copy U"))) return rc;
+    if (M && (rc = check_cuda(c, cudaMemcpyAsync(M, c->M, sizeof(int32_t) * n, cudaMemcpyDeviceToHost, c->stream), "copy M"))) return rc;
+    return check_cuda(c, cudaStreamSynchronize(c->stream), "sync energies");
+}
+
+int sg_get_thresholds(sg_ctx *c, uint64_t *out)
+{
+    if (!c || !out) return SG_EINVAL;
+    memcpy(out, c->thr.data(), sizeof(uint64_t) * c->thr.size());
+    return SG_OK;
+}
+
+int sg_get_moments(sg_ctx *c, double *out, int64_t *n_meas)
+{
+    if (!c) return SG_EINVAL;
+    if (out) {
+        const size_t n = (size_t)c->d.n_samples * c->d.NT * SG_NMOM;
+        int rc;
+        if ((rc = check_cuda(c, cudaMemcpyAsync(out, c->acc, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream), "copy moments"))) return rc;
+        if ((rc = check_cuda(c, cudaStreamSynchronize(c->stream), "sync moments"))) return rc;
+    }
+    if (n_meas) *n_meas = c->n_meas;
+    return SG_OK;
+}
+
+int sg_get_counters(sg_ctx *c, uint64_t *sweeps_done, uint64_t *exchanges_done)
+{
+    if (!c) return SG_EINVAL;
+    if (sweeps_done) *sweeps_done = c->sweeps;
+    if (exchanges_done) *exchanges_done = c->exchanges;
+    return SG_OK;
+}
+
+int sg_get_launch_count(sg_ctx *c, uint64_t *launches)
+{
+    if (!c || !launches) return SG_EINVAL;
+    *launches = c->launches;
+    return SG_OK;
+}
+
+const char *sg_last_error(sg_ctx *c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,94 @@
+// sg_internal.h — host-side context and kernel-launcher declarations of libsg_b200 (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/sg.h"
+
+namespace sg {
+
+constexpr int MAX_NT = 64;
+constexpr int N_HIST = 9;   // plane histograms per (sample, slot, pair): x, y, z, x+y, x-y, x+z, x-z, y+z, y-z
+
+// Geometry and keys handed to kernels by value.
+struct Dims {
+    int L, Lh, N, H;          // L, L/2, L^3, N/2 (sites per colour)
+    int R, NT, P;             // replicas, temperature slots, replica pairs
+    int W;                    // packed words (PMJ) — ceil(n_samples/32); for GAUSS: n_samples
+    int n_samples;
+    uint32_t k0, k1;          // Philox key = (seed lo, seed hi)
+    uint32_t neg_h;           // 1 if h < 0 (field alignment a = ~s)
+    int fast_accept;          // |h| <= 1 and threshold table monotone: comparator path
+};
+
+// Per-slot device tables (one struct array in the workspace).
+struct SlotTab {
+    // PMJ fast path: c64[c] = (uint64)(0 - thr(code c)), code c = 2 n_u + (1 - a), c = 0..6
+    uint2 c64[7];
+    uint2 pad;
+    // general path: c64g[n_u][a]
+    uint2 c64g[7][2];
+    double beta;
+    float beta_f;
+    float pad2;
+};
+
+}  // namespace sg
+
+struct sg_ctx {
+    sg::Dims d;
+    int kind;
+    double h;
+    uint64_t seed;
+    cudaStream_t stream;
+    std::vector<double> temps, beta;
+    std::vector<uint64_t> thr;          // [NT][7][2]
+    std::string err;
+    uint64_t sweeps, exchanges, launches;
+    int64_t n_meas;
+    // device memory
+    void *ws;                           // base of the workspace
+    size_t ws_bytes;
+    bool own_ws;
+    uint32_t *spins;                    // PMJ: [W][R][NT][2][H] colour-compacted words
+    uint32_t *J;                        // PMJ: [W][2][3][H]
+    int8_t *spins8;                     // GAUSS: [S][R][NT][2][H] colour-compacted bytes
+    float *Jg;                          // GAUSS: [S][2][3][H]
+    sg::SlotTab *tab;                   // [NT]
+    double *exp64_tab;                  // [5761]
+    float *exp32_tab;                   // [1441]
+    double *twiddle;                    // [2][L] cos, sin (2 pi m / L)
+    int64_t *U;                         // [S_pad][R][NT]  (S_pad = 32 W for PMJ)
+    int32_t *M;                         // [S_pad][R][NT]
+    uint32_t *swapmask;                 // PMJ: [W][R][NT/2]; GAUSS: [S][R][NT/2] (0/1)
+    double *acc;                        // [n_samples][NT][SG_NMOM]
+    uint16_t *hist;                     // scratch [chunk samples][NT][P][N_HIST][L]
+    double *rec;                        // scratch [chunk samples][NT][P][SG_REC]
+    int chunk_samples;                  // samples per measurement chunk (multiple of 32)
+    int8_t *stage8;                     // staging for get/set spins: [chunk][R][NT][N] bytes
+};
+
+namespace sg {
+
+// ---- launchers (each returns the number of kernels it launched; errors via cudaGetLastError) ----
+int launch_init_pmj(sg_ctx *c);
+int launch_init_gauss(sg_ctx *c);
+int launch_sweep_pmj(sg_ctx *c, uint64_t sweep);            // both colours
+int launch_sweep_gauss(sg_ctx *c, uint64_t sweep);
+int launch_energy_pmj(sg_ctx *c);
+int launch_energy_gauss(sg_ctx *c);
+int launch_pt_pmj(sg_ctx *c, uint64_t exchange);            // decide + swap (energies must be fresh)
+int launch_pt_gauss(sg_ctx *c, uint64_t exchange);
+int launch_hist_pmj(sg_ctx *c, int s0, int ns);             // samples [s0, s0+ns) -> c->hist
+int launch_hist_gauss(sg_ctx *c, int s0, int ns);
+int launch_finalize(sg_ctx *c, int s0, int ns, bool want_rec);   // hist -> rec (optional), acc
+int launch_unpack_pmj(sg_ctx *c, int s0, int ns);           // spins -> stage8 (canonical bytes)
+int launch_pack_pmj(sg_ctx *c, int s0, int ns);             // stage8 -> spins (lanes of [s0, s0+ns))
+int launch_unpack_gauss(sg_ctx *c, int s0, int ns);
+int launch_pack_gauss(sg_ctx *c, int s0, int ns);
+int launch_couplings_pmj(sg_ctx *c, int s0, int ns, float *dev_out);   // -> [ns][3][N] float
+int launch_couplings_gauss(sg_ctx *c, int s0, int ns, float *dev_out);
+
+}  // namespace sg

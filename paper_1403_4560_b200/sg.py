@@ -1,0 +1,200 @@
+"""ctypes binding of libsg_b200 (include/sg.h): same names, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of paper_1403_4560_b200/csrc; PyTorch supplies the
+device workspace tensor and the CUDA stream.  There is no CPU fallback: if the library has not been
+built (python -m paper_1403_4560_b200.build or __graft_entry__.build()) the import raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+PMJ, GAUSS = 0, 1
+NK, REC, NMOM = 12, 25, 66
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ESTATE = 0, -1, -2, -3, -4, -5
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "csrc", "libsg_b200.so")
+
+EXPORTS = {
+    # name: (restype, argtypes)
+    "sg_workspace_bytes": (C.c_size_t, [C.c_int] * 5),
+    "sg_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_int,
+                            C.c_int, C.c_uint64, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "sg_reset": (C.c_int, [C.c_void_p]),
+    "sg_sweep": (C.c_int, [C.c_void_p, C.c_int]),
+    "sg_pt_exchange": (C.c_int, [C.c_void_p]),
+    "sg_measure": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "sg_run": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
+    "sg_synchronize": (C.c_int, [C.c_void_p]),
+    "sg_destroy": (C.c_int, [C.c_void_p]),
+    "sg_get_spins": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "sg_set_spins": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "sg_get_couplings": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "sg_get_spins_range": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
+    "sg_set_spins_range": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
+    "sg_get_couplings_range": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_void_p]),
+    "sg_get_energies": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "sg_get_thresholds": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "sg_get_moments": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "sg_get_counters": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "sg_get_launch_count": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "sg_last_error": (C.c_char_p, [C.c_void_p]),
+}
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError("libsg_b200.so is not built (%s); run `python -m paper_1403_4560_b200.build` — "
+                      "there is no CPU fallback" % LIB_PATH)
+_lib = C.CDLL(LIB_PATH)
+for _name, (_res, _args) in EXPORTS.items():
+    _fn = getattr(_lib, _name)
+    _fn.restype = _res
+    _fn.argtypes = _args
+
+
+class SgError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libsg_b200 error %d: %s" % (code, msg))
+        self.code = code
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def sg_workspace_bytes(L, n_samples, n_replicas, n_temps, coupling_kind):
+    return int(_lib.sg_workspace_bytes(L, n_samples, n_replicas, n_temps, coupling_kind))
+
+
+class Simulation:
+    """One sg_ctx.  `workspace`: a torch CUDA uint8 tensor (allocated here with torch if None);
+    `stream`: a torch.cuda.Stream (current stream if None)."""
+
+    def __init__(self, L, h, n_samples, n_replicas, temps, coupling_kind=PMJ, seed=1, workspace=None,
+                 stream=None, device=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("libsg_b200 needs a CUDA device; there is no CPU fallback")
+        self.L, self.N = int(L), int(L) ** 3
+        self.h = float(h)
+        self.n_samples, self.R = int(n_samples), int(n_replicas)
+        self.temps = np.ascontiguousarray(temps, dtype=np.float64)
+        self.NT = int(self.temps.size)
+        self.kind = int(coupling_kind)
+        self.n_pairs = self.R * (self.R - 1) // 2
+        self._h = C.c_void_p()
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        need = sg_workspace_bytes(self.L, self.n_samples, self.R, self.NT, self.kind)
+        if need == 0:
+            raise SgError(EINVAL, "invalid parameters (sg_workspace_bytes returned 0)")
+        with torch.cuda.device(self.device):
+            if workspace is None:
+                workspace = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+            self.workspace = workspace
+            ptr = workspace.data_ptr()
+            aligned = (ptr + 255) // 256 * 256
+            avail = workspace.numel() - (aligned - ptr)
+            self.stream = torch.cuda.current_stream(self.device) if stream is None else stream
+            rc = _lib.sg_create(C.byref(self._h), self.L, self.h, self.n_samples, self.R, _p(self.temps), self.NT,
+                                self.kind, int(seed), C.c_void_p(aligned), avail, C.c_void_p(self.stream.cuda_stream))
+        if rc != OK:
+            self._h = C.c_void_p()
+            raise SgError(rc, (_lib.sg_last_error(None) or b"").decode())
+
+    # -- helpers
+    def _check(self, rc):
+        if rc != OK:
+            raise SgError(rc, (_lib.sg_last_error(self._h) or b"").decode())
+
+    def close(self):
+        if self._h:
+            _lib.sg_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the path
+    def sg_reset(self):
+        self._check(_lib.sg_reset(self._h))
+
+    def sg_sweep(self, n=1):
+        self._check(_lib.sg_sweep(self._h, int(n)))
+
+    def sg_pt_exchange(self):
+        self._check(_lib.sg_pt_exchange(self._h))
+
+    def sg_measure(self, want=True):
+        if not want:
+            self._check(_lib.sg_measure(self._h, None))
+            return None
+        out = np.empty((self.n_samples, self.NT, self.n_pairs, REC), dtype=np.float64)
+        self._check(_lib.sg_measure(self._h, _p(out)))
+        return out
+
+    def sg_run(self, n_sweeps, pt_every=0, meas_every=0):
+        self._check(_lib.sg_run(self._h, int(n_sweeps), int(pt_every), int(meas_every)))
+
+    def sg_synchronize(self):
+        self._check(_lib.sg_synchronize(self._h))
+
+    # -- introspection
+    def sg_get_spins(self, s0=None, ns=None):
+        if s0 is None:
+            s0, ns = 0, self.n_samples
+        out = np.empty((ns, self.R, self.NT, self.N), dtype=np.int8)
+        self._check(_lib.sg_get_spins_range(self._h, int(s0), int(ns), _p(out)))
+        return out
+
+    def sg_set_spins(self, spins, s0=0):
+        spins = np.ascontiguousarray(spins, dtype=np.int8)
+        ns = spins.size // (self.R * self.NT * self.N)
+        self._check(_lib.sg_set_spins_range(self._h, int(s0), int(ns), _p(spins)))
+
+    def sg_get_couplings(self, s0=None, ns=None):
+        if s0 is None:
+            s0, ns = 0, self.n_samples
+        out = np.empty((ns, 3, self.N), dtype=np.float32)
+        self._check(_lib.sg_get_couplings_range(self._h, int(s0), int(ns), _p(out)))
+        return out
+
+    def sg_get_energies(self):
+        U = np.empty((self.n_samples, self.R, self.NT), dtype=np.int64)
+        M = np.empty((self.n_samples, self.R, self.NT), dtype=np.int32)
+        self._check(_lib.sg_get_energies(self._h, _p(U), _p(M)))
+        return U, M
+
+    def sg_get_thresholds(self):
+        out = np.empty((self.NT, 7, 2), dtype=np.uint64)
+        self._check(_lib.sg_get_thresholds(self._h, _p(out)))
+        return out
+
+    def sg_get_moments(self, want=True):
+        n = C.c_int64()
+        out = None
+        if want:
+            out = np.empty((self.n_samples, self.NT, NMOM), dtype=np.float64)
+            self._check(_lib.sg_get_moments(self._h, _p(out), C.byref(n)))
+        else:
+            self._check(_lib.sg_get_moments(self._h, None, C.byref(n)))
+        return out, n.value
+
+    def sg_get_moments_into(self, out):
+        """Fill a caller-owned (e.g. pinned) host buffer; returns n_meas."""
+        n = C.c_int64()
+        self._check(_lib.sg_get_moments(self._h, C.c_void_p(out.ctypes.data if hasattr(out, "ctypes") else out.data_ptr()),
+                                        C.byref(n)))
+        return n.value
+
+    def sg_get_counters(self):
+        a, b = C.c_uint64(), C.c_uint64()
+        self._check(_lib.sg_get_counters(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def sg_get_launch_count(self):
+        a = C.c_uint64()
+        self._check(_lib.sg_get_launch_count(self._h, C.byref(a)))
+        return a.value

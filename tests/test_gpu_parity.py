@@ -1,0 +1,211 @@
+"""GPU parity: libsg_b200 (through its C-ABI binding) vs the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): spins, couplings, thresholds, energies bit-exact on every config
+(+-J and Gaussian); overlaps / moments within 1e-12 * max(|value|, 1).
+Sizes here are ones the oracle finishes in seconds; the full-size cases are in
+test_gpu_fullsize.py.
+"""
+import numpy as np
+import pytest
+
+from paper_1403_4560_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sg():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1403_4560_b200 import sg as _sg
+    return _sg
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import ea_oracle
+    return ea_oracle
+
+
+def close(a, b, tol=1e-12):
+    a = np.asarray(a)
+    b = np.asarray(b)
+    return np.all(np.abs(a - b) <= tol * np.maximum(np.abs(b), 1.0))
+
+
+def make_pair(sg, O, L, h, n_samples, R, temps, kind, seed, samples):
+    sim = sg.Simulation(L, h, n_samples, R, temps, kind, seed)
+    orc = {s: O.Oracle(L, h, R, temps, kind=kind, seed=seed, sample=s) for s in samples}
+    return sim, orc
+
+
+def check_state(sim, orc, what=""):
+    U, M = sim.sg_get_energies()
+    for s, o in orc.items():
+        got = sim.sg_get_spins(s, 1)[0]
+        want = o.spins()
+        assert np.array_equal(got, want), "%s spins differ, sample %d: %d sites" % (what, s, int((got != want).sum()))
+        Uo, Mo = o.energies()
+        assert np.array_equal(U[s], Uo), "%s U differs, sample %d" % (what, s)
+        assert np.array_equal(M[s], Mo), "%s M differs, sample %d" % (what, s)
+
+
+CASES = [
+    # name, L, h, n_samples, R, NT, T range, kind, seed, samples to check
+    ("C1", 4, 0.3, 1, 4, 8, (0.5, 2.0), 0, 1, [0]),
+    ("L4-two-words", 4, 0.3, 40, 4, 5, (0.5, 2.0), 0, 11, [0, 5, 31, 32, 39]),
+    ("L6-ragged-quads", 6, 0.2, 33, 2, 4, (0.5, 2.0), 0, 12, [0, 17, 32]),
+    ("L8", 8, 0.2, 64, 4, 6, (0.5, 2.0), 0, 2, [0, 13, 31, 63]),
+    ("L12", 12, 0.1, 32, 4, 3, (0.4, 1.8), 0, 3, [0, 31]),
+    ("L8-neg-h", 8, -0.7, 32, 2, 4, (0.6, 1.5), 0, 4, [3, 30]),
+    ("L4-h0", 4, 0.0, 32, 2, 4, (0.5, 2.0), 0, 5, [1, 2]),
+    ("L4-big-h-general-path", 4, 1.7, 32, 2, 4, (0.5, 3.0), 0, 6, [7, 8]),
+    ("L4-huge-h", 4, 5.0, 32, 2, 3, (0.5, 3.0), 0, 7, [0, 9]),
+    ("G-L4", 4, 0.3, 5, 4, 6, (0.2, 1.5), 1, 4, [0, 2, 4]),
+    ("G-L6", 6, -0.3, 3, 2, 4, (0.3, 1.5), 1, 8, [0, 2]),
+    ("G-L8", 8, 0.3, 4, 4, 4, (0.2, 1.5), 1, 9, [1, 3]),
+]
+
+
+@pytest.mark.parametrize("case", CASES, ids=[c[0] for c in CASES])
+def test_initial_state_tables_and_couplings(sg, O, case):
+    _, L, h, ns, R, NT, (Tlo, Thi), kind, seed, samples = case
+    temps = W.ladder(Tlo, Thi, NT)
+    sim, orc = make_pair(sg, O, L, h, ns, R, temps, kind, seed, samples)
+    assert np.array_equal(sim.sg_get_thresholds(), next(iter(orc.values())).thresholds())
+    for s, o in orc.items():
+        Jg = sim.sg_get_couplings(s, 1)[0]
+        Jo = o.couplings()
+        assert np.array_equal(Jg.view(np.uint32), Jo.view(np.uint32)), "couplings differ (bitwise), sample %d" % s
+    check_state(sim, orc, "initial")
+    assert sim.sg_get_counters() == (0, 0)
+    sim.close()
+
+
+@pytest.mark.parametrize("case", CASES, ids=[c[0] for c in CASES])
+def test_sweeps_pt_measure_bit_exact(sg, O, case):
+    _, L, h, ns, R, NT, (Tlo, Thi), kind, seed, samples = case
+    temps = W.ladder(Tlo, Thi, NT)
+    sim, orc = make_pair(sg, O, L, h, ns, R, temps, kind, seed, samples)
+    n_meas = 0
+    for step in range(12):
+        sim.sg_sweep(1)
+        for o in orc.values():
+            o.sweep(1)
+        if step in (0, 5, 11):
+            check_state(sim, orc, "after sweep %d" % step)
+        sim.sg_pt_exchange()
+        for o in orc.values():
+            o.pt_exchange()
+        if step in (0, 1, 6, 11):
+            check_state(sim, orc, "after exchange %d" % step)
+        if step % 4 == 3:
+            rec = sim.sg_measure()
+            n_meas += 1
+            for s, o in orc.items():
+                want = o.measure()
+                assert close(rec[s], want), "records differ, sample %d: %g" % (s, np.abs(rec[s] - want).max())
+    mom, n = sim.sg_get_moments()
+    assert n == n_meas
+    for s, o in orc.items():
+        want, no = o.moments()
+        assert no == n_meas
+        assert close(mom[s], want), "moments differ, sample %d: %g" % (s, np.abs(mom[s] - want).max())
+    assert sim.sg_get_counters() == (12, 12)
+    sim.close()
+
+
+@pytest.mark.parametrize("case", [CASES[0], CASES[3], CASES[9]], ids=["C1", "L8", "G-L4"])
+def test_run_equals_primitive_sequence_and_oracle(sg, O, case):
+    _, L, h, ns, R, NT, (Tlo, Thi), kind, seed, samples = case
+    temps = W.ladder(Tlo, Thi, NT)
+    sim, orc = make_pair(sg, O, L, h, ns, R, temps, kind, seed, samples)
+    sim2 = sg.Simulation(L, h, ns, R, temps, kind, seed)
+    sim.sg_run(40, 2, 10)
+    for k in range(1, 41):
+        sim2.sg_sweep(1)
+        if k % 2 == 0:
+            sim2.sg_pt_exchange()
+        if k % 10 == 0:
+            sim2.sg_measure(False)
+    assert np.array_equal(sim.sg_get_spins(), sim2.sg_get_spins())
+    m1, n1 = sim.sg_get_moments()
+    m2, n2 = sim2.sg_get_moments()
+    assert n1 == n2 == 4 and np.array_equal(m1, m2)
+    for o in orc.values():
+        o.run(40, 2, 10)
+    check_state(sim, orc, "after run")
+    for s, o in orc.items():
+        assert close(m1[s], o.moments()[0])
+    # reset returns to the initial state
+    sim.sg_reset()
+    fresh = {s: O.Oracle(L, h, R, temps, kind=kind, seed=seed, sample=s) for s in samples}
+    check_state(sim, fresh, "after reset")
+    assert sim.sg_get_moments()[1] == 0 and not sim.sg_get_moments()[0].any()
+    sim.close(); sim2.close()
+
+
+def test_c1_full_config(sg, O):
+    """BASELINE.json config 1 exactly: 1000 sweeps, PT every sweep, measure every 10."""
+    w = W.BY_NAME["C1"]
+    sim, orc = make_pair(sg, O, w.L, w.h, w.n_samples, w.n_replicas, w.temps(), w.kind, w.seed, [0])
+    sim.sg_run(w.n_sweeps, w.pt_every, w.meas_every)
+    orc[0].run(w.n_sweeps, w.pt_every, w.meas_every)
+    check_state(sim, orc, "C1 end")
+    mom, n = sim.sg_get_moments()
+    want, no = orc[0].moments()
+    assert n == no == 100
+    assert close(mom[0], want)
+    sim.close()
+
+
+def test_set_spins_roundtrip_and_closed_forms(sg):
+    """set/get round trip; identical replicas -> q(0)=1, q(k)=0; stripe closed form."""
+    import math
+    L, R, NT, ns = 8, 2, 2, 35
+    N = L**3
+    sim = sg.Simulation(L, 0.0, ns, R, [1.0, 2.0], 0, 3)
+    rng = np.random.default_rng(0)
+    S = rng.choice([-1, 1], size=(ns, R, NT, N)).astype(np.int8)
+    sim.sg_set_spins(S)
+    assert np.array_equal(sim.sg_get_spins(), S)
+    sub = rng.choice([-1, 1], size=(3, R, NT, N)).astype(np.int8)
+    sim.sg_set_spins(sub, s0=30)
+    S[30:33] = sub
+    assert np.array_equal(sim.sg_get_spins(), S)
+    x = np.arange(N) % L
+    S[:, 1] = S[:, 0]
+    S[5, 0] = 1
+    S[5, 1] = np.where(x < L // 2, 1, -1)
+    S[6, 1] = -S[6, 0]
+    sim.sg_set_spins(S)
+    rec = sim.sg_measure()
+    assert np.all(rec[0, :, 0, 0] == 1.0) and np.all(np.abs(rec[0, :, 0, 1:]) < 1e-15)
+    assert np.all(rec[6, :, 0, 0] == -1.0)
+    assert abs(rec[5, 0, 0, 1] - 2.0 / L) < 1e-14 and abs(rec[5, 0, 0, 2] - 2.0 / L / math.tan(math.pi / L)) < 1e-14
+    assert np.all(np.abs(rec[5, 0, 0, 3:]) < 1e-14) and abs(rec[5, 0, 0, 0]) < 1e-15
+    sim.close()
+
+
+def test_error_paths(sg):
+    with pytest.raises(sg.SgError) as e:
+        sg.Simulation(5, 0.1, 4, 4, [1.0])
+    assert e.value.code == sg.EINVAL
+    with pytest.raises(sg.SgError):
+        sg.Simulation(4, 0.1, 4, 3, [1.0])
+    with pytest.raises(sg.SgError):
+        sg.Simulation(4, 0.1, 4, 4, [2.0, 1.0])
+    with pytest.raises(sg.SgError):
+        sg.Simulation(4, 0.1, 4, 4, [0.0, 1.0])
+    import torch
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(sg.SgError) as e:
+        sg.Simulation(4, 0.1, 4, 4, [1.0], workspace=small)
+    assert e.value.code == sg.ENOMEM
+    sim = sg.Simulation(4, 0.1, 4, 4, [1.0])
+    with pytest.raises(sg.SgError):
+        sim.sg_run(-1, 0, 0)
+    with pytest.raises(sg.SgError):
+        sim.sg_get_spins(3, 5)
+    sim.close()
