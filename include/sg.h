@@ -74,6 +74,12 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
               int n_temps, int coupling_kind, uint64_t seed, void *workspace, size_t workspace_bytes,
               void *cuda_stream);
 
+/* Multi-GPU sharding: declare that local sample 0 is global sample `first_sample`
+ * of a larger disorder pool, so that every Philox stream is keyed by the GLOBAL sample / word index
+ * and results do not depend on how the pool is split over GPUs.  first_sample >= 0, a multiple of
+ * 32 for SG_PMJ.  Takes effect at the next sg_reset (call both right after sg_create). */
+int sg_set_first_sample(sg_ctx *ctx, int64_t first_sample);
+
 /* Regenerate couplings and initial spins from the seed, zero the counters and the accumulators:
  * the state right after sg_create, without reallocating.  Asynchronous. */
 int sg_reset(sg_ctx *ctx);

@@ -253,6 +253,7 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     d.k0 = (uint32_t)seed; d.k1 = (uint32_t)(seed >> 32);
     d.neg_h = h < 0.0 ? 1u : 0u;
     d.fast_accept = 0;
+    d.s_first = 0;
     c->own_ws = workspace == nullptr;
     c->ws_bytes = lo.total;
     if (workspace) c->ws = workspace;
@@ -290,6 +291,15 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
         return rc;
     }
     *out = c;
+    return SG_OK;
+}
+
+int sg_set_first_sample(sg_ctx *c, int64_t first_sample)
+{
+    if (!c) return SG_EINVAL;
+    if (first_sample < 0 || first_sample > 0x7fffffff - c->d.n_samples - 32 || (c->kind == SG_PMJ && (first_sample & 31)))
+        return fail(c, SG_EINVAL, "sg_set_first_sample: need 0 <= first_sample < 2^31, a multiple of 32 for SG_PMJ");
+    c->d.s_first = (int)first_sample;
     return SG_OK;
 }
 

@@ -51,7 +51,7 @@ __global__ void k_init_J_gauss(Dims d, float *__restrict__ Jg)
     const int s = (int)(tid / d.N);
     int c, n;
     site_to_compact_g(d, i, c, n);
-    const uint4 o = philox4x32_10((uint32_t)i, 0u, (uint32_t)s, ctr3(1, 0, 0), d.k0, d.k1);
+    const uint4 o = philox4x32_10((uint32_t)i, 0u, (uint32_t)(s + d.s_first), ctr3(1, 0, 0), d.k0, d.k1);
     const double u0 = __dmul_rn(__dadd_rn((double)o.x, 0.5), 0x1p-32);
     const double u1 = __dmul_rn(__dadd_rn((double)o.y, 0.5), 0x1p-32);
     const double u2 = __dmul_rn(__dadd_rn((double)o.z, 0.5), 0x1p-32);
@@ -77,7 +77,7 @@ __global__ void k_init_S_gauss(Dims d, int8_t *__restrict__ spins)
     const int t = (int)(sys % d.NT), a = (int)((sys / d.NT) % d.R), s = (int)(sys / (d.NT * d.R));
     int c, n;
     site_to_compact_g(d, i, c, n);
-    const uint4 o = philox4x32_10((uint32_t)i, 0u, (uint32_t)s, ctr3(2, a, t), d.k0, d.k1);
+    const uint4 o = philox4x32_10((uint32_t)i, 0u, (uint32_t)(s + d.s_first), ctr3(2, a, t), d.k0, d.k1);
     spins[((size_t)sys * 2 + c) * d.H + n] = (o.x & 1u) ? 1 : -1;
 }
 
@@ -102,7 +102,7 @@ k_sweep_gauss(Dims d, int8_t *__restrict__ spins, const float *__restrict__ Jg,
     const float beta_f = tab[t].beta_f;
 
     char4 sv = *reinterpret_cast<char4 *>(act + 4 * q);
-    const uint4 r4 = philox4x32_10((uint32_t)q, 2u * sweep + (uint32_t)colour, (uint32_t)s, ctr3(3, a, t), d.k0, d.k1);
+    const uint4 r4 = philox4x32_10((uint32_t)q, 2u * sweep + (uint32_t)colour, (uint32_t)(s + d.s_first), ctr3(3, a, t), d.k0, d.k1);
     signed char sp[4] = {sv.x, sv.y, sv.z, sv.w};
     const uint32_t r[4] = {r4.x, r4.y, r4.z, r4.w};
 #pragma unroll
@@ -187,7 +187,7 @@ k_pt_decide_gauss(Dims d, const int64_t *__restrict__ U, const int32_t *__restri
     const double Et = __dsub_rn(__dmul_rn((double)U[o], 0x1p-32), __dmul_rn(h, (double)M[o]));
     const double Eu = __dsub_rn(__dmul_rn((double)U[o + 1], 0x1p-32), __dmul_rn(h, (double)M[o + 1]));
     const double x = __dmul_rn(__dsub_rn(tab[t].beta, tab[t + 1].beta), __dsub_rn(Et, Eu));
-    const uint4 r = philox4x32_10(0u, exchange, (uint32_t)s, ctr3(4, a, t), d.k0, d.k1);
+    const uint4 r = philox4x32_10(0u, exchange, (uint32_t)(s + d.s_first), ctr3(4, a, t), d.k0, d.k1);
     const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(exp_tab, -x));
     swapmask[((size_t)s * d.R + a) * (d.NT / 2) + pair] = accept ? 1u : 0u;
 }

@@ -18,6 +18,7 @@ struct Dims {
     int R, NT, P;             // replicas, temperature slots, replica pairs
     int W;                    // packed words (PMJ) — ceil(n_samples/32); for GAUSS: n_samples
     int n_samples;
+    int s_first;              // global index of local sample 0 (multi-GPU sharding; multiple of 32 for PMJ)
     uint32_t k0, k1;          // Philox key = (seed lo, seed hi)
     uint32_t neg_h;           // 1 if h < 0 (field alignment a = ~s)
     int fast_accept;          // |h| <= 1 and threshold table monotone: comparator path

@@ -121,7 +121,7 @@ __global__ void k_init_J_pmj(Dims d, uint32_t *__restrict__ J)
     const int w = (int)(tid / d.N);
     int c, n;
     site_to_compact(d, i, c, n);
-    const uint4 o = philox4x32_10((uint32_t)i, 0u, (uint32_t)w, ctr3(1, 0, 0), d.k0, d.k1);
+    const uint4 o = philox4x32_10((uint32_t)i, 0u, (uint32_t)(w + (d.s_first >> 5)), ctr3(1, 0, 0), d.k0, d.k1);
     uint32_t *base = J + ((size_t)(w * 2 + c) * 3) * d.H + n;
     base[0] = o.x;
     base[d.H] = o.y;
@@ -138,7 +138,7 @@ __global__ void k_init_S_pmj(Dims d, uint32_t *__restrict__ spins)
     const int t = sys % d.NT, a = (sys / d.NT) % d.R, w = sys / (d.NT * d.R);
     int c, n;
     site_to_compact(d, i, c, n);
-    const uint4 o = philox4x32_10((uint32_t)i, 0u, (uint32_t)w, ctr3(2, a, t), d.k0, d.k1);
+    const uint4 o = philox4x32_10((uint32_t)i, 0u, (uint32_t)(w + (d.s_first >> 5)), ctr3(2, a, t), d.k0, d.k1);
     spins[((size_t)sys * 2 + c) * d.H + n] = o.x;
 }
 
@@ -160,7 +160,7 @@ k_sweep_pmj(Dims d, uint32_t *__restrict__ spins, const uint32_t *__restrict__ J
     const uint32_t *Joth = J + ((size_t)(w * 2 + 1 - colour) * 3) * d.H;
 
     uint4 s4 = *reinterpret_cast<uint4 *>(act + 4 * q);
-    const uint4 r4 = philox4x32_10((uint32_t)q, 2u * sweep + (uint32_t)colour, (uint32_t)w, ctr3(3, a, t), d.k0, d.k1);
+    const uint4 r4 = philox4x32_10((uint32_t)q, 2u * sweep + (uint32_t)colour, (uint32_t)(w + (d.s_first >> 5)), ctr3(3, a, t), d.k0, d.k1);
     uint32_t s[4] = {s4.x, s4.y, s4.z, s4.w};
     const uint32_t r[4] = {r4.x, r4.y, r4.z, r4.w};
     const SlotTab &tb = tab[t];
@@ -254,7 +254,7 @@ k_pt_decide_pmj(Dims d, const int64_t *__restrict__ U, const int32_t *__restrict
     const double Et = __dsub_rn((double)(2 * U[o] - 3 * (int64_t)d.N), __dmul_rn(h, (double)M[o]));
     const double Eu = __dsub_rn((double)(2 * U[o + 1] - 3 * (int64_t)d.N), __dmul_rn(h, (double)M[o + 1]));
     const double x = __dmul_rn(__dsub_rn(tab[t].beta, tab[t + 1].beta), __dsub_rn(Et, Eu));
-    const uint4 r = philox4x32_10(0u, exchange, (uint32_t)s, ctr3(4, a, t), d.k0, d.k1);
+    const uint4 r = philox4x32_10(0u, exchange, (uint32_t)(s + d.s_first), ctr3(4, a, t), d.k0, d.k1);
     const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(exp_tab, -x));
     const uint32_t mask = __ballot_sync(0xffffffffu, accept && s < d.n_samples);
     if (lane == 0) swapmask[(size_t)(w * d.R + a) * (d.NT / 2) + pair] = mask;

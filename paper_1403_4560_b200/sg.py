@@ -21,6 +21,7 @@ EXPORTS = {
     "sg_workspace_bytes": (C.c_size_t, [C.c_int] * 5),
     "sg_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_int,
                             C.c_int, C.c_uint64, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "sg_set_first_sample": (C.c_int, [C.c_void_p, C.c_int64]),
     "sg_reset": (C.c_int, [C.c_void_p]),
     "sg_sweep": (C.c_int, [C.c_void_p, C.c_int]),
     "sg_pt_exchange": (C.c_int, [C.c_void_p]),
@@ -118,6 +119,9 @@ class Simulation:
             pass
 
     # -- the path
+    def sg_set_first_sample(self, first_sample):
+        self._check(_lib.sg_set_first_sample(self._h, int(first_sample)))
+
     def sg_reset(self):
         self._check(_lib.sg_reset(self._h))
 
