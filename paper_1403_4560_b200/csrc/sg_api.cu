@@ -202,10 +202,21 @@ int do_measure(sg_ctx *c, double *out)
     return SG_OK;
 }
 
-int do_sweep(sg_ctx *c)
+// n consecutive sweeps with nothing in between
+int do_sweeps(sg_ctx *c, int n)
 {
-    c->launches += c->kind == SG_PMJ ? launch_sweep_pmj(c, c->sweeps) : launch_sweep_gauss(c, c->sweeps);
-    c->sweeps += 1;
+    if (n <= 0) return SG_OK;
+    if (ladder_supported(c)) {
+        const int k = launch_ladder_pmj(c, c->sweeps, n);
+        if (k < 0) return check_launch(c, "ladder kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "ladder kernel launch failed");
+        c->launches += k;
+        c->sweeps += n;
+        return SG_OK;
+    }
+    for (int i = 0; i < n; ++i) {
+        c->launches += c->kind == SG_PMJ ? launch_sweep_pmj(c, c->sweeps) : launch_sweep_gauss(c, c->sweeps);
+        c->sweeps += 1;
+    }
     return SG_OK;
 }
 
@@ -313,7 +324,8 @@ int sg_sweep(sg_ctx *c, int n)
 {
     if (!c) return SG_EINVAL;
     if (n < 0) return fail(c, SG_EINVAL, "sg_sweep: n < 0");
-    for (int k = 0; k < n; ++k) do_sweep(c);
+    int rc = do_sweeps(c, n);
+    if (rc) return rc;
     return check_launch(c, "sweep kernels");
 }
 
@@ -333,9 +345,15 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
 {
     if (!c) return SG_EINVAL;
     if (n_sweeps < 0 || pt_every < 0 || meas_every < 0) return fail(c, SG_EINVAL, "sg_run: negative argument");
-    for (int k = 0; k < n_sweeps; ++k) {
-        do_sweep(c);
+    int left = n_sweeps;
+    while (left > 0) {
+        // sweeps until the next exchange / measurement is due (or the end)
+        uint64_t run = (uint64_t)left;
+        if (pt_every > 0) run = std::min<uint64_t>(run, (uint64_t)pt_every - c->sweeps % (uint64_t)pt_every);
+        if (meas_every > 0) run = std::min<uint64_t>(run, (uint64_t)meas_every - c->sweeps % (uint64_t)meas_every);
         int rc;
+        if ((rc = do_sweeps(c, (int)run))) return rc;
+        left -= (int)run;
         if (pt_every > 0 && c->sweeps % (uint64_t)pt_every == 0)
             if ((rc = do_exchange(c))) return rc;
         if (meas_every > 0 && c->sweeps % (uint64_t)meas_every == 0)

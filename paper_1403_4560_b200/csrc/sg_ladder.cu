@@ -1,0 +1,312 @@
+// sg_ladder.cu — the fast +-J path for lattices whose temperature ladder fits in shared memory.
+//
+// One CTA owns one (packed word w, replica a) ladder: its NT systems (NT * N words) and the word's
+// couplings (3 N words) stay in shared memory for `n_sweeps` consecutive checkerboard sweeps, so
+// global memory is touched once per launch.  A thread owns one quad q of 4 consecutive same-colour
+// sites (= one Philox call, R6) for the systems t = g, g+G, ... of its group; the 24 coupling words
+// of its quad live in registers across those systems.  Bit-sliced arithmetic as in sg_pmj.cu:
+// per word-site 6 XOR3 + 8 (count) + 8 (accept/flip) + 5 (Philox share) = 27 ALU-pipe lane-ops; the
+// seven "r < thr" masks and the Philox products are IMAD.WIDE on the FMA pipe.
+#include "sg_device.cuh"
+#include "sg_internal.h"
+
+#include <algorithm>
+
+namespace sg {
+
+struct LadderArgs {
+    Dims d;
+    uint32_t *spins;
+    const uint32_t *J;
+    const SlotTab *tab;
+    uint32_t rk[20];          // Philox round keys: rk[2r] = k0 + r*0x9E3779B9, rk[2r+1] = k1 + r*0xBB67AE85
+    uint32_t one;             // = 1 (run-time value so that mad.wide stays an IMAD.WIDE)
+    uint32_t sweep0;          // global index of the first sweep of this launch
+    int n_sweeps;
+    int G;                    // system groups: thread (q, g) handles systems g, g+G, ...
+};
+
+__device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                           const uint32_t (&rk)[20])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = xor3((uint32_t)(p1 >> 32), c1, rk[2 * r]);
+        const uint32_t n2 = xor3((uint32_t)(p0 >> 32), c3, rk[2 * r + 1]);
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// all ones iff r < thr, c64 = (uint64)(0 - thr): high word of r * 1 + c64, one IMAD.WIDE
+__device__ __forceinline__ uint32_t lt_mask_mad(uint32_t r, uint32_t one, uint2 c64)
+{
+    uint64_t v;
+    const uint64_t c = ((uint64_t)c64.y << 32) | c64.x;
+    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(v) : "r"(r), "r"(one), "l"(c));
+    return (uint32_t)(v >> 32);
+}
+
+// Metropolis update of one word-site: returns the new spin word.  u0..u5 are the unsatisfied-bond
+// words, na = ~a (a = field alignment), B[c] = all ones iff r < thr[code c]  (comparator path).
+__device__ __forceinline__ uint32_t flip_word(uint32_t s, uint32_t u0, uint32_t u1, uint32_t u2, uint32_t u3,
+                                              uint32_t u4, uint32_t u5, uint32_t na, const uint32_t (&B)[7])
+{
+    const uint32_t s0 = xor3(u0, u1, u2), c0 = maj3(u0, u1, u2);
+    const uint32_t s1 = xor3(u3, u4, u5), c1 = maj3(u3, u4, u5);
+    const uint32_t n0 = s0 ^ s1;
+    const uint32_t k = s0 & s1;
+    const uint32_t n1 = xor3(c0, c1, k);
+    const uint32_t n2 = maj3(c0, c1, k);
+    const uint32_t nK0 = xor3(xor3(B[0], B[1], B[2]), xor3(B[3], B[4], B[5]), B[6]);
+    const uint32_t K1 = lop3<LUT_K1>(B[1], B[3], B[5]);
+    const uint32_t g0 = na | nK0;
+    const uint32_t g1 = lop3<LUT_GE>(n0, K1, g0);
+    const uint32_t g2 = lop3<(0xF0 & 0xCC) | ((0xF0 ^ 0xCC) & 0xAA)>(n1, B[3], g1);   // GE(n1, K2, g1) with K2 = ~B3 folded in
+    return lop3<LUT_FLIP>(s, n2, g2);
+}
+
+template <int L>
+struct Geo {
+    static constexpr int Lh = L / 2, N = L * L * L, H = N / 2, Q = H / 4;
+    static constexpr bool VEC = (Lh % 4) == 0;
+    static constexpr int QR = VEC ? Lh / 4 : 1;     // quads per row (vector path)
+};
+
+template <int L>
+__global__ void __launch_bounds__(512, 1) k_ladder_pmj(const __grid_constant__ LadderArgs A)
+{
+    using G_ = Geo<L>;
+    constexpr int Lh = G_::Lh, N = G_::N, H = G_::H, Q = G_::Q;
+    extern __shared__ __align__(16) uint32_t smem[];
+    const Dims &d = A.d;
+    const int NT = d.NT;
+    uint32_t *S = smem;                                   // [NT][2][H]
+    uint32_t *Jsm = S + (size_t)NT * N;                   // [2][3][H]
+    uint2 *thr = reinterpret_cast<uint2 *>(Jsm + 3 * N);  // [NT][8]
+
+    const int w = blockIdx.x / d.R, a = blockIdx.x % d.R;
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    uint32_t *gS = A.spins + ((size_t)(w * d.R + a) * NT) * N;
+    const uint32_t *gJ = A.J + (size_t)w * 3 * N;
+
+    // ---- load the ladder, the couplings and the threshold constants
+    {
+        const uint4 *src = reinterpret_cast<const uint4 *>(gS);
+        uint4 *dst = reinterpret_cast<uint4 *>(S);
+        for (int i = tid; i < NT * N / 4; i += nthr) dst[i] = src[i];
+        const uint4 *js = reinterpret_cast<const uint4 *>(gJ);
+        uint4 *jd = reinterpret_cast<uint4 *>(Jsm);
+        for (int i = tid; i < 3 * N / 4; i += nthr) jd[i] = js[i];
+        for (int i = tid; i < NT * 8; i += nthr) {
+            const int t = i >> 3, c = i & 7;
+            thr[i] = c < 7 ? A.tab[t].c64[c] : make_uint2(0u, 0u);
+        }
+    }
+    __syncthreads();
+
+    const int q = tid % Q, g = tid / Q;
+    const bool active = g < A.G;
+    const uint32_t amask = d.neg_h ? 0xffffffffu : 0u;     // a = s ^ amask ; na = ~a
+    const uint32_t wglob = (uint32_t)(w + (d.s_first >> 5));
+
+    for (int sw = 0; sw < A.n_sweeps; ++sw) {
+#pragma unroll 1
+        for (int colour = 0; colour < 2; ++colour) {
+            if (active) {
+                const uint32_t time = 2u * (A.sweep0 + (uint32_t)sw) + (uint32_t)colour;
+                const uint32_t *Jown = Jsm + (colour * 3) * H;
+                const uint32_t *Joth = Jsm + ((1 - colour) * 3) * H;
+                if constexpr (G_::VEC) {
+                    constexpr int QR = G_::QR;
+                    const int r = q / QR, kq = q % QR;
+                    const int y = r % L, z = r / L;
+                    const int p = (colour + y + z) & 1;
+                    const int q_yp = (y + 1 == L) ? q - (L - 1) * QR : q + QR;
+                    const int q_ym = (y == 0) ? q + (L - 1) * QR : q - QR;
+                    const int q_zp = (z + 1 == L) ? q - (L - 1) * L * QR : q + L * QR;
+                    const int q_zm = (z == 0) ? q + (L - 1) * L * QR : q - L * QR;
+                    int side[4];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int m = 4 * kq + e;
+                        const int ms = p ? (m + 1 == Lh ? 0 : m + 1) : (m == 0 ? Lh - 1 : m - 1);
+                        side[e] = r * Lh + ms;
+                    }
+                    // couplings of this quad -> registers (shared by all systems of the group)
+                    uint32_t JA[4], JB[4], Jyp[4], Jym[4], Jzp[4], Jzm[4];
+                    {
+                        const uint4 jx = reinterpret_cast<const uint4 *>(Jown)[q];
+                        const uint4 jox = reinterpret_cast<const uint4 *>(Joth)[q];
+                        const uint4 jy = reinterpret_cast<const uint4 *>(Jown + H)[q];
+                        const uint4 joy = reinterpret_cast<const uint4 *>(Joth + H)[q_ym];
+                        const uint4 jz = reinterpret_cast<const uint4 *>(Jown + 2 * H)[q];
+                        const uint4 joz = reinterpret_cast<const uint4 *>(Joth + 2 * H)[q_zm];
+                        const uint32_t jxv[4] = {jx.x, jx.y, jx.z, jx.w}, joxv[4] = {jox.x, jox.y, jox.z, jox.w};
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            // bond to the neighbour at the same compact index / at the side index
+                            JA[e] = p ? joxv[e] : jxv[e];
+                            JB[e] = p ? jxv[e] : Joth[side[e]];
+                        }
+                        Jyp[0] = jy.x; Jyp[1] = jy.y; Jyp[2] = jy.z; Jyp[3] = jy.w;
+                        Jym[0] = joy.x; Jym[1] = joy.y; Jym[2] = joy.z; Jym[3] = joy.w;
+                        Jzp[0] = jz.x; Jzp[1] = jz.y; Jzp[2] = jz.z; Jzp[3] = jz.w;
+                        Jzm[0] = joz.x; Jzm[1] = joz.y; Jzm[2] = joz.z; Jzm[3] = joz.w;
+                    }
+#pragma unroll 1
+                    for (int t = g; t < NT; t += A.G) {
+                        uint32_t *Sa = S + t * N + colour * H;
+                        const uint32_t *So = S + t * N + (1 - colour) * H;
+                        const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[q];
+                        const uint4 o0 = reinterpret_cast<const uint4 *>(So)[q];
+                        const uint4 oyp = reinterpret_cast<const uint4 *>(So)[q_yp];
+                        const uint4 oym = reinterpret_cast<const uint4 *>(So)[q_ym];
+                        const uint4 ozp = reinterpret_cast<const uint4 *>(So)[q_zp];
+                        const uint4 ozm = reinterpret_cast<const uint4 *>(So)[q_zm];
+                        const uint32_t os[4] = {So[side[0]], So[side[1]], So[side[2]], So[side[3]]};
+                        const uint4 r4 = philox_rk((uint32_t)q, time, wglob, ctr3(3, a, t), A.rk);
+                        uint2 c64[7];
+#pragma unroll
+                        for (int c = 0; c < 7; ++c) c64[c] = thr[t * 8 + c];
+                        const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
+                        const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
+                        const uint32_t v0[4] = {o0.x, o0.y, o0.z, o0.w}, vyp[4] = {oyp.x, oyp.y, oyp.z, oyp.w};
+                        const uint32_t vym[4] = {oym.x, oym.y, oym.z, oym.w}, vzp[4] = {ozp.x, ozp.y, ozp.z, ozp.w};
+                        const uint32_t vzm[4] = {ozm.x, ozm.y, ozm.z, ozm.w};
+                        uint32_t out[4];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            uint32_t B[7];
+#pragma unroll
+                            for (int c = 0; c < 7; ++c) B[c] = lt_mask_mad(rr[e], A.one, c64[c]);
+                            out[e] = flip_word(s[e], xor3(s[e], v0[e], JA[e]), xor3(s[e], os[e], JB[e]),
+                                               xor3(s[e], vyp[e], Jyp[e]), xor3(s[e], vym[e], Jym[e]),
+                                               xor3(s[e], vzp[e], Jzp[e]), xor3(s[e], vzm[e], Jzm[e]),
+                                               ~(s[e] ^ amask), B);
+                        }
+                        reinterpret_cast<uint4 *>(Sa)[q] = make_uint4(out[0], out[1], out[2], out[3]);
+                    }
+                } else {
+                    // generic lattice: per-element neighbour indices (compile-time L), couplings from smem
+#pragma unroll 1
+                    for (int t = g; t < NT; t += A.G) {
+                        uint32_t *Sa = S + t * N + colour * H;
+                        const uint32_t *So = S + t * N + (1 - colour) * H;
+                        const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[q];
+                        const uint4 r4 = philox_rk((uint32_t)q, time, wglob, ctr3(3, a, t), A.rk);
+                        uint2 c64[7];
+#pragma unroll
+                        for (int c = 0; c < 7; ++c) c64[c] = thr[t * 8 + c];
+                        const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
+                        const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
+                        uint32_t out[4];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const int n = 4 * q + e;
+                            const int row = n / Lh, m = n - row * Lh;
+                            const int z = row / L, y = row - z * L;
+                            const int p = (colour + y + z) & 1;
+                            const int sd = row * Lh + (p ? (m + 1 == Lh ? 0 : m + 1) : (m == 0 ? Lh - 1 : m - 1));
+                            const int xp = p ? sd : n, xm = p ? n : sd;
+                            const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m;
+                            const int ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
+                            const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m;
+                            const int zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
+                            uint32_t B[7];
+#pragma unroll
+                            for (int c = 0; c < 7; ++c) B[c] = lt_mask_mad(rr[e], A.one, c64[c]);
+                            out[e] = flip_word(s[e], xor3(s[e], So[xp], Jown[n]), xor3(s[e], So[xm], Joth[xm]),
+                                               xor3(s[e], So[yp], Jown[H + n]), xor3(s[e], So[ym], Joth[H + ym]),
+                                               xor3(s[e], So[zp], Jown[2 * H + n]), xor3(s[e], So[zm], Joth[2 * H + zm]),
+                                               ~(s[e] ^ amask), B);
+                        }
+                        reinterpret_cast<uint4 *>(Sa)[q] = make_uint4(out[0], out[1], out[2], out[3]);
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    // ---- write the ladder back
+    {
+        uint4 *dst = reinterpret_cast<uint4 *>(gS);
+        const uint4 *src = reinterpret_cast<const uint4 *>(S);
+        for (int i = tid; i < NT * N / 4; i += nthr) dst[i] = src[i];
+    }
+}
+
+// ------------------------------------------------------------------------------- host side
+size_t ladder_smem_bytes(int L, int NT)
+{
+    const size_t N = (size_t)L * L * L;
+    return (size_t)NT * N * 4 + 3 * N * 4 + (size_t)NT * 8 * sizeof(uint2);
+}
+
+bool ladder_supported(const sg_ctx *c)
+{
+    const Dims &d = c->d;
+    if (c->kind != SG_PMJ || !d.fast_accept) return false;
+    if (d.L != 4 && d.L != 6 && d.L != 8 && d.L != 10 && d.L != 12 && d.L != 16) return false;
+    return ladder_smem_bytes(d.L, d.NT) <= (size_t)227 * 1024;
+}
+
+template <int L>
+static cudaError_t launch_l(const LadderArgs &A, int threads, size_t smem, cudaStream_t st, int grid)
+{
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_ladder_pmj<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    k_ladder_pmj<L><<<grid, threads, smem, st>>>(A);
+    return cudaGetLastError();
+}
+
+// n_sweeps consecutive sweeps starting at global sweep index `sweep0`; returns kernels launched (or -1)
+int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps)
+{
+    const Dims &d = c->d;
+    LadderArgs A;
+    A.d = d;
+    A.spins = c->spins;
+    A.J = c->J;
+    A.tab = c->tab;
+    for (int r = 0; r < 10; ++r) {
+        A.rk[2 * r] = d.k0 + (uint32_t)r * 0x9E3779B9u;
+        A.rk[2 * r + 1] = d.k1 + (uint32_t)r * 0xBB67AE85u;
+    }
+    A.one = 1u;
+    A.sweep0 = (uint32_t)sweep0;
+    A.n_sweeps = n_sweeps;
+    const int Q = d.N / 8;
+    // groups: as many as fit in <= 512 threads, at most NT, preferring a divisor of NT
+    int G = std::max(1, std::min(d.NT, 512 / Q));
+    for (int gtry = G; gtry >= 1 && gtry * 2 > G; --gtry)
+        if (d.NT % gtry == 0) { G = gtry; break; }
+    A.G = G;
+    int threads = (Q * G + 31) / 32 * 32;
+    if (threads > 512) return -1;
+    const size_t smem = ladder_smem_bytes(d.L, d.NT);
+    const int grid = d.W * d.R;
+    cudaError_t e;
+    switch (d.L) {
+    case 4: e = launch_l<4>(A, threads, smem, c->stream, grid); break;
+    case 6: e = launch_l<6>(A, threads, smem, c->stream, grid); break;
+    case 8: e = launch_l<8>(A, threads, smem, c->stream, grid); break;
+    case 10: e = launch_l<10>(A, threads, smem, c->stream, grid); break;
+    case 12: e = launch_l<12>(A, threads, smem, c->stream, grid); break;
+    case 16: e = launch_l<16>(A, threads, smem, c->stream, grid); break;
+    default: return -1;
+    }
+    return e == cudaSuccess ? 1 : -1;
+}
+
+}  // namespace sg
