@@ -80,6 +80,8 @@ int launch_sweep_pmj(sg_ctx *c, uint64_t sweep);            // both colours
 int launch_sweep_gauss(sg_ctx *c, uint64_t sweep);
 bool ladder_supported(const sg_ctx *c);                    // shared-memory-resident ladder kernel usable?
 int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps);   // n consecutive sweeps, 1 launch (-1 on error)
+bool ladder8_supported(const sg_ctx *c);                   // L = 8 kernel with fused parallel tempering
+int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_sweeps, int pt_every);
 int launch_energy_pmj(sg_ctx *c);
 int launch_energy_gauss(sg_ctx *c);
 int launch_pt_pmj(sg_ctx *c, uint64_t exchange);            // decide + swap (energies must be fresh)

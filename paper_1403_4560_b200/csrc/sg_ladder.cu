@@ -20,7 +20,7 @@ struct LadderArgs {
     const uint32_t *J;
     const SlotTab *tab;
     uint32_t rk[20];          // Philox round keys: rk[2r] = k0 + r*0x9E3779B9, rk[2r+1] = k1 + r*0xBB67AE85
-    uint32_t one;             // = 1 (run-time value so that mad.wide stays an IMAD.WIDE)
+    uint32_t pad0;
     uint32_t sweep0;          // global index of the first sweep of this launch
     int n_sweeps;
     int G;                    // system groups: thread (q, g) handles systems g, g+G, ...
@@ -43,12 +43,11 @@ __device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, uint32_t c2
     return make_uint4(c0, c1, c2, c3);
 }
 
-// all ones iff r < thr, c64 = (uint64)(0 - thr): high word of r * 1 + c64, one IMAD.WIDE
-__device__ __forceinline__ uint32_t lt_mask_mad(uint32_t r, uint32_t one, uint2 c64)
+// all ones iff r < thr, c64 = (uint64)(0 - thr): high word of r + c64.  ptxas emits one IADD3 (carry
+// out, ALU pipe) + one IMAD.X (c64.hi + carry, FMA pipe); a mad.wide formulation is split the same way.
+__device__ __forceinline__ uint32_t lt_mask64(uint32_t r, uint2 c64)
 {
-    uint64_t v;
-    const uint64_t c = ((uint64_t)c64.y << 32) | c64.x;
-    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(v) : "r"(r), "r"(one), "l"(c));
+    const uint64_t v = (uint64_t)r + (((uint64_t)c64.y << 32) | c64.x);
     return (uint32_t)(v >> 32);
 }
 
@@ -76,10 +75,13 @@ struct Geo {
     static constexpr int Lh = L / 2, N = L * L * L, H = N / 2, Q = H / 4;
     static constexpr bool VEC = (Lh % 4) == 0;
     static constexpr int QR = VEC ? Lh / 4 : 1;     // quads per row (vector path)
+    // launch bounds: L=8 runs two 320-thread CTAs per SM (256 ladders of config 2 on 148 SMs)
+    static constexpr int MAXT = L == 8 ? 320 : 512;
+    static constexpr int MINB = L == 8 ? 2 : 1;
 };
 
 template <int L>
-__global__ void __launch_bounds__(512, 1) k_ladder_pmj(const __grid_constant__ LadderArgs A)
+__global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const __grid_constant__ LadderArgs A)
 {
     using G_ = Geo<L>;
     constexpr int Lh = G_::Lh, N = G_::N, H = G_::H, Q = G_::Q;
@@ -184,7 +186,7 @@ __global__ void __launch_bounds__(512, 1) k_ladder_pmj(const __grid_constant__ L
                         for (int e = 0; e < 4; ++e) {
                             uint32_t B[7];
 #pragma unroll
-                            for (int c = 0; c < 7; ++c) B[c] = lt_mask_mad(rr[e], A.one, c64[c]);
+                            for (int c = 0; c < 7; ++c) B[c] = lt_mask64(rr[e], c64[c]);
                             out[e] = flip_word(s[e], xor3(s[e], v0[e], JA[e]), xor3(s[e], os[e], JB[e]),
                                                xor3(s[e], vyp[e], Jyp[e]), xor3(s[e], vym[e], Jym[e]),
                                                xor3(s[e], vzp[e], Jzp[e]), xor3(s[e], vzm[e], Jzm[e]),
@@ -220,7 +222,7 @@ __global__ void __launch_bounds__(512, 1) k_ladder_pmj(const __grid_constant__ L
                             const int zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
                             uint32_t B[7];
 #pragma unroll
-                            for (int c = 0; c < 7; ++c) B[c] = lt_mask_mad(rr[e], A.one, c64[c]);
+                            for (int c = 0; c < 7; ++c) B[c] = lt_mask64(rr[e], c64[c]);
                             out[e] = flip_word(s[e], xor3(s[e], So[xp], Jown[n]), xor3(s[e], So[xm], Joth[xm]),
                                                xor3(s[e], So[yp], Jown[H + n]), xor3(s[e], So[ym], Joth[H + ym]),
                                                xor3(s[e], So[zp], Jown[2 * H + n]), xor3(s[e], So[zm], Joth[2 * H + zm]),
@@ -283,17 +285,18 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps)
         A.rk[2 * r] = d.k0 + (uint32_t)r * 0x9E3779B9u;
         A.rk[2 * r + 1] = d.k1 + (uint32_t)r * 0xBB67AE85u;
     }
-    A.one = 1u;
+    A.pad0 = 0;
     A.sweep0 = (uint32_t)sweep0;
     A.n_sweeps = n_sweeps;
     const int Q = d.N / 8;
     // groups: as many as fit in <= 512 threads, at most NT, preferring a divisor of NT
-    int G = std::max(1, std::min(d.NT, 512 / Q));
+    const int maxt = d.L == 8 ? 320 : 512;
+    int G = std::max(1, std::min(d.NT, maxt / Q));
     for (int gtry = G; gtry >= 1 && gtry * 2 > G; --gtry)
         if (d.NT % gtry == 0) { G = gtry; break; }
     A.G = G;
     int threads = (Q * G + 31) / 32 * 32;
-    if (threads > 512) return -1;
+    if (threads > maxt) return -1;
     const size_t smem = ladder_smem_bytes(d.L, d.NT);
     const int grid = d.W * d.R;
     cudaError_t e;

@@ -1,0 +1,415 @@
+// sg_ladder8.cu — L = 8 specialisation of the shared-memory ladder kernel (BASELINE.json config 2),
+// with parallel tempering fused in: one launch runs `n_sweeps` sweeps and every exchange that falls
+// due between them, without leaving the SM.
+//
+// L = 8: a quad (4 same-colour sites = one Philox call) is exactly one (y, z) row.  Rows are kept in
+// shared memory sorted by the parity pi = (y+z)&1 ("slot" order), so that every warp owns 32 rows of
+// one parity: the row parity p = (colour + pi) & 1 that decides whether the second x-neighbour sits
+// at m-1 or m+1 is then warp-uniform and becomes a static register renaming (no selects, no extra
+// loads, no bank conflicts: all neighbour rows of a quarter-warp are contiguous 128-byte runs).
+// Thread (g, pi, j) owns slot pi*32+j for the systems t = g, g+G, ...; the two warps of a group only
+// synchronise with each other (named barrier) between half sweeps.
+//
+// Exchange step (R12), all in shared memory: per-lane U and M of every system are reduced from the
+// bit planes produced during the colour-1 half sweep (U = sum over colour-1 sites of their post-flip
+// unsatisfied count; M = sum of all spin words) by three bit-sliced 4:1 adder stages and one warp
+// bit-transpose per system; one thread per (pair, lane) decides; masked swap of the two systems.
+#include "sg_device.cuh"
+#include "sg_internal.h"
+
+namespace sg {
+
+struct Ladder8Args {
+    Dims d;
+    uint32_t *spins;
+    const uint32_t *J;
+    const SlotTab *tab;
+    const double *exp_tab;
+    double h;
+    uint32_t rk[20];
+    uint64_t sweep0;          // global index of the first sweep of this launch
+    uint64_t exchange0;       // global index of the first exchange of this launch
+    int n_sweeps;
+    int pt_every;             // 0 = never
+    int G;
+};
+
+__device__ __forceinline__ int slot_of_row(int y, int z) { return ((y + z) & 1) * 32 + z * 4 + (y >> 1); }
+
+__device__ __forceinline__ uint4 philox_rk8(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const uint32_t (&rk)[20])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = xor3((uint32_t)(p1 >> 32), c1, rk[2 * r]);
+        const uint32_t n2 = xor3((uint32_t)(p0 >> 32), c3, rk[2 * r + 1]);
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+__device__ __forceinline__ uint32_t lt_mask8(uint32_t r, uint2 c64)
+{
+    const uint64_t v = (uint64_t)r + (((uint64_t)c64.y << 32) | c64.x);
+    return (uint32_t)(v >> 32);
+}
+
+// One word-site: count the unsatisfied bonds (n0 n1 n2), decide, return the accept word.
+__device__ __forceinline__ uint32_t accept_word(uint32_t u0, uint32_t u1, uint32_t u2, uint32_t u3, uint32_t u4,
+                                                uint32_t u5, uint32_t na, const uint32_t (&B)[7], uint32_t &n0,
+                                                uint32_t &n1, uint32_t &n2)
+{
+    const uint32_t s0 = xor3(u0, u1, u2), c0 = maj3(u0, u1, u2);
+    const uint32_t s1 = xor3(u3, u4, u5), c1 = maj3(u3, u4, u5);
+    n0 = s0 ^ s1;
+    const uint32_t k = s0 & s1;
+    n1 = xor3(c0, c1, k);
+    n2 = maj3(c0, c1, k);
+    const uint32_t nK0 = xor3(xor3(B[0], B[1], B[2]), xor3(B[3], B[4], B[5]), B[6]);
+    const uint32_t K1 = lop3<LUT_K1>(B[1], B[3], B[5]);
+    const uint32_t g0 = na | nK0;
+    const uint32_t g1 = lop3<LUT_GE>(n0, K1, g0);
+    const uint32_t g2 = lop3<LUT_MAJ>(n1, B[3], g1);            // GE(n1, K2, g1) with K2 = ~B3
+    return n2 | g2;
+}
+
+// bit-sliced a (NA planes) + b (NA planes) -> NA+1 planes
+template <int NA>
+__device__ __forceinline__ void bs_sum(const uint32_t (&a)[NA], const uint32_t (&b)[NA], uint32_t (&o)[NA + 1])
+{
+    uint32_t carry = a[0] & b[0];
+    o[0] = a[0] ^ b[0];
+#pragma unroll
+    for (int k = 1; k < NA; ++k) {
+        o[k] = xor3(a[k], b[k], carry);
+        carry = maj3(a[k], b[k], carry);
+    }
+    o[NA] = carry;
+}
+
+constexpr int PU1 = 5, PM1 = 4;             // planes per thread after the in-thread stage (U <= 24, M <= 8)
+constexpr int PW1 = PU1 + PM1;              // words per (system, thread) in the reduction buffer
+
+// 4:1 adder stage over the reduction buffer: in[sys][PU+PM][n_in] -> out[sys][PU+2+PM+2][n_in/4]
+template <int PU, int PM>
+__device__ __forceinline__ void reduce4(const uint32_t *__restrict__ in, uint32_t *__restrict__ out, int n_sys,
+                                        int n_in, int tid, int nthr)
+{
+    const int n_out = n_in >> 2;
+    for (int item = tid; item < n_sys * n_out; item += nthr) {
+        const int sys = item / n_out, c = item - sys * n_out;
+        const uint32_t *src = in + (size_t)sys * (PU + PM) * n_in + 4 * c;
+        uint32_t a[PU], b[PU], ab[PU + 1], cd[PU + 1], u[PU + 2];
+#pragma unroll
+        for (int k = 0; k < PU; ++k) { a[k] = src[k * n_in]; b[k] = src[k * n_in + 1]; }
+        bs_sum<PU>(a, b, ab);
+#pragma unroll
+        for (int k = 0; k < PU; ++k) { a[k] = src[k * n_in + 2]; b[k] = src[k * n_in + 3]; }
+        bs_sum<PU>(a, b, cd);
+        bs_sum<PU + 1>(ab, cd, u);
+        uint32_t ma[PM], mb[PM], mab[PM + 1], mcd[PM + 1], m[PM + 2];
+        const uint32_t *srm = src + PU * n_in;
+#pragma unroll
+        for (int k = 0; k < PM; ++k) { ma[k] = srm[k * n_in]; mb[k] = srm[k * n_in + 1]; }
+        bs_sum<PM>(ma, mb, mab);
+#pragma unroll
+        for (int k = 0; k < PM; ++k) { ma[k] = srm[k * n_in + 2]; mb[k] = srm[k * n_in + 3]; }
+        bs_sum<PM>(ma, mb, mcd);
+        bs_sum<PM + 1>(mab, mcd, m);
+        uint32_t *dst = out + (size_t)sys * (PU + PM + 4) * n_out + c;
+#pragma unroll
+        for (int k = 0; k < PU + 2; ++k) dst[k * n_out] = u[k];
+#pragma unroll
+        for (int k = 0; k < PM + 2; ++k) dst[(PU + 2 + k) * n_out] = m[k];
+    }
+}
+
+template <int P>
+__device__ __forceinline__ void half_sweep_quad(uint32_t *__restrict__ Sa, const uint32_t *__restrict__ So, int slot,
+                                                int s_yp, int s_ym, int s_zp, int s_zm, const uint32_t (&JA)[4],
+                                                const uint32_t (&JB)[4], const uint32_t (&Jyp)[4],
+                                                const uint32_t (&Jym)[4], const uint32_t (&Jzp)[4],
+                                                const uint32_t (&Jzm)[4], const uint4 r4, const uint2 *__restrict__ thr_t,
+                                                uint32_t amask, bool want_energy, uint32_t *__restrict__ red)
+{
+    const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[slot];
+    const uint4 o0 = reinterpret_cast<const uint4 *>(So)[slot];
+    const uint4 oyp = reinterpret_cast<const uint4 *>(So)[s_yp];
+    const uint4 oym = reinterpret_cast<const uint4 *>(So)[s_ym];
+    const uint4 ozp = reinterpret_cast<const uint4 *>(So)[s_zp];
+    const uint4 ozm = reinterpret_cast<const uint4 *>(So)[s_zm];
+    uint2 c64[7];
+#pragma unroll
+    for (int c = 0; c < 7; ++c) c64[c] = thr_t[c];
+    const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
+    const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
+    const uint32_t v0[4] = {o0.x, o0.y, o0.z, o0.w};
+    // second x-neighbour: m+1 for p = 1, m-1 for p = 0 (periodic within the row) — static renaming
+    const uint32_t vB[4] = {P ? o0.y : o0.w, P ? o0.z : o0.x, P ? o0.w : o0.y, P ? o0.x : o0.z};
+    const uint32_t vyp[4] = {oyp.x, oyp.y, oyp.z, oyp.w}, vym[4] = {oym.x, oym.y, oym.z, oym.w};
+    const uint32_t vzp[4] = {ozp.x, ozp.y, ozp.z, ozp.w}, vzm[4] = {ozm.x, ozm.y, ozm.z, ozm.w};
+    uint32_t out[4], w[4][3];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        uint32_t B[7], n0, n1, n2;
+#pragma unroll
+        for (int c = 0; c < 7; ++c) B[c] = lt_mask8(rr[e], c64[c]);
+        const uint32_t acc = accept_word(xor3(s[e], v0[e], JA[e]), xor3(s[e], vB[e], JB[e]), xor3(s[e], vyp[e], Jyp[e]),
+                                         xor3(s[e], vym[e], Jym[e]), xor3(s[e], vzp[e], Jzp[e]),
+                                         xor3(s[e], vzm[e], Jzm[e]), ~(s[e] ^ amask), B, n0, n1, n2);
+        out[e] = s[e] ^ acc;
+        // post-flip unsatisfied count of this site: n if not flipped, 6 - n if flipped
+        w[e][0] = n0;
+        w[e][1] = n1;
+        w[e][2] = n2;
+        if (want_energy) {
+            // 6 - n: bit0 = n0; bit1 = 1 for n in {0,3,4}; bit2 = 1 for n in {0,1,2}
+            const uint32_t f1 = (~n2 & ~(n1 ^ n0)) | (n2 & ~n1 & ~n0);
+            const uint32_t f2 = ~n2 & ~(n1 & n0);
+            w[e][1] = (acc & f1) | (~acc & n1);
+            w[e][2] = (acc & f2) | (~acc & n2);
+        }
+    }
+    reinterpret_cast<uint4 *>(Sa)[slot] = make_uint4(out[0], out[1], out[2], out[3]);
+    if (want_energy) {
+        uint32_t ab[4], cd[4], U[5];
+        bs_sum<3>(w[0], w[1], ab);
+        bs_sum<3>(w[2], w[3], cd);
+        bs_sum<4>(ab, cd, U);
+        // M: 8 words (4 new own-colour + 4 other-colour of the same row) -> 4 planes
+        const uint32_t a1 = xor3(out[0], out[1], out[2]), c1 = maj3(out[0], out[1], out[2]);
+        const uint32_t a2 = xor3(out[3], v0[0], v0[1]), c2 = maj3(out[3], v0[0], v0[1]);
+        const uint32_t a3 = xor3(a1, a2, v0[2]), c3 = maj3(a1, a2, v0[2]);
+        const uint32_t ones = a3 ^ v0[3], c4 = a3 & v0[3];
+        const uint32_t t1 = xor3(c1, c2, c3), f1 = maj3(c1, c2, c3);
+        const uint32_t twos = t1 ^ c4, f2 = t1 & c4;
+        const uint32_t fours = f1 ^ f2, eights = f1 & f2;
+        // red[plane][64 threads of the system]
+#pragma unroll
+        for (int k = 0; k < 5; ++k) red[k * 64] = U[k];
+        red[5 * 64] = ones;
+        red[6 * 64] = twos;
+        red[7 * 64] = fours;
+        red[8 * 64] = eights;
+    }
+}
+
+__global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ Ladder8Args A)
+{
+    constexpr int N = 512, H = 256;
+    extern __shared__ __align__(16) uint32_t smem[];
+    const Dims &d = A.d;
+    const int NT = d.NT;
+    uint32_t *S = smem;                                    // [NT][2][64 slots][4]
+    uint32_t *Jsm = S + NT * N;                            // [2][3][64 slots][4]
+    uint2 *thr = reinterpret_cast<uint2 *>(Jsm + 3 * N);   // [NT][8]
+    uint32_t *masks = reinterpret_cast<uint32_t *>(thr + NT * 8);     // [32]
+    // exchange scratch (allocated only when pt_every > 0); later stages alias dead earlier ones
+    uint32_t *red0 = masks + 32;                           // [NT][9][64]   stage-1 planes
+    uint32_t *red1 = red0 + NT * PW1 * 64;                 // [NT][13][16]
+    uint32_t *red2 = red0;                                 // [NT][17][4]   (red0 is dead after stage 2)
+    uint32_t *red3 = red1;                                 // [NT][21][1]   (red1 is dead after stage 3)
+    int *Uint = reinterpret_cast<int *>(red0 + NT * 17 * 4);   // [NT][32]  (behind red2, inside red0's area)
+    int *Mint = Uint + NT * 32;                            // [NT][32]
+
+    const int w = blockIdx.x / d.R, a = blockIdx.x % d.R;
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    uint32_t *gS = A.spins + ((size_t)(w * d.R + a) * NT) * N;
+    const uint32_t *gJ = A.J + (size_t)w * 3 * N;
+
+    // ---- load (global compact order -> slot order)
+    for (int i = tid; i < NT * 128; i += nthr) {           // quads of all systems, both colours
+        const int qq = i & 63, tc = i >> 6;                // tc = t*2 + colour
+        reinterpret_cast<uint4 *>(S)[tc * 64 + slot_of_row(qq & 7, qq >> 3)] = reinterpret_cast<const uint4 *>(gS)[i];
+    }
+    for (int i = tid; i < 6 * 64; i += nthr) {             // [colour][d][quad]
+        const int qq = i & 63, cd = i >> 6;
+        reinterpret_cast<uint4 *>(Jsm)[cd * 64 + slot_of_row(qq & 7, qq >> 3)] = reinterpret_cast<const uint4 *>(gJ)[i];
+    }
+    for (int i = tid; i < NT * 8; i += nthr) {
+        const int t = i >> 3, c = i & 7;
+        thr[i] = c < 7 ? A.tab[t].c64[c] : make_uint2(0u, 0u);
+    }
+    __syncthreads();
+
+    // ---- thread geometry (colour independent)
+    const int g = tid >> 6, pi = (tid >> 5) & 1, j = tid & 31;
+    const int z = j >> 2, yy = j & 3, y = 2 * yy + ((pi + z) & 1);
+    const int slot = pi * 32 + j, q = z * 8 + y;
+    const int ob = (1 - pi) * 32;
+    const int s_yp = ob + z * 4 + (((y + 1) & 7) >> 1), s_ym = ob + z * 4 + (((y + 7) & 7) >> 1);
+    const int s_zp = ob + ((z + 1) & 7) * 4 + yy, s_zm = ob + ((z + 7) & 7) * 4 + yy;
+    const bool active = g < A.G;
+    const uint32_t amask = d.neg_h ? 0xffffffffu : 0u;
+    const uint32_t wglob = (uint32_t)(w + (d.s_first >> 5));
+    uint64_t exchange = A.exchange0;
+
+    for (int sw = 0; sw < A.n_sweeps; ++sw) {
+        const uint64_t sweep = A.sweep0 + (uint64_t)sw;
+        const bool pt_due = A.pt_every > 0 && ((sweep + 1) % (uint64_t)A.pt_every) == 0;
+#pragma unroll 1
+        for (int colour = 0; colour < 2; ++colour) {
+            if (active) {
+                const uint32_t time = 2u * (uint32_t)sweep + (uint32_t)colour;
+                const int p = (colour + pi) & 1;
+                const uint32_t *Jown = Jsm + (colour * 3) * H;
+                const uint32_t *Joth = Jsm + ((1 - colour) * 3) * H;
+                uint32_t JA[4], JB[4], Jyp[4], Jym[4], Jzp[4], Jzm[4];
+                {
+                    const uint4 jx = reinterpret_cast<const uint4 *>(Jown)[slot];
+                    const uint4 jox = reinterpret_cast<const uint4 *>(Joth)[slot];
+                    const uint4 jy = reinterpret_cast<const uint4 *>(Jown + H)[slot];
+                    const uint4 joy = reinterpret_cast<const uint4 *>(Joth + H)[s_ym];
+                    const uint4 jz = reinterpret_cast<const uint4 *>(Jown + 2 * H)[slot];
+                    const uint4 joz = reinterpret_cast<const uint4 *>(Joth + 2 * H)[s_zm];
+                    if (p) {       // neighbour at the same m is the -x one (its bond), at m+1 the +x one (own bond)
+                        JA[0] = jox.x; JA[1] = jox.y; JA[2] = jox.z; JA[3] = jox.w;
+                        JB[0] = jx.x; JB[1] = jx.y; JB[2] = jx.z; JB[3] = jx.w;
+                    } else {       // neighbour at the same m is the +x one (own bond), at m-1 the -x one (its bond)
+                        JA[0] = jx.x; JA[1] = jx.y; JA[2] = jx.z; JA[3] = jx.w;
+                        JB[0] = jox.w; JB[1] = jox.x; JB[2] = jox.y; JB[3] = jox.z;
+                    }
+                    Jyp[0] = jy.x; Jyp[1] = jy.y; Jyp[2] = jy.z; Jyp[3] = jy.w;
+                    Jym[0] = joy.x; Jym[1] = joy.y; Jym[2] = joy.z; Jym[3] = joy.w;
+                    Jzp[0] = jz.x; Jzp[1] = jz.y; Jzp[2] = jz.z; Jzp[3] = jz.w;
+                    Jzm[0] = joz.x; Jzm[1] = joz.y; Jzm[2] = joz.z; Jzm[3] = joz.w;
+                }
+                const bool want_energy = pt_due && colour == 1;
+                uint4 r4 = philox_rk8((uint32_t)q, time, wglob, ctr3(3, a, g), A.rk);
+#pragma unroll 1
+                for (int t = g; t < NT; t += A.G) {
+                    uint32_t *Sa = S + t * N + colour * H;
+                    const uint32_t *So = S + t * N + (1 - colour) * H;
+                    const uint4 r_cur = r4;
+                    if (t + A.G < NT) r4 = philox_rk8((uint32_t)q, time, wglob, ctr3(3, a, t + A.G), A.rk);   // next system's draws
+                    uint32_t *red = red0 + (size_t)t * PW1 * 64 + (pi * 32 + j);
+                    if (p) half_sweep_quad<1>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm, r_cur,
+                                              thr + t * 8, amask, want_energy, red);
+                    else   half_sweep_quad<0>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm, r_cur,
+                                              thr + t * 8, amask, want_energy, red);
+                }
+                // the two warps of this group share systems; other groups are independent
+                asm volatile("bar.sync %0, 64;" ::"r"(g + 1) : "memory");
+            }
+        }
+        if (pt_due) {
+            __syncthreads();
+            // ---- per-lane energies: three 4:1 bit-sliced adder stages, then one transpose per system
+            reduce4<5, 4>(red0, red1, NT, 64, tid, nthr);
+            __syncthreads();
+            reduce4<7, 6>(red1, red2, NT, 16, tid, nthr);
+            __syncthreads();
+            reduce4<9, 8>(red2, red3, NT, 4, tid, nthr);
+            __syncthreads();
+            {
+                const int lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
+                for (int t = warp; t < NT; t += nwarp) {
+                    const uint32_t x = lane < 21 ? red3[t * 21 + lane] : 0u;      // 11 planes of U, 10 of M
+                    const uint32_t v = transpose32(x, lane);
+                    Uint[t * 32 + lane] = (int)(v & 0x7ffu);
+                    Mint[t * 32 + lane] = 2 * (int)((v >> 11) & 0x3ffu) - N;
+                }
+            }
+            __syncthreads();
+            // ---- decisions: one thread per (pair, lane)
+            const int e1 = (int)(exchange & 1u);
+            const int npairs = (NT - e1) / 2;
+            for (int item = tid; item < npairs * 32; item += nthr) {       // whole warps: npairs*32 is a multiple of 32
+                const int pair = item >> 5, lane = item & 31;
+                const int t = e1 + 2 * pair;
+                const int s = w * 32 + lane;
+                const int U0 = Uint[t * 32 + lane], U1 = Uint[(t + 1) * 32 + lane];
+                const int M0 = Mint[t * 32 + lane], M1 = Mint[(t + 1) * 32 + lane];
+                const double Et = __dsub_rn((double)(2 * U0 - 3 * N), __dmul_rn(A.h, (double)M0));
+                const double Eu = __dsub_rn((double)(2 * U1 - 3 * N), __dmul_rn(A.h, (double)M1));
+                const double x = __dmul_rn(__dsub_rn(A.tab[t].beta, A.tab[t + 1].beta), __dsub_rn(Et, Eu));
+                const uint4 r = philox_rk8(0u, (uint32_t)exchange, (uint32_t)(s + d.s_first), ctr3(4, a, t), A.rk);
+                const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
+                const uint32_t mask = __ballot_sync(0xffffffffu, accept && s < d.n_samples);
+                if (lane == 0) masks[pair] = mask;
+            }
+            __syncthreads();
+            // ---- masked swap of the two configurations (layout independent: same slot in both systems)
+            for (int item = tid; item < npairs * 128; item += nthr) {
+                const int pair = item >> 7, k = item & 127;
+                const uint32_t mask = masks[pair];
+                if (mask == 0u) continue;
+                const int t = e1 + 2 * pair;
+                uint4 *X = reinterpret_cast<uint4 *>(S + t * N) + k;
+                uint4 *Y = reinterpret_cast<uint4 *>(S + (t + 1) * N) + k;
+                uint4 xv = *X, yv = *Y;
+                uint32_t dd;
+                dd = (xv.x ^ yv.x) & mask; xv.x ^= dd; yv.x ^= dd;
+                dd = (xv.y ^ yv.y) & mask; xv.y ^= dd; yv.y ^= dd;
+                dd = (xv.z ^ yv.z) & mask; xv.z ^= dd; yv.z ^= dd;
+                dd = (xv.w ^ yv.w) & mask; xv.w ^= dd; yv.w ^= dd;
+                *X = xv;
+                *Y = yv;
+            }
+            exchange += 1;
+            __syncthreads();
+        }
+    }
+    __syncthreads();
+
+    // ---- write back (slot order -> global compact order)
+    for (int i = tid; i < NT * 128; i += nthr) {
+        const int qq = i & 63, tc = i >> 6;
+        reinterpret_cast<uint4 *>(gS)[i] = reinterpret_cast<const uint4 *>(S)[tc * 64 + slot_of_row(qq & 7, qq >> 3)];
+    }
+}
+
+// ------------------------------------------------------------------------------- host side
+static size_t ladder8_smem(int NT, bool with_pt)
+{
+    size_t b = (size_t)NT * 512 * 4 + 3 * 512 * 4 + (size_t)NT * 8 * sizeof(uint2) + 32 * 4;
+    if (with_pt) b += (size_t)NT * 4 * (PW1 * 64 + 13 * 16);
+    return b;
+}
+
+bool ladder8_supported(const sg_ctx *c)
+{
+    const Dims &d = c->d;
+    return c->kind == SG_PMJ && d.fast_accept && d.L == 8 && ladder8_smem(d.NT, true) <= (size_t)113 * 1024;
+}
+
+// n_sweeps sweeps (global indices sweep0...) with the exchanges that fall due (pt_every; 0 = none).
+// Returns kernels launched (1) or -1.  The caller advances its sweep / exchange counters.
+int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_sweeps, int pt_every)
+{
+    static bool configured = false;
+    if (!configured) {
+        if (cudaFuncSetAttribute(k_ladder8_pmj, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess) return -1;
+        configured = true;
+    }
+    const Dims &d = c->d;
+    Ladder8Args A;
+    A.d = d;
+    A.spins = c->spins;
+    A.J = c->J;
+    A.tab = c->tab;
+    A.exp_tab = c->exp64_tab;
+    A.h = c->h;
+    for (int r = 0; r < 10; ++r) {
+        A.rk[2 * r] = d.k0 + (uint32_t)r * 0x9E3779B9u;
+        A.rk[2 * r + 1] = d.k1 + (uint32_t)r * 0xBB67AE85u;
+    }
+    A.sweep0 = sweep0;
+    A.exchange0 = exchange0;
+    A.n_sweeps = n_sweeps;
+    A.pt_every = pt_every;
+    int G = d.NT < 5 ? d.NT : 5;
+    for (int gtry = G; gtry >= 1; --gtry)
+        if (d.NT % gtry == 0) { G = gtry; break; }
+    A.G = G;
+    // whole-CTA phases assume complete warps; always launch 64*G threads (G <= 5 -> <= 320)
+    const int threads = 64 * G;
+    k_ladder8_pmj<<<d.W * d.R, threads, ladder8_smem(d.NT, pt_every > 0), c->stream>>>(A);
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+}  // namespace sg

@@ -209,3 +209,28 @@ def test_error_paths(sg):
     with pytest.raises(sg.SgError):
         sim.sg_get_spins(3, 5)
     sim.close()
+
+
+@pytest.mark.parametrize("h,NT,R,pt_every,n_samples", [(0.2, 20, 4, 1, 64), (-0.4, 7, 2, 3, 33), (0.0, 5, 4, 2, 32),
+                                                     (1.0, 10, 2, 1, 96)])
+def test_l8_fused_ladder_with_pt(sg, O, h, NT, R, pt_every, n_samples):
+    """The L=8 shared-memory ladder kernel with in-kernel parallel tempering (sg_run) vs the oracle:
+    spins, energies bit-exact after 50 sweeps incl. a measurement boundary; moments to 1e-12."""
+    temps = W.ladder(0.5, 2.0, NT)
+    samples = sorted({0, 13, n_samples - 1, n_samples // 2})
+    sim, orc = make_pair(sg, O, 8, h, n_samples, R, temps, 0, 21, samples)
+    sim.sg_run(50, pt_every, 16)
+    for o in orc.values():
+        o.run(50, pt_every, 16)
+    check_state(sim, orc, "fused L8")
+    assert sim.sg_get_counters() == (50, 50 // pt_every)
+    mom, n = sim.sg_get_moments()
+    assert n == 3
+    for s, o in orc.items():
+        assert close(mom[s], o.moments()[0])
+    # continue with primitives from the fused state: counters and RNG streams line up
+    sim.sg_sweep(1); sim.sg_pt_exchange(); sim.sg_run(5, pt_every, 0)
+    for o in orc.values():
+        o.sweep(1); o.pt_exchange(); o.run(5, pt_every, 0)
+    check_state(sim, orc, "fused L8 + primitives")
+    sim.close()
