@@ -32,6 +32,7 @@ struct Ladder8Args {
     int n_sweeps;
     int pt_every;             // 0 = never
     int G;
+    uint32_t one, mone;       // 1 and 0xFFFFFFFF as run-time values: mad.lo with them stays an IMAD (FMA pipe)
 };
 
 __device__ __forceinline__ int slot_of_row(int y, int z) { return ((y + z) & 1) * 32 + z * 4 + (y >> 1); }
@@ -52,16 +53,40 @@ __device__ __forceinline__ uint4 philox_rk8(uint32_t c0, uint32_t c1, uint32_t c
     return make_uint4(c0, c1, c2, c3);
 }
 
-__device__ __forceinline__ uint32_t lt_mask8(uint32_t r, uint2 c64)
+// acc * one + [r + lo carries]: one IADD3 (carry out only, ALU pipe) + one IMAD.X (FMA pipe).  `one` is a
+// run-time 1, so ptxas keeps the multiply-add-with-carry on the FMA pipe instead of an IADD3.X.
+__device__ __forceinline__ uint32_t cadd(uint32_t r, uint32_t lo, uint32_t acc, uint32_t one)
 {
-    const uint64_t v = (uint64_t)r + (((uint64_t)c64.y << 32) | c64.x);
-    return (uint32_t)(v >> 32);
+    uint32_t d;
+    asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\tmadc.lo.u32 %0, %3, %4, 0;\n\t}" : "=r"(d) : "r"(r), "r"(lo), "r"(acc), "r"(one));
+    return d;
 }
 
+__device__ __forceinline__ uint32_t imad(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t d;
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+
+// Per-slot acceptance constants: lo[c] = 2^32 - thr[c] (mod 2^32) for the 7 sorted
+// non-trivial thresholds (code c = 2 n_u + (1-a)); the carry of r + lo[c] is C_c = [r >= thr[c]]
+// (a threshold of 0 cannot carry: its C_c = 1 is folded into the chain start constants).
+//   B3  = C_3 - 1                       all ones iff r <  thr[3]   (K2 = ~B3)
+//   Nn  = C_1 + C_5 - 1
+//   E   = C_0 + C_2 + C_4 + C_6 - 2
+//   K1m = B3 - Nn        = -(k bit 1),  K0m = Nn + B3 - E = -(k bit 0),  k = #{c : r >= thr[c]}
+// (exact because the thresholds are sorted: C_0 >= C_1 >= ... >= C_6).
+struct SlotK {
+    uint32_t lo[7];
+    uint32_t b3c, nc, ec;
+};
+
 // One word-site: count the unsatisfied bonds (n0 n1 n2), decide, return the accept word.
+// ALU pipe: 8 (count) + 7 (carries) + 3 (comparator) + 1 (n2 | g2, folded into the flip by the caller).
 __device__ __forceinline__ uint32_t accept_word(uint32_t u0, uint32_t u1, uint32_t u2, uint32_t u3, uint32_t u4,
-                                                uint32_t u5, uint32_t na, const uint32_t (&B)[7], uint32_t &n0,
-                                                uint32_t &n1, uint32_t &n2)
+                                                uint32_t u5, uint32_t na, uint32_t r, const SlotK &K, uint32_t one,
+                                                uint32_t mone, uint32_t &n0, uint32_t &n1, uint32_t &n2)
 {
     const uint32_t s0 = xor3(u0, u1, u2), c0 = maj3(u0, u1, u2);
     const uint32_t s1 = xor3(u3, u4, u5), c1 = maj3(u3, u4, u5);
@@ -69,11 +94,14 @@ __device__ __forceinline__ uint32_t accept_word(uint32_t u0, uint32_t u1, uint32
     const uint32_t k = s0 & s1;
     n1 = xor3(c0, c1, k);
     n2 = maj3(c0, c1, k);
-    const uint32_t nK0 = xor3(xor3(B[0], B[1], B[2]), xor3(B[3], B[4], B[5]), B[6]);
-    const uint32_t K1 = lop3<LUT_K1>(B[1], B[3], B[5]);
-    const uint32_t g0 = na | nK0;
-    const uint32_t g1 = lop3<LUT_GE>(n0, K1, g0);
-    const uint32_t g2 = lop3<LUT_MAJ>(n1, B[3], g1);            // GE(n1, K2, g1) with K2 = ~B3
+    const uint32_t B3 = cadd(r, K.lo[3], K.b3c, one);
+    const uint32_t Nn = cadd(r, K.lo[5], cadd(r, K.lo[1], K.nc, one), one);
+    const uint32_t E = cadd(r, K.lo[6], cadd(r, K.lo[4], cadd(r, K.lo[2], cadd(r, K.lo[0], K.ec, one), one), one), one);
+    const uint32_t K1m = imad(Nn, mone, B3);
+    const uint32_t K0m = imad(Nn, one, imad(E, mone, B3));
+    const uint32_t g0 = na | ~K0m;
+    const uint32_t g1 = lop3<LUT_GE>(n0, K1m, g0);
+    const uint32_t g2 = lop3<LUT_MAJ>(n1, B3, g1);             // GE(n1, K2, g1) with K2 = ~B3
     return n2 | g2;
 }
 
@@ -128,13 +156,13 @@ __device__ __forceinline__ void reduce4(const uint32_t *__restrict__ in, uint32_
     }
 }
 
-template <int P>
+template <int P, bool ENERGY>
 __device__ __forceinline__ void half_sweep_quad(uint32_t *__restrict__ Sa, const uint32_t *__restrict__ So, int slot,
                                                 int s_yp, int s_ym, int s_zp, int s_zm, const uint32_t (&JA)[4],
                                                 const uint32_t (&JB)[4], const uint32_t (&Jyp)[4],
                                                 const uint32_t (&Jym)[4], const uint32_t (&Jzp)[4],
-                                                const uint32_t (&Jzm)[4], const uint4 r4, const uint2 *__restrict__ thr_t,
-                                                uint32_t amask, bool want_energy, uint32_t *__restrict__ red)
+                                                const uint32_t (&Jzm)[4], const uint4 r4, const uint4 *__restrict__ thr_t,
+                                                uint32_t amask, uint32_t one, uint32_t mone, uint32_t *__restrict__ red)
 {
     const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[slot];
     const uint4 o0 = reinterpret_cast<const uint4 *>(So)[slot];
@@ -142,9 +170,13 @@ __device__ __forceinline__ void half_sweep_quad(uint32_t *__restrict__ Sa, const
     const uint4 oym = reinterpret_cast<const uint4 *>(So)[s_ym];
     const uint4 ozp = reinterpret_cast<const uint4 *>(So)[s_zp];
     const uint4 ozm = reinterpret_cast<const uint4 *>(So)[s_zm];
-    uint2 c64[7];
-#pragma unroll
-    for (int c = 0; c < 7; ++c) c64[c] = thr_t[c];
+    SlotK K;
+    {
+        const uint4 k0 = thr_t[0], k1 = thr_t[1], k2 = thr_t[2];
+        K.lo[0] = k0.x; K.lo[1] = k0.y; K.lo[2] = k0.z; K.lo[3] = k0.w;
+        K.lo[4] = k1.x; K.lo[5] = k1.y; K.lo[6] = k1.z; K.b3c = k1.w;
+        K.nc = k2.x; K.ec = k2.y;
+    }
     const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
     const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
     const uint32_t v0[4] = {o0.x, o0.y, o0.z, o0.w};
@@ -155,18 +187,16 @@ __device__ __forceinline__ void half_sweep_quad(uint32_t *__restrict__ Sa, const
     uint32_t out[4], w[4][3];
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
-        uint32_t B[7], n0, n1, n2;
-#pragma unroll
-        for (int c = 0; c < 7; ++c) B[c] = lt_mask8(rr[e], c64[c]);
+        uint32_t n0, n1, n2;
         const uint32_t acc = accept_word(xor3(s[e], v0[e], JA[e]), xor3(s[e], vB[e], JB[e]), xor3(s[e], vyp[e], Jyp[e]),
                                          xor3(s[e], vym[e], Jym[e]), xor3(s[e], vzp[e], Jzp[e]),
-                                         xor3(s[e], vzm[e], Jzm[e]), ~(s[e] ^ amask), B, n0, n1, n2);
+                                         xor3(s[e], vzm[e], Jzm[e]), ~(s[e] ^ amask), rr[e], K, one, mone, n0, n1, n2);
         out[e] = s[e] ^ acc;
         // post-flip unsatisfied count of this site: n if not flipped, 6 - n if flipped
         w[e][0] = n0;
         w[e][1] = n1;
         w[e][2] = n2;
-        if (want_energy) {
+        if (ENERGY) {
             // 6 - n: bit0 = n0; bit1 = 1 for n in {0,3,4}; bit2 = 1 for n in {0,1,2}
             const uint32_t f1 = (~n2 & ~(n1 ^ n0)) | (n2 & ~n1 & ~n0);
             const uint32_t f2 = ~n2 & ~(n1 & n0);
@@ -175,7 +205,7 @@ __device__ __forceinline__ void half_sweep_quad(uint32_t *__restrict__ Sa, const
         }
     }
     reinterpret_cast<uint4 *>(Sa)[slot] = make_uint4(out[0], out[1], out[2], out[3]);
-    if (want_energy) {
+    if (ENERGY) {
         uint32_t ab[4], cd[4], U[5];
         bs_sum<3>(w[0], w[1], ab);
         bs_sum<3>(w[2], w[3], cd);
@@ -198,6 +228,8 @@ __device__ __forceinline__ void half_sweep_quad(uint32_t *__restrict__ Sa, const
     }
 }
 
+// SPT = systems per thread (NT / G) when it is a compile-time constant (unrolled), 0 = run-time loop
+template <int SPT>
 __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ Ladder8Args A)
 {
     constexpr int N = 512, H = 256;
@@ -206,8 +238,8 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
     const int NT = d.NT;
     uint32_t *S = smem;                                    // [NT][2][64 slots][4]
     uint32_t *Jsm = S + NT * N;                            // [2][3][64 slots][4]
-    uint2 *thr = reinterpret_cast<uint2 *>(Jsm + 3 * N);   // [NT][8]
-    uint32_t *masks = reinterpret_cast<uint32_t *>(thr + NT * 8);     // [32]
+    uint4 *thr = reinterpret_cast<uint4 *>(Jsm + 3 * N);   // [NT][3] = SlotK: lo[7], b3c, nc, ec, 0, 0
+    uint32_t *masks = reinterpret_cast<uint32_t *>(thr + NT * 3);     // [32]
     // exchange scratch (allocated only when pt_every > 0); later stages alias dead earlier ones
     uint32_t *red0 = masks + 32;                           // [NT][9][64]   stage-1 planes
     uint32_t *red1 = red0 + NT * PW1 * 64;                 // [NT][13][16]
@@ -230,9 +262,16 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
         const int qq = i & 63, cd = i >> 6;
         reinterpret_cast<uint4 *>(Jsm)[cd * 64 + slot_of_row(qq & 7, qq >> 3)] = reinterpret_cast<const uint4 *>(gJ)[i];
     }
-    for (int i = tid; i < NT * 8; i += nthr) {
-        const int t = i >> 3, c = i & 7;
-        thr[i] = c < 7 ? A.tab[t].c64[c] : make_uint2(0u, 0u);
+    for (int t = tid; t < NT; t += nthr) {                 // acceptance constants (see SlotK)
+        uint32_t lo[7], zc[7];
+        for (int c = 0; c < 7; ++c) {
+            const uint2 v = A.tab[t].c64[c];               // (0 - thr) as 64 bits: hi = 0 only for thr = 0
+            lo[c] = v.x;
+            zc[c] = v.y == 0u ? 1u : 0u;
+        }
+        thr[t * 3 + 0] = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+        thr[t * 3 + 1] = make_uint4(lo[4], lo[5], lo[6], zc[3] - 1u);
+        thr[t * 3 + 2] = make_uint4(zc[1] + zc[5] - 1u, zc[0] + zc[2] + zc[4] + zc[6] - 2u, 0u, 0u);
     }
     __syncthreads();
 
@@ -279,18 +318,33 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
                     Jzm[0] = joz.x; Jzm[1] = joz.y; Jzm[2] = joz.z; Jzm[3] = joz.w;
                 }
                 const bool want_energy = pt_due && colour == 1;
-                uint4 r4 = philox_rk8((uint32_t)q, time, wglob, ctr3(3, a, g), A.rk);
-#pragma unroll 1
-                for (int t = g; t < NT; t += A.G) {
+                auto body = [&](int t, const uint4 r_cur) {
                     uint32_t *Sa = S + t * N + colour * H;
                     const uint32_t *So = S + t * N + (1 - colour) * H;
-                    const uint4 r_cur = r4;
-                    if (t + A.G < NT) r4 = philox_rk8((uint32_t)q, time, wglob, ctr3(3, a, t + A.G), A.rk);   // next system's draws
                     uint32_t *red = red0 + (size_t)t * PW1 * 64 + (pi * 32 + j);
-                    if (p) half_sweep_quad<1>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm, r_cur,
-                                              thr + t * 8, amask, want_energy, red);
-                    else   half_sweep_quad<0>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm, r_cur,
-                                              thr + t * 8, amask, want_energy, red);
+                    const uint4 *kt = thr + t * 3;
+                    if (want_energy) {
+                        if (p) half_sweep_quad<1, true>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
+                                                        r_cur, kt, amask, A.one, A.mone, red);
+                        else   half_sweep_quad<0, true>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
+                                                        r_cur, kt, amask, A.one, A.mone, red);
+                    } else {
+                        if (p) half_sweep_quad<1, false>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
+                                                         r_cur, kt, amask, A.one, A.mone, red);
+                        else   half_sweep_quad<0, false>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
+                                                         r_cur, kt, amask, A.one, A.mone, red);
+                    }
+                };
+                if constexpr (SPT > 0) {
+#pragma unroll 1
+                    for (int i = 0; i < SPT; ++i) {
+                        const int t = g + i * A.G;
+                        body(t, philox_rk8((uint32_t)q, time, wglob, ctr3(3, a, t), A.rk));
+                    }
+                } else {
+#pragma unroll 1
+                    for (int t = g; t < NT; t += A.G)
+                        body(t, philox_rk8((uint32_t)q, time, wglob, ctr3(3, a, t), A.rk));
                 }
                 // the two warps of this group share systems; other groups are independent
                 asm volatile("bar.sync %0, 64;" ::"r"(g + 1) : "memory");
@@ -366,7 +420,7 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
 // ------------------------------------------------------------------------------- host side
 static size_t ladder8_smem(int NT, bool with_pt)
 {
-    size_t b = (size_t)NT * 512 * 4 + 3 * 512 * 4 + (size_t)NT * 8 * sizeof(uint2) + 32 * 4;
+    size_t b = (size_t)NT * 512 * 4 + 3 * 512 * 4 + (size_t)NT * 3 * sizeof(uint4) + 32 * 4;
     if (with_pt) b += (size_t)NT * 4 * (PW1 * 64 + 13 * 16);
     return b;
 }
@@ -383,7 +437,11 @@ int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_swe
 {
     static bool configured = false;
     if (!configured) {
-        if (cudaFuncSetAttribute(k_ladder8_pmj, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess) return -1;
+        if (cudaFuncSetAttribute(k_ladder8_pmj<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess ||
+            cudaFuncSetAttribute(k_ladder8_pmj<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess ||
+            cudaFuncSetAttribute(k_ladder8_pmj<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess ||
+            cudaFuncSetAttribute(k_ladder8_pmj<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess)
+            return -1;
         configured = true;
     }
     const Dims &d = c->d;
@@ -408,7 +466,14 @@ int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_swe
     A.G = G;
     // whole-CTA phases assume complete warps; always launch 64*G threads (G <= 5 -> <= 320)
     const int threads = 64 * G;
-    k_ladder8_pmj<<<d.W * d.R, threads, ladder8_smem(d.NT, pt_every > 0), c->stream>>>(A);
+    A.one = 1u;
+    A.mone = 0xffffffffu;
+    const size_t smem = ladder8_smem(d.NT, pt_every > 0);
+    const int spt = d.NT % G == 0 ? d.NT / G : 0;
+    if (spt == 4) k_ladder8_pmj<4><<<d.W * d.R, threads, smem, c->stream>>>(A);
+    else if (spt == 2) k_ladder8_pmj<2><<<d.W * d.R, threads, smem, c->stream>>>(A);
+    else if (spt == 1) k_ladder8_pmj<1><<<d.W * d.R, threads, smem, c->stream>>>(A);
+    else k_ladder8_pmj<0><<<d.W * d.R, threads, smem, c->stream>>>(A);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
