@@ -185,8 +185,14 @@ int do_measure(sg_ctx *c, double *out)
     const Dims &d = c->d;
     for (int s0 = 0; s0 < d.n_samples; s0 += c->chunk_samples) {
         const int ns = std::min(c->chunk_samples, d.n_samples - s0);
-        c->launches += c->kind == SG_PMJ ? launch_hist_pmj(c, s0, ns) : launch_hist_gauss(c, s0, ns);
-        c->launches += launch_finalize(c, s0, ns, out != nullptr);
+        if (measure_fused_supported(c)) {
+            const int k = launch_measure_pmj(c, s0, ns, out != nullptr);
+            if (k < 0) return check_launch(c, "measure kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "measure kernel launch failed");
+            c->launches += k;
+        } else {
+            c->launches += c->kind == SG_PMJ ? launch_hist_pmj(c, s0, ns) : launch_hist_gauss(c, s0, ns);
+            c->launches += launch_finalize(c, s0, ns, out != nullptr);
+        }
         int rc = check_launch(c, "measure kernels");
         if (rc) return rc;
         if (out) {

@@ -89,6 +89,8 @@ int launch_pt_gauss(sg_ctx *c, uint64_t exchange);
 int launch_hist_pmj(sg_ctx *c, int s0, int ns);             // samples [s0, s0+ns) -> c->hist
 int launch_hist_gauss(sg_ctx *c, int s0, int ns);
 int launch_finalize(sg_ctx *c, int s0, int ns, bool want_rec);   // hist -> rec (optional), acc
+bool measure_fused_supported(const sg_ctx *c);             // bit-sliced one-launch measurement usable?
+int launch_measure_pmj(sg_ctx *c, int s0, int ns, bool want_rec);   // spins -> rec (optional), acc; -1 on error
 int launch_unpack_pmj(sg_ctx *c, int s0, int ns);           // spins -> stage8 (canonical bytes)
 int launch_pack_pmj(sg_ctx *c, int s0, int ns);             // stage8 -> spins (lanes of [s0, s0+ns))
 int launch_unpack_gauss(sg_ctx *c, int s0, int ns);

@@ -90,4 +90,280 @@ int launch_finalize(sg_ctx *c, int s0, int ns, bool want_rec)
     return 1;
 }
 
+
+// ------------------------------------------------------------------ fused bit-sliced measurement
+// k_measure_pmj<L>: one CTA per (packed word w, slot t) does everything of a6 + a7 for the 32
+// samples of the word: differing-site words D = S^a xor S^b of every replica pair in canonical
+// site order (shared memory) -> one thread per (pair, histogram bin) counts its L^2 words with a
+// carry-save adder network (bit-sliced: all 32 samples at once) -> one warp transpose per 4 (or 2)
+// bins turns the count planes into per-sample integers -> one thread per (pair, sample) does the
+// L-point transforms of R7/R8 in double (same arithmetic as k_finalize) -> one thread per
+// (sample, moment) adds into the accumulators of R9.
+//
+// A bin (histogram hh, value b) is the set of sites whose coordinate_hh equals b; it is walked as
+// L "outer" x L "inner" sites: idx = u*su + v*sv + ((ku*u + kb) mod L)*sd  (see bin_geometry).
+
+// carry-save adder: (carry, sum) of three one-bit planes
+__device__ __forceinline__ void csa(uint32_t &hi, uint32_t &lo, uint32_t a, uint32_t b, uint32_t c)
+{
+    lo = xor3(a, b, c);
+    hi = maj3(a, b, c);
+}
+
+template <int L>
+struct MeasureCfg {
+    static constexpr int N = L * L * L;
+    static constexpr int NB = N_HIST * L;                      // bins per pair
+    static constexpr int BPB = (L * L < 256) ? 8 : 16;         // bits per bin after the transpose
+    static constexpr int PER = 32 / BPB;                       // bins per transposed word
+    static constexpr int NG = (NB + PER - 1) / PER;            // 32-word transpose groups per pair
+    static constexpr int HI = BPB - 3;                         // planes above ones/twos/fours
+    static constexpr int PLW = NG * 32;                        // plane words per pair
+};
+
+struct BinGeom {
+    int su, sv, sd, ku, kb;
+};
+
+template <int L>
+__device__ __forceinline__ BinGeom bin_geometry(int hh, int b)
+{
+    constexpr int L2 = L * L;
+    BinGeom g;
+    switch (hh) {
+    case 0: g = {L, L2, 1, 0, b}; break;          // x = b;       outer y, inner z
+    case 1: g = {1, L2, L, 0, b}; break;          // y = b;       outer x, inner z
+    case 2: g = {1, L, L2, 0, b}; break;          // z = b;       outer x, inner y
+    case 3: g = {1, L2, L, -1, b}; break;         // x + y = b:   y = b - x; outer x, inner z
+    case 4: g = {1, L2, L, 1, -b}; break;         // x - y = b:   y = x - b
+    case 5: g = {1, L, L2, -1, b}; break;         // x + z = b:   z = b - x; outer x, inner y
+    case 6: g = {1, L, L2, 1, -b}; break;         // x - z = b:   z = x - b
+    case 7: g = {L, 1, L2, -1, b}; break;         // y + z = b:   z = b - y; outer y, inner x
+    default: g = {L, 1, L2, 1, -b}; break;        // y - z = b:   z = y - b
+    }
+    return g;
+}
+
+template <int L>
+__global__ void __launch_bounds__(256)
+k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restrict__ tw, int w0, int s0,
+              double *__restrict__ rec, double *__restrict__ acc)
+{
+    using C = MeasureCfg<L>;
+    constexpr int N = C::N, NB = C::NB, Lh = L / 2, H = N / 2;
+    extern __shared__ __align__(16) unsigned char sm_raw[];
+    const int P = d.P;
+    // region A: D words [P][N] during the counting phase, then records [P][SG_REC][32] doubles
+    uint32_t *Dsm = reinterpret_cast<uint32_t *>(sm_raw);
+    double *REC = reinterpret_cast<double *>(sm_raw);
+    const size_t regA = ((size_t)P * N * 4 > (size_t)P * SG_REC * 32 * 8) ? (size_t)P * N * 4 : (size_t)P * SG_REC * 32 * 8;
+    uint32_t *PL = reinterpret_cast<uint32_t *>(sm_raw + regA);          // [P][NG*32]
+    __shared__ int pa[6], pb[6];
+
+    const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
+    const int t = blockIdx.x % d.NT;
+    const int w = w0 + blockIdx.x / d.NT;
+    if (tid == 0) {
+        int p = 0;
+        for (int a = 0; a < d.R; ++a)
+            for (int b = a + 1; b < d.R; ++b) { pa[p] = a; pb[p] = b; ++p; }
+    }
+    __syncthreads();
+
+    // ---- phase 0: D = S^a xor S^b, canonical order
+    for (int item = tid; item < P * N; item += nthr) {
+        const int pair = item / N, k = item - pair * N;            // k = colour * H + n
+        const int c = k / H, n = k - c * H;
+        const int row = n / Lh, m = n - row * Lh;
+        const int z = row / L, y = row - z * L;
+        const int x = 2 * m + ((c + y + z) & 1);
+        const uint32_t *A = spins + (((size_t)w * d.R + pa[pair]) * d.NT + t) * N;
+        const uint32_t *B = spins + (((size_t)w * d.R + pb[pair]) * d.NT + t) * N;
+        Dsm[pair * N + x + L * (y + L * z)] = A[k] ^ B[k];
+    }
+    for (int i = tid; i < P * C::PLW; i += nthr) PL[i] = 0u;
+    __syncthreads();
+
+    // ---- phase 1: one thread per (pair, bin): bit-sliced count of its L^2 words
+    for (int item = tid; item < P * NB; item += nthr) {
+        const int pair = item / NB, bin = item - pair * NB;
+        const int hh = bin / L, b = bin - hh * L;
+        const BinGeom g = bin_geometry<L>(hh, b);
+        const uint32_t *Dp = Dsm + pair * N;
+        uint32_t ones = 0, twos = 0, fours = 0, hi[C::HI];
+#pragma unroll
+        for (int k = 0; k < C::HI; ++k) hi[k] = 0;
+#pragma unroll 1
+        for (int u = 0; u < L; ++u) {
+            int dd = (g.ku * u + g.kb) % L;
+            if (dd < 0) dd += L;
+            const uint32_t *base = Dp + u * g.su + dd * g.sd;
+#pragma unroll
+            for (int v0 = 0; v0 < L; v0 += 8) {
+                uint32_t x[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) x[j] = (v0 + j < L) ? base[(v0 + j) * g.sv] : 0u;
+                uint32_t tA, tB, fA, fB, e;
+                csa(tA, ones, ones, x[0], x[1]);
+                csa(tB, ones, ones, x[2], x[3]);
+                csa(fA, twos, twos, tA, tB);
+                csa(tA, ones, ones, x[4], x[5]);
+                csa(tB, ones, ones, x[6], x[7]);
+                csa(fB, twos, twos, tA, tB);
+                csa(e, fours, fours, fA, fB);
+                // ripple the weight-8 carry into the high planes
+#pragma unroll
+                for (int k = 0; k < C::HI; ++k) {
+                    const uint32_t hk = hi[k];
+                    hi[k] = hk ^ e;
+                    e = hk & e;
+                }
+            }
+        }
+        uint32_t *out = PL + pair * C::PLW + (bin / C::PER) * 32 + (bin % C::PER) * C::BPB;
+        out[0] = ones;
+        out[1] = twos;
+        out[2] = fours;
+#pragma unroll
+        for (int k = 0; k < C::HI; ++k) out[3 + k] = hi[k];
+    }
+    __syncthreads();
+
+    // ---- phase 2: one warp transpose per group: lane l receives the counts of sample 32 w + l
+    for (int item = warp; item < P * C::NG; item += nwarp) {
+        uint32_t *grp = PL + item * 32;
+        const uint32_t v = transpose32(grp[lane], lane);
+        __syncwarp();
+        grp[lane] = v;
+    }
+    __syncthreads();
+
+    // ---- phase 3: one thread per (pair, sample): records (same arithmetic as k_finalize)
+    const double invN = 1.0 / (double)N;
+    for (int item = tid; item < P * 32; item += nthr) {
+        const int pair = item >> 5, l = item & 31;
+        const uint32_t *cw = PL + pair * C::PLW + l;
+        auto cnt = [&](int bin) -> int {
+            const uint32_t wv = cw[(bin / C::PER) * 32];
+            return (int)((wv >> ((bin % C::PER) * C::BPB)) & ((1u << C::BPB) - 1u));
+        };
+        double *r = REC + (size_t)pair * SG_REC * 32 + l;         // r[j * 32]
+        // REC aliases Dsm (dead since the barrier after phase 1); PL is a separate region
+        int D0 = 0;
+        for (int m = 0; m < L; ++m) D0 += cnt(m);
+        r[0] = (double)(N - 2 * D0) * invN;
+        const double *cosv = tw, *sinv = tw + L;
+#pragma unroll 1
+        for (int k = 0; k < SG_NK; ++k) {
+            const int hh = k < 6 ? k % 3 : k - 3;
+            const int mul = (k >= 3 && k < 6) ? 2 : 1;
+            double re = 0.0, im = 0.0;
+            int idx = 0;
+            for (int m = 0; m < L; ++m) {
+                const double v = (double)(L * L - 2 * cnt(hh * L + m));
+                re += v * cosv[idx];
+                im += v * sinv[idx];
+                idx += mul;
+                if (idx >= L) idx -= L;
+            }
+            r[(1 + 2 * k) * 32] = re * invN;
+            r[(2 + 2 * k) * 32] = im * invN;
+        }
+    }
+    __syncthreads();
+
+    // ---- optional record output: rec[(s - s0)][t][pair][j]
+    if (rec) {
+        for (int item = tid; item < 32 * P * SG_REC; item += nthr) {
+            const int l = item / (P * SG_REC), rest = item - l * (P * SG_REC);
+            const int pair = rest / SG_REC, j = rest - pair * SG_REC;
+            const int sl = w * 32 + l - s0;
+            rec[(((size_t)sl * d.NT + t) * P + pair) * SG_REC + j] = REC[((size_t)pair * SG_REC + j) * 32 + l];
+        }
+    }
+
+    // ---- phase 4: one thread per (sample, moment)
+    for (int item = tid; item < 32 * SG_NMOM; item += nthr) {
+        const int l = item / SG_NMOM, j = item - l * SG_NMOM;
+        const int s = w * 32 + l;
+        if (s >= d.n_samples) continue;
+        const double *R0 = REC + l;
+        auto rr = [&](int pair, int jj) -> double { return R0[((size_t)pair * SG_REC + jj) * 32]; };
+        double sum = 0.0;
+        if (j < 4) {
+            for (int p = 0; p < P; ++p) {
+                const double v = rr(p, 0);
+                sum += j == 0 ? v : j == 1 ? v * v : j == 2 ? v * v * v : (v * v) * (v * v);
+            }
+        } else {
+            int k, cc;                             // k = -1: the k = 0 cross terms [64], [65]
+            if (j >= 64) { k = -1; cc = j - 64 + 3; }
+            else { k = (j - 4) / 5; cc = (j - 4) - 5 * k; }
+            const int jre = k < 0 ? 0 : 1 + 2 * k, jim = jre + 1;
+            if (cc < 3) {
+                for (int p = 0; p < P; ++p) {
+                    const double re = rr(p, jre), im = rr(p, jim);
+                    sum += cc == 0 ? re : cc == 1 ? im : re * re + im * im;
+                }
+            } else {
+                const int want_shared = cc == 3 ? 1 : 0;
+                for (int p = 0; p < P; ++p)
+                    for (int p2 = p + 1; p2 < P; ++p2) {
+                        const int shared = (pa[p] == pa[p2]) + (pa[p] == pb[p2]) + (pb[p] == pa[p2]) + (pb[p] == pb[p2]);
+                        if (shared != want_shared) continue;
+                        if (k < 0) sum += rr(p, 0) * rr(p2, 0);
+                        else sum += rr(p, jre) * rr(p2, jre) + rr(p, jim) * rr(p2, jim);
+                    }
+            }
+        }
+        double *A = acc + ((size_t)s * d.NT + t) * SG_NMOM + j;
+        *A += sum;
+    }
+}
+
+template <int L>
+static size_t measure_smem(int P)
+{
+    using C = MeasureCfg<L>;
+    const size_t a = (size_t)P * C::N * 4, b = (size_t)P * SG_REC * 32 * 8;
+    return (a > b ? a : b) + (size_t)P * C::PLW * 4;
+}
+
+template <int L>
+static int launch_measure_L(sg_ctx *c, int s0, int ns, bool want_rec)
+{
+    const Dims &d = c->d;
+    const size_t smem = measure_smem<L>(d.P);
+    static bool configured = false;
+    if (!configured) {
+        if (cudaFuncSetAttribute(k_measure_pmj<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)measure_smem<L>(6)) != cudaSuccess)
+            return -1;
+        configured = true;
+    }
+    const int w0 = s0 >> 5, nw = (ns + 31) >> 5;
+    k_measure_pmj<L><<<(unsigned)(nw * d.NT), 256, smem, c->stream>>>(d, c->spins, c->twiddle, w0, s0,
+                                                                      want_rec ? c->rec : nullptr, c->acc);
+    return 1;
+}
+
+bool measure_fused_supported(const sg_ctx *c)
+{
+    const int L = c->d.L;
+    return c->kind == SG_PMJ && (L == 4 || L == 6 || L == 8 || L == 10 || L == 12 || L == 16);
+}
+
+// samples [s0, s0+ns), s0 a multiple of 32: records (optional) and accumulators in one launch
+int launch_measure_pmj(sg_ctx *c, int s0, int ns, bool want_rec)
+{
+    switch (c->d.L) {
+    case 4: return launch_measure_L<4>(c, s0, ns, want_rec);
+    case 6: return launch_measure_L<6>(c, s0, ns, want_rec);
+    case 8: return launch_measure_L<8>(c, s0, ns, want_rec);
+    case 10: return launch_measure_L<10>(c, s0, ns, want_rec);
+    case 12: return launch_measure_L<12>(c, s0, ns, want_rec);
+    case 16: return launch_measure_L<16>(c, s0, ns, want_rec);
+    default: return -1;
+    }
+}
+
 }  // namespace sg

@@ -59,6 +59,8 @@ CASES = [
     ("L8", 8, 0.2, 64, 4, 6, (0.5, 2.0), 0, 2, [0, 13, 31, 63]),
     ("L12", 12, 0.1, 32, 4, 3, (0.4, 1.8), 0, 3, [0, 31]),
     ("L8-neg-h", 8, -0.7, 32, 2, 4, (0.6, 1.5), 0, 4, [3, 30]),
+    ("L10", 10, 0.1, 34, 4, 3, (0.5, 1.8), 0, 13, [0, 33]),
+    ("L16-pmj", 16, 0.2, 32, 2, 3, (0.5, 1.8), 0, 14, [5, 31]),
     ("L4-h0", 4, 0.0, 32, 2, 4, (0.5, 2.0), 0, 5, [1, 2]),
     ("L4-big-h-general-path", 4, 1.7, 32, 2, 4, (0.5, 3.0), 0, 6, [7, 8]),
     ("L4-huge-h", 4, 5.0, 32, 2, 3, (0.5, 3.0), 0, 7, [0, 9]),
