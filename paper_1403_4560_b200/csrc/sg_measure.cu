@@ -158,7 +158,7 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
     double *REC = reinterpret_cast<double *>(sm_raw);
     const size_t regA = ((size_t)P * N * 4 > (size_t)P * SG_REC * 32 * 8) ? (size_t)P * N * 4 : (size_t)P * SG_REC * 32 * 8;
     uint32_t *PL = reinterpret_cast<uint32_t *>(sm_raw + regA);          // [P][NG*32]
-    __shared__ int pa[6], pb[6];
+    __shared__ int pa[6], pb[6], couples[15], n_couples;      // couples: p | p2 << 4 | shared << 8
 
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
     const int t = blockIdx.x % d.NT;
@@ -167,6 +167,13 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
         int p = 0;
         for (int a = 0; a < d.R; ++a)
             for (int b = a + 1; b < d.R; ++b) { pa[p] = a; pb[p] = b; ++p; }
+        int q = 0;
+        for (int p1 = 0; p1 < p; ++p1)
+            for (int p2 = p1 + 1; p2 < p; ++p2) {
+                const int shared = (pa[p1] == pa[p2]) + (pa[p1] == pb[p2]) + (pb[p1] == pa[p2]) + (pb[p1] == pb[p2]);
+                couples[q++] = p1 | (p2 << 4) | (shared << 8);
+            }
+        n_couples = q;
     }
     __syncthreads();
 
@@ -282,13 +289,16 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
         }
     }
 
-    // ---- phase 4: one thread per (sample, moment)
+    // ---- phase 4: one thread per (moment j, sample l), l fastest: j is warp-uniform (no divergence,
+    // conflict-free record reads); the sums are staged in shared memory (OUT aliases the plane words,
+    // dead since phase 3) and added to the accumulators in coalesced 528-byte runs.
+    double *OUT = reinterpret_cast<double *>(PL);                       // [32][OUT_LD]
+    constexpr int OUT_LD = SG_NMOM + 1;
+    __syncthreads();
     for (int item = tid; item < 32 * SG_NMOM; item += nthr) {
-        const int l = item / SG_NMOM, j = item - l * SG_NMOM;
-        const int s = w * 32 + l;
-        if (s >= d.n_samples) continue;
+        const int j = item >> 5, l = item & 31;
         const double *R0 = REC + l;
-        auto rr = [&](int pair, int jj) -> double { return R0[((size_t)pair * SG_REC + jj) * 32]; };
+        auto rr = [&](int pair, int jj) -> double { return R0[(pair * SG_REC + jj) * 32]; };
         double sum = 0.0;
         if (j < 4) {
             for (int p = 0; p < P; ++p) {
@@ -307,17 +317,24 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
                 }
             } else {
                 const int want_shared = cc == 3 ? 1 : 0;
-                for (int p = 0; p < P; ++p)
-                    for (int p2 = p + 1; p2 < P; ++p2) {
-                        const int shared = (pa[p] == pa[p2]) + (pa[p] == pb[p2]) + (pb[p] == pa[p2]) + (pb[p] == pb[p2]);
-                        if (shared != want_shared) continue;
-                        if (k < 0) sum += rr(p, 0) * rr(p2, 0);
-                        else sum += rr(p, jre) * rr(p2, jre) + rr(p, jim) * rr(p2, jim);
-                    }
+                for (int q = 0; q < n_couples; ++q) {
+                    const int cp = couples[q];
+                    if ((cp >> 8) != want_shared) continue;
+                    const int p = cp & 15, p2 = (cp >> 4) & 15;
+                    if (k < 0) sum += rr(p, 0) * rr(p2, 0);
+                    else sum += rr(p, jre) * rr(p2, jre) + rr(p, jim) * rr(p2, jim);
+                }
             }
         }
+        OUT[l * OUT_LD + j] = sum;
+    }
+    __syncthreads();
+    for (int item = tid; item < 32 * SG_NMOM; item += nthr) {
+        const int l = item / SG_NMOM, j = item - l * SG_NMOM;
+        const int s = w * 32 + l;
+        if (s >= d.n_samples) continue;
         double *A = acc + ((size_t)s * d.NT + t) * SG_NMOM + j;
-        *A += sum;
+        *A += OUT[l * OUT_LD + j];
     }
 }
 
@@ -326,7 +343,8 @@ static size_t measure_smem(int P)
 {
     using C = MeasureCfg<L>;
     const size_t a = (size_t)P * C::N * 4, b = (size_t)P * SG_REC * 32 * 8;
-    return (a > b ? a : b) + (size_t)P * C::PLW * 4;
+    const size_t pl = (size_t)P * C::PLW * 4, out = (size_t)32 * (SG_NMOM + 1) * 8;
+    return (a > b ? a : b) + (pl > out ? pl : out);
 }
 
 template <int L>
