@@ -110,6 +110,14 @@ __device__ __forceinline__ void csa(uint32_t &hi, uint32_t &lo, uint32_t a, uint
     hi = maj3(a, b, c);
 }
 
+// replica pairs in the order (0,1),(0,2),(0,3),(1,2),(1,3),(2,3) (for R = 2 only pair 0 exists):
+// do pairs p and p2 share exactly one replica?
+__host__ __device__ constexpr bool pairs_share(int p, int p2)
+{
+    constexpr int A[6] = {0, 0, 0, 1, 1, 2}, B[6] = {1, 2, 3, 2, 3, 3};
+    return (A[p] == A[p2]) + (A[p] == B[p2]) + (B[p] == A[p2]) + (B[p] == B[p2]) == 1;
+}
+
 template <int L>
 struct MeasureCfg {
     static constexpr int N = L * L * L;
@@ -158,6 +166,7 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
     double *REC = reinterpret_cast<double *>(sm_raw);
     const size_t regA = ((size_t)P * N * 4 > (size_t)P * SG_REC * 32 * 8) ? (size_t)P * N * 4 : (size_t)P * SG_REC * 32 * 8;
     uint32_t *PL = reinterpret_cast<uint32_t *>(sm_raw + regA);          // [P][NG*32]
+    __shared__ double twsm[2 * L];
     __shared__ int pa[6], pb[6], couples[15], n_couples;      // couples: p | p2 << 4 | shared << 8
 
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
@@ -175,6 +184,7 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
             }
         n_couples = q;
     }
+    if (tid < 2 * L) twsm[tid] = tw[tid];
     __syncthreads();
 
     // ---- phase 0: D = S^a xor S^b, canonical order
@@ -256,25 +266,39 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
         };
         double *r = REC + (size_t)pair * SG_REC * 32 + l;         // r[j * 32]
         // REC aliases Dsm (dead since the barrier after phase 1); PL is a separate region
-        int D0 = 0;
-        for (int m = 0; m < L; ++m) D0 += cnt(m);
-        r[0] = (double)(N - 2 * D0) * invN;
-        const double *cosv = tw, *sinv = tw + L;
+        // per histogram: counts -> plane sums v[m] = L^2 - 2 cnt (registers), then the harmonics that
+        // use it (x, y, z: harmonics 1 and 2 = K0-2, K3-5; diagonals: harmonic 1 = K6-11)
+        const double *cosv = twsm, *sinv = twsm + L;
 #pragma unroll 1
-        for (int k = 0; k < SG_NK; ++k) {
-            const int hh = k < 6 ? k % 3 : k - 3;
-            const int mul = (k >= 3 && k < 6) ? 2 : 1;
-            double re = 0.0, im = 0.0;
-            int idx = 0;
+        for (int hh = 0; hh < N_HIST; ++hh) {
+            double v[L];
+            int tot = 0;
+#pragma unroll
             for (int m = 0; m < L; ++m) {
-                const double v = (double)(L * L - 2 * cnt(hh * L + m));
-                re += v * cosv[idx];
-                im += v * sinv[idx];
-                idx += mul;
-                if (idx >= L) idx -= L;
+                const int cm = cnt(hh * L + m);
+                tot += cm;
+                v[m] = (double)(L * L - 2 * cm);
             }
-            r[(1 + 2 * k) * 32] = re * invN;
-            r[(2 + 2 * k) * 32] = im * invN;
+            if (hh == 0) r[0] = (double)(N - 2 * tot) * invN;
+            double re = 0.0, im = 0.0;
+#pragma unroll
+            for (int m = 0; m < L; ++m) {
+                re += v[m] * cosv[m];
+                im += v[m] * sinv[m];
+            }
+            const int k1 = hh < 3 ? hh : hh + 3;
+            r[(1 + 2 * k1) * 32] = re * invN;
+            r[(2 + 2 * k1) * 32] = im * invN;
+            if (hh < 3) {
+                double re2 = 0.0, im2 = 0.0;
+#pragma unroll
+                for (int m = 0; m < L; ++m) {
+                    re2 += v[m] * cosv[(2 * m) % L];
+                    im2 += v[m] * sinv[(2 * m) % L];
+                }
+                r[(1 + 2 * (hh + 3)) * 32] = re2 * invN;
+                r[(2 + 2 * (hh + 3)) * 32] = im2 * invN;
+            }
         }
     }
     __syncthreads();
@@ -295,38 +319,55 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
     double *OUT = reinterpret_cast<double *>(PL);                       // [32][OUT_LD]
     constexpr int OUT_LD = SG_NMOM + 1;
     __syncthreads();
-    for (int item = tid; item < 32 * SG_NMOM; item += nthr) {
-        const int j = item >> 5, l = item & 31;
+    // item = (block kb, sample l): kb < 12: the five moments of wave vector K_kb; kb = 12: q(0) moments
+    for (int item = tid; item < 13 * 32; item += nthr) {
+        const int kb = item >> 5, l = item & 31;
         const double *R0 = REC + l;
-        auto rr = [&](int pair, int jj) -> double { return R0[(pair * SG_REC + jj) * 32]; };
-        double sum = 0.0;
-        if (j < 4) {
-            for (int p = 0; p < P; ++p) {
-                const double v = rr(p, 0);
-                sum += j == 0 ? v : j == 1 ? v * v : j == 2 ? v * v * v : (v * v) * (v * v);
+        double *o = OUT + l * OUT_LD;
+        if (kb == 12) {
+            double v[6], s1 = 0.0, s2 = 0.0, s3 = 0.0, s4 = 0.0;
+#pragma unroll
+            for (int p = 0; p < 6; ++p) {
+                v[p] = 0.0;
+                if (p < P) {
+                    v[p] = R0[(p * SG_REC) * 32];
+                    const double vv = v[p];
+                    s1 += vv; s2 += vv * vv; s3 += vv * vv * vv; s4 += (vv * vv) * (vv * vv);
+                }
             }
+            double c1 = 0.0, c0 = 0.0;
+#pragma unroll
+            for (int p = 0; p < 6; ++p)
+#pragma unroll
+                for (int p2 = p + 1; p2 < 6; ++p2)
+                    if (p2 < P) {
+                        const double pr = v[p] * v[p2];
+                        if (pairs_share(p, p2)) c1 += pr; else c0 += pr;
+                    }
+            o[0] = s1; o[1] = s2; o[2] = s3; o[3] = s4; o[64] = c1; o[65] = c0;
         } else {
-            int k, cc;                             // k = -1: the k = 0 cross terms [64], [65]
-            if (j >= 64) { k = -1; cc = j - 64 + 3; }
-            else { k = (j - 4) / 5; cc = (j - 4) - 5 * k; }
-            const int jre = k < 0 ? 0 : 1 + 2 * k, jim = jre + 1;
-            if (cc < 3) {
-                for (int p = 0; p < P; ++p) {
-                    const double re = rr(p, jre), im = rr(p, jim);
-                    sum += cc == 0 ? re : cc == 1 ? im : re * re + im * im;
-                }
-            } else {
-                const int want_shared = cc == 3 ? 1 : 0;
-                for (int q = 0; q < n_couples; ++q) {
-                    const int cp = couples[q];
-                    if ((cp >> 8) != want_shared) continue;
-                    const int p = cp & 15, p2 = (cp >> 4) & 15;
-                    if (k < 0) sum += rr(p, 0) * rr(p2, 0);
-                    else sum += rr(p, jre) * rr(p2, jre) + rr(p, jim) * rr(p2, jim);
+            double re[6], im[6], sr = 0.0, si = 0.0, sa = 0.0;
+#pragma unroll
+            for (int p = 0; p < 6; ++p) {
+                re[p] = im[p] = 0.0;
+                if (p < P) {
+                    re[p] = R0[(p * SG_REC + 1 + 2 * kb) * 32];
+                    im[p] = R0[(p * SG_REC + 2 + 2 * kb) * 32];
+                    sr += re[p]; si += im[p]; sa += re[p] * re[p] + im[p] * im[p];
                 }
             }
+            double c1 = 0.0, c0 = 0.0;
+#pragma unroll
+            for (int p = 0; p < 6; ++p)
+#pragma unroll
+                for (int p2 = p + 1; p2 < 6; ++p2)
+                    if (p2 < P) {
+                        const double pr = re[p] * re[p2] + im[p] * im[p2];
+                        if (pairs_share(p, p2)) c1 += pr; else c0 += pr;
+                    }
+            double *ok = o + 4 + 5 * kb;
+            ok[0] = sr; ok[1] = si; ok[2] = sa; ok[3] = c1; ok[4] = c0;
         }
-        OUT[l * OUT_LD + j] = sum;
     }
     __syncthreads();
     for (int item = tid; item < 32 * SG_NMOM; item += nthr) {
