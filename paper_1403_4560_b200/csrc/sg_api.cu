@@ -167,10 +167,10 @@ int do_reset(sg_ctx *c)
     return check_launch(c, "init kernels");
 }
 
-int do_exchange(sg_ctx *c)
+int do_exchange(sg_ctx *c, bool energies_fresh = false)
 {
     if (c->kind == SG_PMJ) {
-        c->launches += launch_energy_pmj(c);
+        if (!energies_fresh) c->launches += launch_energy_pmj(c);
         c->launches += launch_pt_pmj(c, c->exchanges);
     } else {
         c->launches += launch_energy_gauss(c);
@@ -209,9 +209,19 @@ int do_measure(sg_ctx *c, double *out)
 }
 
 // n consecutive sweeps with nothing in between
-int do_sweeps(sg_ctx *c, int n)
+// (energy_after: the caller runs an exchange next; *fresh is set if the kernel left U, M up to date)
+int do_sweeps(sg_ctx *c, int n, bool energy_after = false, bool *fresh = nullptr)
 {
+    if (fresh) *fresh = false;
     if (n <= 0) return SG_OK;
+    if (res32_supported(c)) {
+        const int k = launch_res32_pmj(c, c->sweeps, n, energy_after);
+        if (k < 0) return check_launch(c, "res32 kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "res32 kernel launch failed");
+        c->launches += k;
+        c->sweeps += n;
+        if (fresh) *fresh = energy_after;
+        return SG_OK;
+    }
     if (ladder8_supported(c)) {
         const int k = launch_ladder8_pmj(c, c->sweeps, c->exchanges, n, 0);
         if (k < 0) return check_launch(c, "ladder8 kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "ladder8 kernel launch failed");
@@ -382,10 +392,12 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
         if (pt_every > 0) run = std::min<uint64_t>(run, (uint64_t)pt_every - c->sweeps % (uint64_t)pt_every);
         if (meas_every > 0) run = std::min<uint64_t>(run, (uint64_t)meas_every - c->sweeps % (uint64_t)meas_every);
         int rc;
-        if ((rc = do_sweeps(c, (int)run))) return rc;
+        const bool pt_due = pt_every > 0 && (c->sweeps + run) % (uint64_t)pt_every == 0;
+        bool fresh = false;
+        if ((rc = do_sweeps(c, (int)run, pt_due, &fresh))) return rc;
         left -= (int)run;
-        if (pt_every > 0 && c->sweeps % (uint64_t)pt_every == 0)
-            if ((rc = do_exchange(c))) return rc;
+        if (pt_due)
+            if ((rc = do_exchange(c, fresh))) return rc;
         if (meas_every > 0 && c->sweeps % (uint64_t)meas_every == 0)
             if ((rc = do_measure(c, nullptr))) return rc;
     }

@@ -82,6 +82,8 @@ bool ladder_supported(const sg_ctx *c);                    // shared-memory-resi
 int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps);   // n consecutive sweeps, 1 launch (-1 on error)
 bool ladder8_supported(const sg_ctx *c);                   // L = 8 kernel with fused parallel tempering
 int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_sweeps, int pt_every);
+bool res32_supported(const sg_ctx *c);                     // L = 32: one system resident per SM, couplings streamed from L2
+int launch_res32_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, bool want_energy);   // 1 launch (-1 on error)
 int launch_energy_pmj(sg_ctx *c);
 int launch_energy_gauss(sg_ctx *c);
 int launch_pt_pmj(sg_ctx *c, uint64_t exchange);            // decide + swap (energies must be fresh)

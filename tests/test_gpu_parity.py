@@ -236,3 +236,26 @@ def test_l8_fused_ladder_with_pt(sg, O, h, NT, R, pt_every, n_samples):
         o.sweep(1); o.pt_exchange(); o.run(5, pt_every, 0)
     check_state(sim, orc, "fused L8 + primitives")
     sim.close()
+
+
+@pytest.mark.parametrize("h,NT,R,pt_every,n_samples", [(0.2, 4, 4, 4, 33), (-0.3, 3, 2, 1, 32), (0.0, 2, 2, 3, 64)])
+def test_l32_resident_kernel_with_pt(sg, O, h, NT, R, pt_every, n_samples):
+    """The L=32 kernel (one system resident in shared memory, couplings streamed, energies for the
+    exchange step produced in the last colour-1 half sweep) vs the oracle: sg_run with exchanges falling
+    inside and at the end, then primitives (sg_sweep + separate energy kernel) from the same state."""
+    temps = W.ladder(0.4, 2.0, NT)
+    samples = sorted({0, 13, n_samples - 1})
+    sim, orc = make_pair(sg, O, 32, h, n_samples, R, temps, 0, 5, samples)
+    sim.sg_run(10, pt_every, 0)
+    for o in orc.values():
+        o.run(10, pt_every, 0)
+    check_state(sim, orc, "resident L32")
+    assert sim.sg_get_counters() == (10, 10 // pt_every)
+    sim.sg_sweep(3); sim.sg_pt_exchange(); sim.sg_run(2, pt_every, 0)
+    for o in orc.values():
+        o.sweep(3); o.pt_exchange(); o.run(2, pt_every, 0)
+    check_state(sim, orc, "resident L32 + primitives")
+    rec = sim.sg_measure()
+    for s, o in orc.items():
+        assert close(rec[s], o.measure())
+    sim.close()
