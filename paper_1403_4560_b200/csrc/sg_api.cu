@@ -22,7 +22,7 @@ constexpr int DEXP64_N = 5761, DEXP32_N = 1441;
 inline size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-    size_t spins, J, tab, exp64, exp32, tw, U, M, swap, acc, hist, rec, stage, total;
+    size_t spins, J, Jp, tab, exp64, exp32, tw, U, M, swap, acc, hist, rec, stage, total;
     int chunk_meas, chunk_stage, S_pad;
 };
 
@@ -48,7 +48,9 @@ Layout make_layout(int L, int n_samples, int R, int NT, int kind)
     if (kind == SG_PMJ) {
         lo.spins = take((size_t)W * R * NT * N * 4);
         lo.J = take((size_t)W * 3 * N * 4);
+        lo.Jp = L == 32 ? take(res32_packed_bytes(W)) : 0;
     } else {
+        lo.Jp = 0;
         lo.spins = take((size_t)n_samples * R * NT * N);
         lo.J = take((size_t)n_samples * 3 * N * 4);
     }
@@ -162,6 +164,7 @@ int do_reset(sg_ctx *c)
     int rc;
     if ((rc = check_cuda(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * (size_t)d.n_samples * d.NT * SG_NMOM, c->stream), "zero acc"))) return rc;
     c->launches += c->kind == SG_PMJ ? launch_init_pmj(c) : launch_init_gauss(c);
+    if (res32_supported(c)) c->launches += launch_pack_J_res32(c);
     c->sweeps = c->exchanges = 0;
     c->n_meas = 0;
     return check_launch(c, "init kernels");
@@ -304,6 +307,7 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     c->spins8 = (int8_t *)(b + lo.spins);
     c->J = (uint32_t *)(b + lo.J);
     c->Jg = (float *)(b + lo.J);
+    c->Jp = (coupling_kind == SG_PMJ && L == 32) ? (uint4 *)(b + lo.Jp) : nullptr;
     c->tab = (SlotTab *)(b + lo.tab);
     c->exp64_tab = (double *)(b + lo.exp64);
     c->exp32_tab = (float *)(b + lo.exp32);

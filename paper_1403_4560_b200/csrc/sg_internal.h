@@ -55,6 +55,7 @@ struct sg_ctx {
     bool own_ws;
     uint32_t *spins;                    // PMJ: [W][R][NT][2][H] colour-compacted words
     uint32_t *J;                        // PMJ: [W][2][3][H]
+    uint4 *Jp;                          // PMJ, L = 32: couplings repacked per warp step for k_res32_pmj (else NULL)
     int8_t *spins8;                     // GAUSS: [S][R][NT][2][H] colour-compacted bytes
     float *Jg;                          // GAUSS: [S][2][3][H]
     sg::SlotTab *tab;                   // [NT]
@@ -83,6 +84,8 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps);   // n consecut
 bool ladder8_supported(const sg_ctx *c);                   // L = 8 kernel with fused parallel tempering
 int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_sweeps, int pt_every);
 bool res32_supported(const sg_ctx *c);                     // L = 32: one system resident per SM, couplings streamed from L2
+size_t res32_packed_bytes(int W);
+int launch_pack_J_res32(sg_ctx *c);                        // J -> Jp
 int launch_res32_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, bool want_energy);   // 1 launch (-1 on error)
 int launch_energy_pmj(sg_ctx *c);
 int launch_energy_gauss(sg_ctx *c);

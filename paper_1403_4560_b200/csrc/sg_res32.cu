@@ -19,13 +19,14 @@
 #include "sg_device.cuh"
 #include "sg_internal.h"
 
+#include <type_traits>
+
 namespace sg {
 
 struct Res32Args {
     Dims d;
     uint32_t *spins;
-    const uint32_t *J;
-    const SlotTab *tab;
+    const uint4 *Jp;          // packed couplings (k_pack_J_res32)
     int64_t *U;
     int32_t *M;
     uint32_t rk[20];
@@ -33,6 +34,7 @@ struct Res32Args {
     int n_sweeps;
     int want_energy;          // write U, M of the final state
     uint32_t one, mone;
+    uint32_t kc[MAX_NT][10];  // per slot: SlotK (lo[7], b3c, nc, ec); read through the constant bank with a uniform index
 };
 
 namespace {
@@ -40,47 +42,84 @@ namespace {
 constexpr int RL = 32, RN = RL * RL * RL, RH = RN / 2, RQ = RH / 4;   // 4096 quads per colour
 constexpr int R_THREADS = 512, R_WARPS = R_THREADS / 32, R_ITERS = RQ / R_THREADS;   // 8 quads per thread and half sweep
 
+// Couplings as the kernel consumes them ("packed" copy, built once per reset by k_pack_J_res32):
+// Jp[w][colour][Z][warp&7][6][32 lanes] uint4 — for every warp step (colour, plane pair Z, row block)
+// the six 4-word sets of each lane's quad, already in the order the update uses them
+//   0: bond to the x-neighbour at the same compact m      1: bond to the other x-neighbour (m+1 / m-1)
+//   2: +y (own)   3: -y (owned by row y-1)   4: +z (own)   5: -z (owned by row z-1)
+// = one contiguous 3 KB chunk per warp step, fetched by ONE bulk-async copy (TMA) into the warp's own
+// two-stage ring in shared memory; completion is tracked by an mbarrier per (warp, stage).
+constexpr int CHUNK_U4 = 6 * 32, CHUNK_BYTES = CHUNK_U4 * 16;              // 3072 B
+constexpr int CHUNKS_PER_WORD = 2 * 16 * 8;                                // colour, Z, row block
+constexpr int N_STAGES = 2;
+
 struct Quad6 {
-    uint4 x, y, z, ox, oy, oz;     // own +x +y +z bonds; other colour's +x (same row), +y (row y-1), +z (row z-1)
+    uint4 a, b, yp, ym, zp, zm;
 };
 
+// A thread's quad inside a z-plane pair is fixed for the whole launch (y, which row of the diagonal
+// pair, quad within the row); only the plane pair Z = 0..15 changes from step to step.
 struct Geo32 {
-    int q, q_yp, q_ym, q_zp, q_zm;  // uint4 indices inside one colour array
-    int p;
+    int qbase;                      // uint4 index of the quad for Z = 0 inside one colour array
+    int dyp, dym;                   // index deltas to the rows y+1, y-1 (periodic)
 };
 
-// task (0..127) of a warp and lane -> quad and its neighbour rows
-__device__ __forceinline__ Geo32 geo_of(int task, int lane, int colour)
+struct Quad32 {
+    int q, q_yp, q_ym, q_zp, q_zm;  // uint4 indices inside one colour array
+};
+
+__device__ __forceinline__ Geo32 geo_of(int wj, int lane)
 {
-    const int Z = task >> 3, pi = (task >> 2) & 1, j = task & 3;
+    const int pi = (wj >> 2) & 1, j = wj & 3;
     const int jj = lane >> 3, dd = (lane >> 2) & 1, m4 = lane & 3;
-    const int y = (2 * (4 * j + jj) + pi + dd) & 31, z = 2 * Z + dd;
+    const int y = (2 * (4 * j + jj) + pi + dd) & 31;
     Geo32 g;
-    g.p = (colour + pi) & 1;
-    g.q = (z * 32 + y) * 4 + m4;
-    g.q_yp = (z * 32 + ((y + 1) & 31)) * 4 + m4;
-    g.q_ym = (z * 32 + ((y + 31) & 31)) * 4 + m4;
-    g.q_zp = (((z + 1) & 31) * 32 + y) * 4 + m4;
-    g.q_zm = (((z + 31) & 31) * 32 + y) * 4 + m4;
+    g.qbase = 128 * dd + 4 * y + m4;
+    g.dyp = 4 * (((y + 1) & 31) - y);
+    g.dym = 4 * (((y + 31) & 31) - y);
     return g;
 }
 
-__device__ __forceinline__ Quad6 load_J(const uint4 *__restrict__ Jw, int colour, const Geo32 &g)
+__device__ __forceinline__ Quad32 quad_of(const Geo32 &g, int Z)
 {
-    const uint4 *Jown = Jw + (size_t)colour * 3 * RQ;
-    const uint4 *Joth = Jw + (size_t)(1 - colour) * 3 * RQ;
-    Quad6 r;
-    r.x = __ldg(Jown + g.q);
-    r.y = __ldg(Jown + RQ + g.q);
-    r.z = __ldg(Jown + 2 * RQ + g.q);
-    r.ox = __ldg(Joth + g.q);
-    r.oy = __ldg(Joth + RQ + g.q_ym);
-    r.oz = __ldg(Joth + 2 * RQ + g.q_zm);
+    Quad32 r;
+    r.q = g.qbase + 256 * Z;
+    r.q_yp = r.q + g.dyp;
+    r.q_ym = r.q + g.dym;
+    r.q_zp = (r.q + 128) & (RQ - 1);
+    r.q_zm = (r.q - 128) & (RQ - 1);
     return r;
 }
 
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "W_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra D_%=;\n\t"
+        "bra W_%=;\n\t"
+        "D_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+
+// one lane: arm the barrier with the byte count and start the bulk copy global -> shared
+__device__ __forceinline__ void bulk_load(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+
 template <int P, bool ENERGY>
-__device__ __forceinline__ void quad_update(uint4 *__restrict__ Sa, const uint4 *__restrict__ So, const Geo32 &g,
+__device__ __forceinline__ void quad_update(uint4 *__restrict__ Sa, const uint4 *__restrict__ So, const Quad32 &g,
                                             const Quad6 &Jq, const uint4 r4, const SlotK &K, uint32_t amask,
                                             uint32_t one, uint32_t mone, int lane, uint32_t (&accU)[8],
                                             uint32_t (&accM)[7])
@@ -94,19 +133,13 @@ __device__ __forceinline__ void quad_update(uint4 *__restrict__ Sa, const uint4 
     const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
     const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
     const uint32_t v0[4] = {o0.x, o0.y, o0.z, o0.w};
-    uint32_t vB[4], JA[4], JB[4];
-    if (P) {       // same m: the -x neighbour (its bond); m+1: the +x neighbour (own bond)
-        vB[0] = o0.y; vB[1] = o0.z; vB[2] = o0.w; vB[3] = side;
-        JA[0] = Jq.ox.x; JA[1] = Jq.ox.y; JA[2] = Jq.ox.z; JA[3] = Jq.ox.w;
-        JB[0] = Jq.x.x; JB[1] = Jq.x.y; JB[2] = Jq.x.z; JB[3] = Jq.x.w;
-    } else {       // same m: the +x neighbour (own bond); m-1: the -x neighbour (its bond)
-        const uint32_t jside = __shfl_sync(0xffffffffu, Jq.ox.w, src);
-        vB[0] = side; vB[1] = o0.x; vB[2] = o0.y; vB[3] = o0.z;
-        JA[0] = Jq.x.x; JA[1] = Jq.x.y; JA[2] = Jq.x.z; JA[3] = Jq.x.w;
-        JB[0] = jside; JB[1] = Jq.ox.x; JB[2] = Jq.ox.y; JB[3] = Jq.ox.z;
-    }
-    const uint32_t Jyp[4] = {Jq.y.x, Jq.y.y, Jq.y.z, Jq.y.w}, Jym[4] = {Jq.oy.x, Jq.oy.y, Jq.oy.z, Jq.oy.w};
-    const uint32_t Jzp[4] = {Jq.z.x, Jq.z.y, Jq.z.z, Jq.z.w}, Jzm[4] = {Jq.oz.x, Jq.oz.y, Jq.oz.z, Jq.oz.w};
+    // second x-neighbour: at m+1 for p = 1, at m-1 for p = 0 (the packed couplings are already in this order)
+    uint32_t vB[4];
+    if (P) { vB[0] = o0.y; vB[1] = o0.z; vB[2] = o0.w; vB[3] = side; }
+    else   { vB[0] = side; vB[1] = o0.x; vB[2] = o0.y; vB[3] = o0.z; }
+    const uint32_t JA[4] = {Jq.a.x, Jq.a.y, Jq.a.z, Jq.a.w}, JB[4] = {Jq.b.x, Jq.b.y, Jq.b.z, Jq.b.w};
+    const uint32_t Jyp[4] = {Jq.yp.x, Jq.yp.y, Jq.yp.z, Jq.yp.w}, Jym[4] = {Jq.ym.x, Jq.ym.y, Jq.ym.z, Jq.ym.w};
+    const uint32_t Jzp[4] = {Jq.zp.x, Jq.zp.y, Jq.zp.z, Jq.zp.w}, Jzm[4] = {Jq.zm.x, Jq.zm.y, Jq.zm.z, Jq.zm.w};
     const uint32_t vyp[4] = {oyp.x, oyp.y, oyp.z, oyp.w}, vym[4] = {oym.x, oym.y, oym.z, oym.w};
     const uint32_t vzp[4] = {ozp.x, ozp.y, ozp.z, ozp.w}, vzm[4] = {ozm.x, ozm.y, ozm.z, ozm.w};
     uint32_t out[4], w[4][3];
@@ -148,90 +181,110 @@ __device__ __forceinline__ void quad_update(uint4 *__restrict__ Sa, const uint4 
 
 __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constant__ Res32Args A)
 {
-    extern __shared__ __align__(16) uint32_t smem[];
-    uint4 *S4 = reinterpret_cast<uint4 *>(smem);               // [2][RQ]
-    int *sUM = reinterpret_cast<int *>(smem + RN);              // [2][32]
+    extern __shared__ __align__(128) uint32_t smem[];
+    uint4 *S4 = reinterpret_cast<uint4 *>(smem);                           // [2][RQ]                  128 KB
+    uint4 *ring = S4 + 2 * RQ;                                             // [16 warps][2 stages][6][32] 96 KB
+    uint64_t *bars = reinterpret_cast<uint64_t *>(ring + R_WARPS * N_STAGES * CHUNK_U4);   // [16][2]
+    int *sUM = reinterpret_cast<int *>(bars + R_WARPS * N_STAGES);         // [2][32]
     const Dims &d = A.d;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int sys = blockIdx.x;
-    const int t = sys % d.NT, a = (sys / d.NT) % d.R, w = sys / (d.NT * d.R);
+    const int t = blockIdx.x, a = blockIdx.y, w = blockIdx.z;      // x fastest: the 128 systems of a word are consecutive CTAs
+    const int sys = (w * d.R + a) * d.NT + t;
     uint4 *gS = reinterpret_cast<uint4 *>(A.spins + (size_t)sys * RN);
-    const uint4 *Jw = reinterpret_cast<const uint4 *>(A.J + (size_t)w * 3 * RN);
+    const int zhalf = warp >> 3, wj = warp & 7;
+    // chunk of (colour, Z) for this warp: Jp_w + ((colour * 16 + Z) * 8 + wj) * CHUNK_U4
+    const uint4 *Jpw = A.Jp + ((size_t)w * CHUNKS_PER_WORD + wj) * CHUNK_U4;
+    uint4 *my_ring = ring + warp * N_STAGES * CHUNK_U4;
+    const uint32_t ring_s = smem_u32(my_ring), bar_s = smem_u32(bars + warp * N_STAGES);
+
+    const int n_half = 2 * A.n_sweeps;
+    const int n_steps = n_half * R_ITERS;
+    // step n (0 .. n_steps-1) of this warp: half sweep n >> 3, iteration n & 7, plane pair Z = 2 it + zhalf
+    auto issue = [&](int n) {          // lane 0 only
+        const int colour = (n >> 3) & 1, Z = 2 * (n & 7) + zhalf;
+        const int st = n & 1;
+        bulk_load(ring_s + st * CHUNK_BYTES, Jpw + (size_t)((colour * 16 + Z) * 8) * CHUNK_U4, CHUNK_BYTES, bar_s + st * 8);
+    };
+    if (lane == 0) {
+        mbar_init(bar_s, 1);
+        mbar_init(bar_s + 8, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        issue(0);
+        if (n_steps > 1) issue(1);
+    }
 
     // ---- load the system (contiguous 128 KB)
 #pragma unroll 8
     for (int i = 0; i < 2 * RQ / R_THREADS; ++i) S4[i * R_THREADS + tid] = gS[i * R_THREADS + tid];
     if (tid < 64) sUM[tid] = 0;
 
-    SlotK K;
-    {
-        uint32_t zc[7];
+    SlotK K;                                                // block-uniform: stays in uniform registers / the constant bank
 #pragma unroll
-        for (int c = 0; c < 7; ++c) {
-            const uint2 v = A.tab[t].c64[c];               // (0 - thr) as 64 bits: hi = 0 only for thr = 0
-            K.lo[c] = v.x;
-            zc[c] = v.y == 0u ? 1u : 0u;
-        }
-        K.b3c = zc[3] - 1u;
-        K.nc = zc[1] + zc[5] - 1u;
-        K.ec = zc[0] + zc[2] + zc[4] + zc[6] - 2u;
-    }
+    for (int c = 0; c < 7; ++c) K.lo[c] = A.kc[t][c];
+    K.b3c = A.kc[t][7];
+    K.nc = A.kc[t][8];
+    K.ec = A.kc[t][9];
     const uint32_t amask = d.neg_h ? 0xffffffffu : 0u;
     const uint32_t wglob = (uint32_t)(w + (d.s_first >> 5));
     const uint32_t c3 = ctr3(3, a, t);
-    uint32_t accU[8], accM[7];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) accU[k] = 0;
-#pragma unroll
-    for (int k = 0; k < 7; ++k) accM[k] = 0;
+    const Geo32 geo = geo_of(wj, lane);
+    const int pi = (wj >> 2) & 1;
     __syncthreads();
 
-    // ---- flat loop over (sweep, colour, iteration); couplings of the next step are loaded one step ahead.
-    // Colour 1 walks the tasks in reverse so that the most recently read coupling lines are still in L1.
-    const int n_steps = A.n_sweeps * 2 * R_ITERS;
-    auto task_of = [&](int step) {
-        const int colour = (step / R_ITERS) & 1, it = step % R_ITERS;
-        const int task = it * R_WARPS + warp;
-        return colour ? 127 - task : task;
-    };
-    Geo32 g = geo_of(task_of(0), lane, 0);
-    Quad6 Jq = load_J(Jw, 0, g);
-#pragma unroll 1
-    for (int step = 0; step < n_steps; ++step) {
-        const int hs = step / R_ITERS;                      // half-sweep index in this launch
+    auto half_sweep = [&](auto P_tag, auto E_tag, int hs) {
+        constexpr int P = decltype(P_tag)::value;
+        constexpr bool ENERGY = decltype(E_tag)::value;
         const int colour = hs & 1;
-        const uint64_t sweep = A.sweep0 + (uint64_t)(hs >> 1);
-        const uint32_t time = 2u * (uint32_t)sweep + (uint32_t)colour;
-        // prefetch the couplings of the next step
-        Geo32 gn = g;
-        Quad6 Jn = Jq;
-        if (step + 1 < n_steps) {
-            const int cn = ((step + 1) / R_ITERS) & 1;
-            gn = geo_of(task_of(step + 1), lane, cn);
-            Jn = load_J(Jw, cn, gn);
-        }
+        const uint32_t time = 2u * (uint32_t)(A.sweep0 + (uint64_t)(hs >> 1)) + (uint32_t)colour;
         uint4 *Sa = S4 + colour * RQ;
         const uint4 *So = S4 + (1 - colour) * RQ;
-        const uint4 r4 = philox_rk8((uint32_t)g.q, time, wglob, c3, A.rk);
-        const bool energy = A.want_energy && hs == 2 * A.n_sweeps - 1;
-        if (energy) {
-            if (g.p) quad_update<1, true>(Sa, So, g, Jq, r4, K, amask, A.one, A.mone, lane, accU, accM);
-            else     quad_update<0, true>(Sa, So, g, Jq, r4, K, amask, A.one, A.mone, lane, accU, accM);
-        } else {
-            if (g.p) quad_update<1, false>(Sa, So, g, Jq, r4, K, amask, A.one, A.mone, lane, accU, accM);
-            else     quad_update<0, false>(Sa, So, g, Jq, r4, K, amask, A.one, A.mone, lane, accU, accM);
+        uint32_t accU[8], accM[7];                          // live in the ENERGY instantiations only
+#pragma unroll
+        for (int k = 0; k < 8; ++k) accU[k] = 0;
+#pragma unroll
+        for (int k = 0; k < 7; ++k) accM[k] = 0;
+#pragma unroll 1
+        for (int it = 0; it < R_ITERS; ++it) {
+            const int n = hs * R_ITERS + it;
+            const int st = n & 1;
+            mbar_wait(bar_s + st * 8, (uint32_t)(n >> 1) & 1u);
+            const uint4 *Jc = my_ring + st * CHUNK_U4 + lane;
+            Quad6 Jq;
+            Jq.a = Jc[0];
+            Jq.b = Jc[32];
+            Jq.yp = Jc[64];
+            Jq.ym = Jc[96];
+            Jq.zp = Jc[128];
+            Jq.zm = Jc[160];
+            __syncwarp();                                   // every lane has read the stage: refill it two steps ahead
+            if (lane == 0 && n + 2 < n_steps) issue(n + 2);
+            const Quad32 g = quad_of(geo, 2 * it + zhalf);
+            quad_update<P, ENERGY>(Sa, So, g, Jq, philox_rk8((uint32_t)g.q, time, wglob, c3, A.rk), K, amask, A.one,
+                                   A.mone, lane, accU, accM);
         }
-        g = gn;
-        Jq = Jn;
-        if (step % R_ITERS == R_ITERS - 1) __syncthreads();
+        if constexpr (ENERGY) {                             // per-lane totals of this warp -> CTA totals
+            const uint32_t totU = bs_warp_total(accU, 8, lane);
+            const uint32_t totM = bs_warp_total(accM, 7, lane);
+            atomicAdd(&sUM[lane], (int)totU);
+            atomicAdd(&sUM[32 + lane], (int)totM);
+        }
+    };
+    using T0 = std::integral_constant<int, 0>;
+    using T1 = std::integral_constant<int, 1>;
+#pragma unroll 1
+    for (int hs = 0; hs < n_half; ++hs) {
+        const int p = ((hs & 1) + pi) & 1;                  // warp-uniform row parity of this half sweep
+        if (A.want_energy && hs == n_half - 1) {
+            if (p) half_sweep(T1{}, std::true_type{}, hs);
+            else   half_sweep(T0{}, std::true_type{}, hs);
+        } else {
+            if (p) half_sweep(T1{}, std::false_type{}, hs);
+            else   half_sweep(T0{}, std::false_type{}, hs);
+        }
+        __syncthreads();
     }
 
-    if (A.want_energy) {
-        const uint32_t totU = bs_warp_total(accU, 8, lane);
-        const uint32_t totM = bs_warp_total(accM, 7, lane);
-        atomicAdd(&sUM[lane], (int)totU);
-        atomicAdd(&sUM[32 + lane], (int)totM);
-        __syncthreads();
+    if (A.want_energy) {                                    // (the loop ended with a __syncthreads)
         if (tid < 32) {
             const size_t o = ((size_t)(w * 32 + tid) * d.R + a) * d.NT + t;
             A.U[o] = (int64_t)sUM[tid];
@@ -244,14 +297,59 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
     for (int i = 0; i < 2 * RQ / R_THREADS; ++i) gS[i * R_THREADS + tid] = S4[i * R_THREADS + tid];
 }
 
-constexpr size_t RES32_SMEM = (size_t)RN * 4 + 64 * 4;
+// canonical couplings J[w][colour][dir][H] -> packed copy (see above); one thread per packed uint4
+__global__ void __launch_bounds__(256) k_pack_J_res32(Dims d, const uint32_t *__restrict__ J, uint4 *__restrict__ Jp)
+{
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)d.W * CHUNKS_PER_WORD * CHUNK_U4) return;
+    const int lane = (int)(idx & 31), arr = (int)((idx >> 5) % 6);
+    long long ch = idx / CHUNK_U4;
+    const int wj = (int)(ch & 7);   ch >>= 3;
+    const int Z = (int)(ch & 15);   ch >>= 4;
+    const int colour = (int)(ch & 1);
+    const int w = (int)(ch >> 1);
+    const int pi = (wj >> 2) & 1, j = wj & 3;
+    const int jj = lane >> 3, dd = (lane >> 2) & 1, m4 = lane & 3;
+    const int y = (2 * (4 * j + jj) + pi + dd) & 31, z = 2 * Z + dd;
+    const int p = (colour + pi) & 1;
+    const uint32_t *Jown = J + ((size_t)(w * 2 + colour) * 3) * RH;
+    const uint32_t *Joth = J + ((size_t)(w * 2 + 1 - colour) * 3) * RH;
+    const int row = z * 32 + y;
+    uint32_t v[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const int m = 4 * m4 + e;
+        switch (arr) {
+        case 0: v[e] = p ? Joth[row * 16 + m] : Jown[row * 16 + m]; break;                   // same m: -x bond (p=1) / +x own bond (p=0)
+        case 1: v[e] = p ? Jown[row * 16 + m] : Joth[row * 16 + ((m + 15) & 15)]; break;     // m+1: own +x bond / m-1: its +x bond
+        case 2: v[e] = Jown[RH + row * 16 + m]; break;
+        case 3: v[e] = Joth[RH + (z * 32 + ((y + 31) & 31)) * 16 + m]; break;
+        case 4: v[e] = Jown[2 * RH + row * 16 + m]; break;
+        default: v[e] = Joth[2 * RH + (((z + 31) & 31) * 32 + y) * 16 + m]; break;
+        }
+    }
+    Jp[idx] = make_uint4(v[0], v[1], v[2], v[3]);
+}
+
+constexpr size_t RES32_SMEM = (size_t)RN * 4 + (size_t)R_WARPS * N_STAGES * CHUNK_BYTES + R_WARPS * N_STAGES * 8 + 64 * 4;
 
 }  // namespace
+
+size_t res32_packed_bytes(int W) { return (size_t)W * CHUNKS_PER_WORD * CHUNK_BYTES; }
 
 bool res32_supported(const sg_ctx *c)
 {
     const Dims &d = c->d;
-    return c->kind == SG_PMJ && d.fast_accept && d.L == 32;
+    return c->kind == SG_PMJ && d.fast_accept && d.L == 32 && c->Jp != nullptr;
+}
+
+// packed copy of the couplings (after every k_init_J_pmj)
+int launch_pack_J_res32(sg_ctx *c)
+{
+    const Dims &d = c->d;
+    const long long n = (long long)d.W * CHUNKS_PER_WORD * CHUNK_U4;
+    k_pack_J_res32<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(d, c->J, c->Jp);
+    return 1;
 }
 
 // n_sweeps consecutive sweeps from global sweep index sweep0; want_energy: also write U, M of the final
@@ -262,17 +360,13 @@ int launch_res32_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, bool want_energy)
     if (!configured) {
         if (cudaFuncSetAttribute(k_res32_pmj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RES32_SMEM) != cudaSuccess)
             return -1;
-        // smallest shared-memory configuration that holds the system: the rest of the 228 KB stays L1
-        // and keeps the coupling lines read by the previous half sweep
-        cudaFuncSetAttribute(k_res32_pmj, cudaFuncAttributePreferredSharedMemoryCarveout, 58);
         configured = true;
     }
     const Dims &d = c->d;
     Res32Args A;
     A.d = d;
     A.spins = c->spins;
-    A.J = c->J;
-    A.tab = c->tab;
+    A.Jp = c->Jp;
     A.U = c->U;
     A.M = c->M;
     for (int r = 0; r < 10; ++r) {
@@ -284,7 +378,18 @@ int launch_res32_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, bool want_energy)
     A.want_energy = want_energy ? 1 : 0;
     A.one = 1u;
     A.mone = 0xffffffffu;
-    k_res32_pmj<<<d.W * d.R * d.NT, R_THREADS, RES32_SMEM, c->stream>>>(A);
+    for (int t = 0; t < d.NT; ++t) {                        // SlotK of sg_accept.cuh from the host threshold table
+        uint32_t zc[7];
+        for (int code = 0; code < 7; ++code) {
+            const uint64_t th = c->thr[((size_t)t * 7 + (code >> 1)) * 2 + (1 - (code & 1))];
+            A.kc[t][code] = (uint32_t)((uint64_t)0 - th);
+            zc[code] = th == 0 ? 1u : 0u;
+        }
+        A.kc[t][7] = zc[3] - 1u;
+        A.kc[t][8] = zc[1] + zc[5] - 1u;
+        A.kc[t][9] = zc[0] + zc[2] + zc[4] + zc[6] - 2u;
+    }
+    k_res32_pmj<<<dim3(d.NT, d.R, d.W), R_THREADS, RES32_SMEM, c->stream>>>(A);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
