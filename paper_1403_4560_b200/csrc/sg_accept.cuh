@@ -74,6 +74,30 @@ __device__ __forceinline__ uint32_t accept_word(uint32_t u0, uint32_t u1, uint32
     return n2 | g2;
 }
 
+// Same decision with the field alignment folded in (a = s ^ amask ^ 1...: na = ~(s ^ amask)) and the flip
+// fused: returns the NEW spin word s ^ accept.  ALU pipe: 8 (count) + 7 (carries) + 4.
+constexpr int LUT_G0 = (~((0xF0 ^ 0xCC) & 0xAA)) & 0xFF;                    // ~((a ^ b) & c) = na | ~c
+__device__ __forceinline__ uint32_t flip_word_k(uint32_t s, uint32_t amask, uint32_t u0, uint32_t u1, uint32_t u2,
+                                                uint32_t u3, uint32_t u4, uint32_t u5, uint32_t r, const SlotK &K,
+                                                uint32_t one, uint32_t mone)
+{
+    const uint32_t s0 = xor3(u0, u1, u2), c0 = maj3(u0, u1, u2);
+    const uint32_t s1 = xor3(u3, u4, u5), c1 = maj3(u3, u4, u5);
+    const uint32_t n0 = s0 ^ s1;
+    const uint32_t k = s0 & s1;
+    const uint32_t n1 = xor3(c0, c1, k);
+    const uint32_t n2 = maj3(c0, c1, k);
+    const uint32_t B3 = cadd(r, K.lo[3], K.b3c, one);
+    const uint32_t Nn = cadd(r, K.lo[5], cadd(r, K.lo[1], K.nc, one), one);
+    const uint32_t E = cadd(r, K.lo[6], cadd(r, K.lo[4], cadd(r, K.lo[2], cadd(r, K.lo[0], K.ec, one), one), one), one);
+    const uint32_t K1m = imad(Nn, mone, B3);
+    const uint32_t K0m = imad(Nn, one, imad(E, mone, B3));
+    const uint32_t g0 = lop3<LUT_G0>(s, amask, K0m);
+    const uint32_t g1 = lop3<LUT_GE>(n0, K1m, g0);
+    const uint32_t g2 = lop3<LUT_MAJ>(n1, B3, g1);
+    return lop3<LUT_FLIP>(s, n2, g2);
+}
+
 // bit-sliced a (NA planes) + b (NA planes) -> NA+1 planes
 template <int NA>
 __device__ __forceinline__ void bs_sum(const uint32_t (&a)[NA], const uint32_t (&b)[NA], uint32_t (&o)[NA + 1])

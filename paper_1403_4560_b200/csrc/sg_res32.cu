@@ -58,14 +58,11 @@ struct Quad6 {
 };
 
 // A thread's quad inside a z-plane pair is fixed for the whole launch (y, which row of the diagonal
-// pair, quad within the row); only the plane pair Z = 0..15 changes from step to step.
+// pair, quad within the row); only the plane pair Z = 0..15 changes from step to step.  All shared-memory
+// addresses are 32-bit byte addresses: (thread constant) + 4096 * Z (warp-uniform).
 struct Geo32 {
-    int qbase;                      // uint4 index of the quad for Z = 0 inside one colour array
-    int dyp, dym;                   // index deltas to the rows y+1, y-1 (periodic)
-};
-
-struct Quad32 {
-    int q, q_yp, q_ym, q_zp, q_zm;  // uint4 indices inside one colour array
+    uint32_t tb;                    // byte offset of the quad for Z = 0 inside one colour array (64 KB)
+    uint32_t dyp, dym;              // byte deltas to the rows y+1, y-1 (periodic)
 };
 
 __device__ __forceinline__ Geo32 geo_of(int wj, int lane)
@@ -74,21 +71,22 @@ __device__ __forceinline__ Geo32 geo_of(int wj, int lane)
     const int jj = lane >> 3, dd = (lane >> 2) & 1, m4 = lane & 3;
     const int y = (2 * (4 * j + jj) + pi + dd) & 31;
     Geo32 g;
-    g.qbase = 128 * dd + 4 * y + m4;
-    g.dyp = 4 * (((y + 1) & 31) - y);
-    g.dym = 4 * (((y + 31) & 31) - y);
+    g.tb = (uint32_t)(128 * dd + 4 * y + m4) * 16u;
+    g.dyp = (uint32_t)(64 * (((y + 1) & 31) - y));
+    g.dym = (uint32_t)(64 * (((y + 31) & 31) - y));
     return g;
 }
 
-__device__ __forceinline__ Quad32 quad_of(const Geo32 &g, int Z)
+__device__ __forceinline__ uint4 lds128(uint32_t addr)
 {
-    Quad32 r;
-    r.q = g.qbase + 256 * Z;
-    r.q_yp = r.q + g.dyp;
-    r.q_ym = r.q + g.dym;
-    r.q_zp = (r.q + 128) & (RQ - 1);
-    r.q_zm = (r.q - 128) & (RQ - 1);
-    return r;
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ void sts128(uint32_t addr, const uint4 v)
+{
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -118,15 +116,16 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void *src, uint32_
                  : "memory");
 }
 
+// sa / so: byte addresses of the own-colour / other-colour array; qb: byte offset of the quad in them
 template <int P, bool ENERGY>
-__device__ __forceinline__ void quad_update(uint4 *__restrict__ Sa, const uint4 *__restrict__ So, const Quad32 &g,
-                                            const Quad6 &Jq, const uint4 r4, const SlotK &K, uint32_t amask,
-                                            uint32_t one, uint32_t mone, int lane, uint32_t (&accU)[8],
-                                            uint32_t (&accM)[7])
+__device__ __forceinline__ void quad_update(uint32_t sa, uint32_t so, uint32_t qb, const Geo32 &g, const Quad6 &Jq,
+                                            const uint4 r4, const SlotK &K, uint32_t amask, uint32_t one, uint32_t mone,
+                                            int lane, uint32_t (&accU)[8], uint32_t (&accM)[7])
 {
-    const uint4 sv = Sa[g.q];
-    const uint4 o0 = So[g.q];
-    const uint4 oyp = So[g.q_yp], oym = So[g.q_ym], ozp = So[g.q_zp], ozm = So[g.q_zm];
+    const uint4 sv = lds128(sa + qb);
+    const uint4 o0 = lds128(so + qb);
+    const uint4 oyp = lds128(so + qb + g.dyp), oym = lds128(so + qb + g.dym);
+    const uint4 ozp = lds128(so + ((qb + 2048u) & 0xffffu)), ozm = lds128(so + ((qb - 2048u) & 0xffffu));
     // word of the adjacent quad of the same row (periodic): m+1 for p = 1, m-1 for p = 0
     const int src = (lane & ~3) | ((lane + (P ? 1 : 3)) & 3);
     const uint32_t side = __shfl_sync(0xffffffffu, P ? o0.x : o0.w, src);
@@ -145,12 +144,14 @@ __device__ __forceinline__ void quad_update(uint4 *__restrict__ Sa, const uint4 
     uint32_t out[4], w[4][3];
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
-        uint32_t n0, n1, n2;
-        const uint32_t acc = accept_word(xor3(s[e], v0[e], JA[e]), xor3(s[e], vB[e], JB[e]), xor3(s[e], vyp[e], Jyp[e]),
-                                         xor3(s[e], vym[e], Jym[e]), xor3(s[e], vzp[e], Jzp[e]),
-                                         xor3(s[e], vzm[e], Jzm[e]), ~(s[e] ^ amask), rr[e], K, one, mone, n0, n1, n2);
-        out[e] = s[e] ^ acc;
-        if (ENERGY) {
+        const uint32_t u0 = xor3(s[e], v0[e], JA[e]), u1 = xor3(s[e], vB[e], JB[e]), u2 = xor3(s[e], vyp[e], Jyp[e]);
+        const uint32_t u3 = xor3(s[e], vym[e], Jym[e]), u4 = xor3(s[e], vzp[e], Jzp[e]), u5 = xor3(s[e], vzm[e], Jzm[e]);
+        if (!ENERGY) {
+            out[e] = flip_word_k(s[e], amask, u0, u1, u2, u3, u4, u5, rr[e], K, one, mone);
+        } else {
+            uint32_t n0, n1, n2;
+            const uint32_t acc = accept_word(u0, u1, u2, u3, u4, u5, ~(s[e] ^ amask), rr[e], K, one, mone, n0, n1, n2);
+            out[e] = s[e] ^ acc;
             // post-flip unsatisfied count: n if not flipped, 6 - n if flipped
             // 6 - n: bit0 = n0; bit1 = 1 for n in {0,3,4}; bit2 = 1 for n in {0,1,2}
             const uint32_t f1 = (~n2 & ~(n1 ^ n0)) | (n2 & ~n1 & ~n0);
@@ -160,7 +161,7 @@ __device__ __forceinline__ void quad_update(uint4 *__restrict__ Sa, const uint4 
             w[e][2] = (acc & f2) | (~acc & n2);
         }
     }
-    Sa[g.q] = make_uint4(out[0], out[1], out[2], out[3]);
+    sts128(sa + qb, make_uint4(out[0], out[1], out[2], out[3]));
     if (ENERGY) {
         uint32_t ab[4], cd[4], U5[5];
         bs_sum<3>(w[0], w[1], ab);
@@ -187,30 +188,29 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
     uint64_t *bars = reinterpret_cast<uint64_t *>(ring + R_WARPS * N_STAGES * CHUNK_U4);   // [16][2]
     int *sUM = reinterpret_cast<int *>(bars + R_WARPS * N_STAGES);         // [2][32]
     const Dims &d = A.d;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);        // warp-uniform for the compiler: uniform datapath
     const int t = blockIdx.x, a = blockIdx.y, w = blockIdx.z;      // x fastest: the 128 systems of a word are consecutive CTAs
     const int sys = (w * d.R + a) * d.NT + t;
     uint4 *gS = reinterpret_cast<uint4 *>(A.spins + (size_t)sys * RN);
     const int zhalf = warp >> 3, wj = warp & 7;
     // chunk of (colour, Z) for this warp: Jp_w + ((colour * 16 + Z) * 8 + wj) * CHUNK_U4
     const uint4 *Jpw = A.Jp + ((size_t)w * CHUNKS_PER_WORD + wj) * CHUNK_U4;
-    uint4 *my_ring = ring + warp * N_STAGES * CHUNK_U4;
-    const uint32_t ring_s = smem_u32(my_ring), bar_s = smem_u32(bars + warp * N_STAGES);
+    const uint32_t S_s = smem_u32(S4);
+    const uint32_t ring_s = smem_u32(ring + warp * N_STAGES * CHUNK_U4), bar_s = smem_u32(bars + warp * N_STAGES);
 
     const int n_half = 2 * A.n_sweeps;
-    const int n_steps = n_half * R_ITERS;
-    // step n (0 .. n_steps-1) of this warp: half sweep n >> 3, iteration n & 7, plane pair Z = 2 it + zhalf
-    auto issue = [&](int n) {          // lane 0 only
-        const int colour = (n >> 3) & 1, Z = 2 * (n & 7) + zhalf;
-        const int st = n & 1;
+    // step (hs, it) of this warp: half sweep hs, iteration it = 0..7, plane pair Z = 2 it + zhalf, stage it & 1
+    auto issue = [&](int hs, int it) {          // lane 0 only
+        const int colour = hs & 1, Z = 2 * it + zhalf, st = it & 1;
         bulk_load(ring_s + st * CHUNK_BYTES, Jpw + (size_t)((colour * 16 + Z) * 8) * CHUNK_U4, CHUNK_BYTES, bar_s + st * 8);
     };
     if (lane == 0) {
         mbar_init(bar_s, 1);
         mbar_init(bar_s + 8, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        issue(0);
-        if (n_steps > 1) issue(1);
+        issue(0, 0);
+        issue(0, 1);
     }
 
     // ---- load the system (contiguous 128 KB)
@@ -236,8 +236,7 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
         constexpr bool ENERGY = decltype(E_tag)::value;
         const int colour = hs & 1;
         const uint32_t time = 2u * (uint32_t)(A.sweep0 + (uint64_t)(hs >> 1)) + (uint32_t)colour;
-        uint4 *Sa = S4 + colour * RQ;
-        const uint4 *So = S4 + (1 - colour) * RQ;
+        const uint32_t sa = S_s + (uint32_t)colour * 65536u, so = S_s + (uint32_t)(1 - colour) * 65536u;
         uint32_t accU[8], accM[7];                          // live in the ENERGY instantiations only
 #pragma unroll
         for (int k = 0; k < 8; ++k) accU[k] = 0;
@@ -245,21 +244,23 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
         for (int k = 0; k < 7; ++k) accM[k] = 0;
 #pragma unroll 1
         for (int it = 0; it < R_ITERS; ++it) {
-            const int n = hs * R_ITERS + it;
-            const int st = n & 1;
-            mbar_wait(bar_s + st * 8, (uint32_t)(n >> 1) & 1u);
-            const uint4 *Jc = my_ring + st * CHUNK_U4 + lane;
+            const int st = it & 1;
+            mbar_wait(bar_s + st * 8, (uint32_t)(it >> 1) & 1u);      // use (8 hs + it) / 2 of the stage: parity = bit 1 of it
+            const uint32_t jc = ring_s + st * CHUNK_BYTES + lane * 16;
             Quad6 Jq;
-            Jq.a = Jc[0];
-            Jq.b = Jc[32];
-            Jq.yp = Jc[64];
-            Jq.ym = Jc[96];
-            Jq.zp = Jc[128];
-            Jq.zm = Jc[160];
+            Jq.a = lds128(jc);
+            Jq.b = lds128(jc + 512);
+            Jq.yp = lds128(jc + 1024);
+            Jq.ym = lds128(jc + 1536);
+            Jq.zp = lds128(jc + 2048);
+            Jq.zm = lds128(jc + 2560);
             __syncwarp();                                   // every lane has read the stage: refill it two steps ahead
-            if (lane == 0 && n + 2 < n_steps) issue(n + 2);
-            const Quad32 g = quad_of(geo, 2 * it + zhalf);
-            quad_update<P, ENERGY>(Sa, So, g, Jq, philox_rk8((uint32_t)g.q, time, wglob, c3, A.rk), K, amask, A.one,
+            if (lane == 0) {
+                if (it + 2 < R_ITERS) issue(hs, it + 2);
+                else if (hs + 1 < n_half) issue(hs + 1, it + 2 - R_ITERS);
+            }
+            const uint32_t qb = geo.tb + 4096u * (uint32_t)(2 * it + zhalf);
+            quad_update<P, ENERGY>(sa, so, qb, geo, Jq, philox_rk8(qb >> 4, time, wglob, c3, A.rk), K, amask, A.one,
                                    A.mone, lane, accU, accM);
         }
         if constexpr (ENERGY) {                             // per-lane totals of this warp -> CTA totals
