@@ -27,7 +27,12 @@ sys.path.insert(0, ROOT)
 
 from paper_1403_4560_b200 import workloads as W  # noqa: E402
 
-ALU_OPS_PER_WORDSITE = 27     # algorithmic ALU-pipe lane-ops per 32-sample word-site update
+ALU_OPS_PER_WORDSITE = 30     # algorithmic ALU-pipe lane-ops per 32-sample word-site update:
+#                               6 bond XOR3 + 8 count + 7 threshold carries + 4 compare/flip + 5 Philox share
+HBM_BYTES_PER_WORDSITE_LAUNCH = 8   # spin word read once + written once per LAUNCH of a resident kernel
+# dram__bytes_read.sum + dram__bytes_write.sum of the roofline launch below, from the ncu --set full captures
+# summarised in profiles/r01_v3_resident_kernels.md (same command line as the default run of this file)
+NCU_TRAFFIC_BYTES = {"C2": 10.92e6, "C5": 8.747e9}
 ALU_LANES_PER_SM = 64         # INT/LOP3 lanes per SM per clock (16 per SMSP x 4; B300_MICROARCH pipe table)
 N_SM = 148
 
@@ -214,17 +219,24 @@ def run_ours(args, w):
     step_ms = [a.elapsed_time(b) for a, b in evs]
     total_ms = float(sum(step_ms))
 
-    # dominant kernel alone (the sweep), same process and clocks: events around n back-to-back sweeps
+    # dominant kernel alone (the sweep), same process and clocks: CUDA events on the library's stream around
+    # each of `reps` launches of n_k back-to-back sweeps (one launch each on the resident-kernel paths)
     n_k = 256 if w.N * w.n_samples < (1 << 28) else 16
+    reps = 3
     sim.sg_sweep(8)
     l0 = sim.sg_get_launch_count()
-    k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    k0.record(stream)
-    sim.sg_sweep(n_k)
-    k1.record(stream)
+    kev = []
+    for _ in range(reps):
+        k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k0.record(stream)
+        sim.sg_sweep(n_k)
+        k1.record(stream)
+        kev.append((k0, k1))
     torch.cuda.synchronize(dev)
     sweep_launches = sim.sg_get_launch_count() - l0
-    sweep_ms = k0.elapsed_time(k1)
+    sweep_ms = float(sum(a.elapsed_time(b) for a, b in kev)) / reps          # per n_k sweeps
+    sweep_launches //= reps
+    alu_peak_measured = sg.sg_probe_alu_peak(stream) / 1e12                  # T lane-ops/s, LOP3 micro-benchmark
     sampler.stop_flag = True
     sampler.join()
 
@@ -266,15 +278,25 @@ def run_ours(args, w):
 
     if rank == 0:
         wordsites_per_sweep = w.N * w.n_words * w.n_replicas * w.n_temps if w.kind == W.PMJ else w.N * w.n_samples * w.n_replicas * w.n_temps
-        peak = ALU_LANES_PER_SM * N_SM * pk["sm_max_mhz"] * 1e6 / 1e12          # T lane-ops / s
+        nominal = ALU_LANES_PER_SM * N_SM * pk["sm_max_mhz"] * 1e6 / 1e12       # T lane-ops / s
+        peak = alu_peak_measured
         ach = ALU_OPS_PER_WORDSITE * wordsites_per_sweep * n_k / (sweep_ms * 1e-3) / 1e12
         sweep_rate = w.flip_attempts(n_k) / (sweep_ms * 1e6)
+        launch_s = sweep_ms * 1e-3 / max(1, sweep_launches)
+        hbm_ach = HBM_BYTES_PER_WORDSITE_LAUNCH * wordsites_per_sweep / launch_s / 1e9 if w.kind == W.PMJ else None
         roofline = {"bound": "alu", "kernel": "sweep (+-J multispin)", "achieved": ach, "peak": peak, "unit": "Tlaneop/s",
-                    "frac": ach / peak, "traffic": None,
-                    "peak_source": "64 INT lanes/SM/clk x 148 SMs x sm_max_mhz (%s MEASURED_PEAKS.json)" % pk["src"],
-                    "alu_ops_per_wordsite": ALU_OPS_PER_WORDSITE, "launch_us": 1e3 * sweep_ms / max(1, sweep_launches),
-                    "launches_timed": sweep_launches, "sweep_only_flips_per_ns": sweep_rate,
-                    "share_of_step": (sweep_ms / n_k) * w.n_sweeps / (total_ms / args.steps)}
+                    "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(w.name),
+                    "peak_source": "measured in this run: dependency-free LOP3 micro-benchmark (sg_probe_alu_peak); "
+                                   "nominal 64 INT lanes/SM/clk x 148 SMs x %.0f MHz = %.2f" % (pk["sm_max_mhz"], nominal),
+                    "peak_nominal": nominal, "frac_of_nominal": ach / nominal,
+                    "alu_ops_per_wordsite": ALU_OPS_PER_WORDSITE, "launch_us": 1e6 * launch_s,
+                    "launches_timed": sweep_launches * reps, "sweeps_per_launch": n_k // max(1, sweep_launches),
+                    "sweep_only_flips_per_ns": sweep_rate,
+                    "share_of_step": (sweep_ms / n_k) * w.n_sweeps / (total_ms / args.steps),
+                    "hbm": {"achieved": hbm_ach, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                            "frac": (hbm_ach / pk["hbm_gbs"]) if hbm_ach else None,
+                            "note": "algorithmic 8 B per word-site per LAUNCH (state resident in shared memory for all "
+                                    "sweeps of a launch): HBM is not the binding roof, the ALU pipe is (DESIGN.md 6)"}}
         if w.kind != W.PMJ:
             roofline.update({"kernel": "sweep (Gaussian fp32)", "note": "no roofline target for the Gaussian path"})
         out = {"metric": "spin_flip_attempts_per_ns", "value": value, "unit": "flips/ns", "n_gpus": world,

@@ -135,6 +135,12 @@ int sg_get_counters(sg_ctx *ctx, uint64_t *sweeps_done, uint64_t *exchanges_done
 /* number of kernels this context has launched so far (for bench.py's gpu_launches) */
 int sg_get_launch_count(sg_ctx *ctx, uint64_t *launches);
 
+/* Measured peak of the ALU (INT/LOP3) pipe of the current device: a dependency-free LOP3 micro-benchmark
+ * (8 independent chains per thread, 2 x 1024 threads per SM, no memory traffic; best of 5 launches, ~10 ms
+ * each) on `cuda_stream` (NULL = default stream).  *lane_ops_per_s = 32-bit lane operations per second.
+ * This is the denominator of bench.py's "alu" roofline.  Synchronous. */
+int sg_probe_alu_peak(void *cuda_stream, double *lane_ops_per_s);
+
 /* Description of the last error of this context (or of the last failed sg_create if ctx is NULL).
  * The string is owned by the library and valid until the next call on the same context. */
 const char *sg_last_error(sg_ctx *ctx);

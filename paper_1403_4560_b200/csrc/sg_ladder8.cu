@@ -106,19 +106,19 @@ __device__ __forceinline__ void half_sweep_quad(uint32_t *__restrict__ Sa, const
     uint32_t out[4], w[4][3];
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
-        uint32_t n0, n1, n2;
-        const uint32_t acc = accept_word(xor3(s[e], v0[e], JA[e]), xor3(s[e], vB[e], JB[e]), xor3(s[e], vyp[e], Jyp[e]),
-                                         xor3(s[e], vym[e], Jym[e]), xor3(s[e], vzp[e], Jzp[e]),
-                                         xor3(s[e], vzm[e], Jzm[e]), ~(s[e] ^ amask), rr[e], K, one, mone, n0, n1, n2);
-        out[e] = s[e] ^ acc;
-        // post-flip unsatisfied count of this site: n if not flipped, 6 - n if flipped
-        w[e][0] = n0;
-        w[e][1] = n1;
-        w[e][2] = n2;
-        if (ENERGY) {
+        const uint32_t u0 = xor3(s[e], v0[e], JA[e]), u1 = xor3(s[e], vB[e], JB[e]), u2 = xor3(s[e], vyp[e], Jyp[e]);
+        const uint32_t u3 = xor3(s[e], vym[e], Jym[e]), u4 = xor3(s[e], vzp[e], Jzp[e]), u5 = xor3(s[e], vzm[e], Jzm[e]);
+        if (!ENERGY) {
+            out[e] = flip_word_k(s[e], amask, u0, u1, u2, u3, u4, u5, rr[e], K, one, mone);
+        } else {
+            uint32_t n0, n1, n2;
+            const uint32_t acc = accept_word(u0, u1, u2, u3, u4, u5, ~(s[e] ^ amask), rr[e], K, one, mone, n0, n1, n2);
+            out[e] = s[e] ^ acc;
+            // post-flip unsatisfied count of this site: n if not flipped, 6 - n if flipped
             // 6 - n: bit0 = n0; bit1 = 1 for n in {0,3,4}; bit2 = 1 for n in {0,1,2}
             const uint32_t f1 = (~n2 & ~(n1 ^ n0)) | (n2 & ~n1 & ~n0);
             const uint32_t f2 = ~n2 & ~(n1 & n0);
+            w[e][0] = n0;
             w[e][1] = (acc & f1) | (~acc & n1);
             w[e][2] = (acc & f2) | (~acc & n2);
         }

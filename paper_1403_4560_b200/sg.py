@@ -41,6 +41,7 @@ EXPORTS = {
     "sg_get_counters": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "sg_get_launch_count": (C.c_int, [C.c_void_p, C.c_void_p]),
     "sg_last_error": (C.c_char_p, [C.c_void_p]),
+    "sg_probe_alu_peak": (C.c_int, [C.c_void_p, C.c_void_p]),
 }
 
 if not os.path.exists(LIB_PATH):
@@ -65,6 +66,15 @@ def _p(a):
 
 def sg_workspace_bytes(L, n_samples, n_replicas, n_temps, coupling_kind):
     return int(_lib.sg_workspace_bytes(L, n_samples, n_replicas, n_temps, coupling_kind))
+
+
+def sg_probe_alu_peak(stream=None):
+    """Measured ALU-pipe (LOP3) peak of the current device in lane-ops/s (include/sg.h)."""
+    v = C.c_double()
+    rc = _lib.sg_probe_alu_peak(C.c_void_p(stream.cuda_stream) if stream is not None else None, C.byref(v))
+    if rc != OK:
+        raise SgError(rc, "sg_probe_alu_peak failed")
+    return v.value
 
 
 class Simulation:
