@@ -259,3 +259,18 @@ def test_l32_resident_kernel_with_pt(sg, O, h, NT, R, pt_every, n_samples):
     for s, o in orc.items():
         assert close(rec[s], o.measure())
     sim.close()
+
+
+def test_estimators_on_device_moments_high_temperature(sg):
+    """End of the path: device accumulators -> Eqs. 3-6 (estimators.py).  At T = 20, 40 and h = 0 spins are nearly
+    independent: chi(k) = 1 + O(beta^2), R12 = 1, g = O(1/N), all within jackknife errors (blocks of whole words)."""
+    from paper_1403_4560_b200 import estimators as E
+    sim = sg.Simulation(8, 0.0, 256, 4, (20.0, 40.0), sg.PMJ, 77)
+    sim.sg_run(96, 1, 4)
+    mom, n = sim.sg_get_moments()
+    assert n == 24
+    out = E.indicators(mom, n, 8, n_pairs=6, block=32)
+    for name in ("chi0", "chi_k1", "chi_k2_paper", "chi_k2_baseline", "chi_k1_4rep", "R12", "R12_baseline"):
+        assert np.all(np.abs(out[name] - 1.0) < 0.03 + 5 * out[name + "_err"]), (name, out[name], out[name + "_err"])
+    assert np.all(np.abs(out["g_std"]) < 0.01 + 5 * out["g_std_err"])
+    sim.close()
