@@ -373,13 +373,14 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
     if (!c) return SG_EINVAL;
     if (n_sweeps < 0 || pt_every < 0 || meas_every < 0) return fail(c, SG_EINVAL, "sg_run: negative argument");
     int left = n_sweeps;
-    if (ladder8_supported(c)) {
+    if (ladder8_supported(c) || ladder_supported(c)) {
         // sweeps and the exchanges between them are fused in one launch; launches end at measurements
         while (left > 0) {
             uint64_t run = (uint64_t)left;
             if (meas_every > 0) run = std::min<uint64_t>(run, (uint64_t)meas_every - c->sweeps % (uint64_t)meas_every);
-            const int k = launch_ladder8_pmj(c, c->sweeps, c->exchanges, (int)run, pt_every);
-            if (k < 0) return check_launch(c, "ladder8 kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "ladder8 kernel launch failed");
+            const int k = ladder8_supported(c) ? launch_ladder8_pmj(c, c->sweeps, c->exchanges, (int)run, pt_every)
+                                               : launch_ladder_pmj(c, c->sweeps, (int)run, c->exchanges, pt_every);
+            if (k < 0) return check_launch(c, "ladder kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "ladder kernel launch failed");
             c->launches += k;
             if (pt_every > 0) c->exchanges += (c->sweeps + run) / (uint64_t)pt_every - c->sweeps / (uint64_t)pt_every;
             c->sweeps += run;

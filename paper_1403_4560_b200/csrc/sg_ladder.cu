@@ -24,6 +24,10 @@ struct LadderArgs {
     uint32_t sweep0;          // global index of the first sweep of this launch
     int n_sweeps;
     int G;                    // system groups: thread (q, g) handles systems g, g+G, ...
+    int pt_every;             // > 0: exchanges fused in (after every pt_every-th sweep, global sweep index)
+    uint64_t exchange0;       // global index of the first exchange of this launch
+    const double *exp_tab;    // dexp64 table (R12)
+    double h;
 };
 
 __device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -80,6 +84,63 @@ struct Geo {
     static constexpr int MINB = L == 8 ? 2 : 1;
 };
 
+// Per-lane U (unsatisfied bonds) and M (sum of spins) of one system resident in shared memory, by ONE warp:
+// the six bonds of every colour-0 site cover each bond once; bit-sliced accumulation (flush every 16 sites),
+// then one warp transpose + popc per plane.  Same arithmetic as k_energy_pmj (sg_pmj.cu), compile-time L.
+template <int L>
+__device__ __forceinline__ void ladder_energy(const uint32_t *__restrict__ Ssys, const uint32_t *__restrict__ Jsm, int lane,
+                                              int &U, int &M)
+{
+    constexpr int Lh = L / 2, N = L * L * L, H = N / 2;
+    const uint32_t *s0 = Ssys, *s1 = Ssys + H;
+    const uint32_t *J0 = Jsm, *J1 = Jsm + 3 * H;
+    uint32_t bigU[16], bigM[16], inU[7], inM[6];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) bigU[k] = bigM[k] = 0;
+#pragma unroll
+    for (int k = 0; k < 7; ++k) inU[k] = 0;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) inM[k] = 0;
+    int pending = 0;
+    for (int n = lane; n < H; n += 32) {
+        const int row = n / Lh, m = n - row * Lh;
+        const int z = row / L, y = row - z * L;
+        const int p = (y + z) & 1;                                     // colour 0
+        const int sd = row * Lh + (p ? (m + 1 == Lh ? 0 : m + 1) : (m == 0 ? Lh - 1 : m - 1));
+        const int xp = p ? sd : n, xm = p ? n : sd;
+        const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m, ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
+        const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m, zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
+        const uint32_t sa = s0[n], sb = s1[n];
+        const uint32_t u0 = xor3(sa, s1[xp], J0[n]), u1 = xor3(sa, s1[xm], J1[xm]);
+        const uint32_t u2 = xor3(sa, s1[yp], J0[H + n]), u3 = xor3(sa, s1[ym], J1[H + ym]);
+        const uint32_t u4 = xor3(sa, s1[zp], J0[2 * H + n]), u5 = xor3(sa, s1[zm], J1[2 * H + zm]);
+        const uint32_t a0 = xor3(u0, u1, u2), c0 = maj3(u0, u1, u2);
+        const uint32_t a1 = xor3(u3, u4, u5), c1 = maj3(u3, u4, u5);
+        const uint32_t kk = a0 & a1;
+        const uint32_t x[3] = {a0 ^ a1, xor3(c0, c1, kk), maj3(c0, c1, kk)};
+        bs_add(inU, x);
+        const uint32_t mm[2] = {sa ^ sb, sa & sb};
+        bs_add(inM, mm);
+        if (++pending == 16) {
+            bs_add(bigU, inU);
+            bs_add(bigM, inM);
+#pragma unroll
+            for (int k = 0; k < 7; ++k) inU[k] = 0;
+#pragma unroll
+            for (int k = 0; k < 6; ++k) inM[k] = 0;
+            pending = 0;
+        }
+    }
+    bs_add(bigU, inU);
+    bs_add(bigM, inM);
+    constexpr int per_thread = (H + 31) / 32;
+    int pu = 1, pm = 1;
+    while ((1 << pu) <= 6 * per_thread) ++pu;
+    while ((1 << pm) <= 2 * per_thread) ++pm;
+    U = (int)bs_warp_total(bigU, pu, lane);
+    M = 2 * (int)bs_warp_total(bigM, pm, lane) - N;
+}
+
 template <int L>
 __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const __grid_constant__ LadderArgs A)
 {
@@ -91,6 +152,9 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     uint32_t *S = smem;                                   // [NT][2][H]
     uint32_t *Jsm = S + (size_t)NT * N;                   // [2][3][H]
     uint2 *thr = reinterpret_cast<uint2 *>(Jsm + 3 * N);  // [NT][8]
+    int *Uint = reinterpret_cast<int *>(thr + NT * 8);    // [NT][32]   exchange scratch (pt_every > 0 only)
+    int *Mint = Uint + NT * 32;                           // [NT][32]
+    uint32_t *masks = reinterpret_cast<uint32_t *>(Mint + NT * 32);   // [NT / 2]
 
     const int w = blockIdx.x / d.R, a = blockIdx.x % d.R;
     const int tid = threadIdx.x, nthr = blockDim.x;
@@ -116,6 +180,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     const bool active = g < A.G;
     const uint32_t amask = d.neg_h ? 0xffffffffu : 0u;     // a = s ^ amask ; na = ~a
     const uint32_t wglob = (uint32_t)(w + (d.s_first >> 5));
+    uint64_t exchange = A.exchange0;
 
     for (int sw = 0; sw < A.n_sweeps; ++sw) {
 #pragma unroll 1
@@ -195,12 +260,38 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         reinterpret_cast<uint4 *>(Sa)[q] = make_uint4(out[0], out[1], out[2], out[3]);
                     }
                 } else {
-                    // generic lattice: per-element neighbour indices (compile-time L), couplings from smem
+                    // generic lattice (rows of L/2 words are not whole quads): per-element neighbour indices and the
+                    // 24 coupling words of the quad are computed / loaded once per half sweep and shared by all
+                    // systems of the group
+                    int ix[4][6];
+                    uint32_t Jq[4][6];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int n = 4 * q + e;
+                        const int row = n / Lh, m = n - row * Lh;
+                        const int z = row / L, y = row - z * L;
+                        const int p = (colour + y + z) & 1;
+                        const int sd = row * Lh + (p ? (m + 1 == Lh ? 0 : m + 1) : (m == 0 ? Lh - 1 : m - 1));
+                        const int xp = p ? sd : n, xm = p ? n : sd;
+                        const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m;
+                        const int ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
+                        const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m;
+                        const int zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
+                        ix[e][0] = xp; ix[e][1] = xm; ix[e][2] = yp; ix[e][3] = ym; ix[e][4] = zp; ix[e][5] = zm;
+                        Jq[e][0] = Jown[n];          Jq[e][1] = Joth[xm];
+                        Jq[e][2] = Jown[H + n];      Jq[e][3] = Joth[H + ym];
+                        Jq[e][4] = Jown[2 * H + n];  Jq[e][5] = Joth[2 * H + zm];
+                    }
 #pragma unroll 1
                     for (int t = g; t < NT; t += A.G) {
                         uint32_t *Sa = S + t * N + colour * H;
                         const uint32_t *So = S + t * N + (1 - colour) * H;
                         const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[q];
+                        uint32_t v[4][6];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+#pragma unroll
+                            for (int k = 0; k < 6; ++k) v[e][k] = So[ix[e][k]];
                         const uint4 r4 = philox_rk((uint32_t)q, time, wglob, ctr3(3, a, t), A.rk);
                         uint2 c64[7];
 #pragma unroll
@@ -210,28 +301,64 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         uint32_t out[4];
 #pragma unroll
                         for (int e = 0; e < 4; ++e) {
-                            const int n = 4 * q + e;
-                            const int row = n / Lh, m = n - row * Lh;
-                            const int z = row / L, y = row - z * L;
-                            const int p = (colour + y + z) & 1;
-                            const int sd = row * Lh + (p ? (m + 1 == Lh ? 0 : m + 1) : (m == 0 ? Lh - 1 : m - 1));
-                            const int xp = p ? sd : n, xm = p ? n : sd;
-                            const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m;
-                            const int ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
-                            const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m;
-                            const int zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
                             uint32_t B[7];
 #pragma unroll
                             for (int c = 0; c < 7; ++c) B[c] = lt_mask64(rr[e], c64[c]);
-                            out[e] = flip_word(s[e], xor3(s[e], So[xp], Jown[n]), xor3(s[e], So[xm], Joth[xm]),
-                                               xor3(s[e], So[yp], Jown[H + n]), xor3(s[e], So[ym], Joth[H + ym]),
-                                               xor3(s[e], So[zp], Jown[2 * H + n]), xor3(s[e], So[zm], Joth[2 * H + zm]),
+                            out[e] = flip_word(s[e], xor3(s[e], v[e][0], Jq[e][0]), xor3(s[e], v[e][1], Jq[e][1]),
+                                               xor3(s[e], v[e][2], Jq[e][2]), xor3(s[e], v[e][3], Jq[e][3]),
+                                               xor3(s[e], v[e][4], Jq[e][4]), xor3(s[e], v[e][5], Jq[e][5]),
                                                ~(s[e] ^ amask), B);
                         }
                         reinterpret_cast<uint4 *>(Sa)[q] = make_uint4(out[0], out[1], out[2], out[3]);
                     }
                 }
             }
+            __syncthreads();
+        }
+        // ---- exchange step (R12), all in shared memory
+        if (A.pt_every > 0 && ((uint64_t)A.sweep0 + (uint64_t)sw + 1) % (uint64_t)A.pt_every == 0) {
+            const int lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
+            for (int t = warp; t < NT; t += nwarp) {
+                int U, M;
+                ladder_energy<L>(S + t * N, Jsm, lane, U, M);
+                Uint[t * 32 + lane] = U;
+                Mint[t * 32 + lane] = M;
+            }
+            __syncthreads();
+            const int e1 = (int)(exchange & 1u);
+            const int npairs = (NT - e1) / 2;
+            for (int item = tid; item < npairs * 32; item += nthr) {       // whole warps
+                const int pair = item >> 5, ln = item & 31;
+                const int t = e1 + 2 * pair;
+                const int smp = w * 32 + ln;
+                const int U0 = Uint[t * 32 + ln], U1 = Uint[(t + 1) * 32 + ln];
+                const int M0 = Mint[t * 32 + ln], M1 = Mint[(t + 1) * 32 + ln];
+                const double Et = __dsub_rn((double)(2 * U0 - 3 * N), __dmul_rn(A.h, (double)M0));
+                const double Eu = __dsub_rn((double)(2 * U1 - 3 * N), __dmul_rn(A.h, (double)M1));
+                const double x = __dmul_rn(__dsub_rn(A.tab[t].beta, A.tab[t + 1].beta), __dsub_rn(Et, Eu));
+                const uint4 r = philox_rk(0u, (uint32_t)exchange, (uint32_t)(smp + d.s_first), ctr3(4, a, t), A.rk);
+                const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
+                const uint32_t mask = __ballot_sync(0xffffffffu, accept && smp < d.n_samples);
+                if (ln == 0) masks[pair] = mask;
+            }
+            __syncthreads();
+            for (int item = tid; item < npairs * (N / 4); item += nthr) {  // masked swap of the two configurations
+                const int pair = item / (N / 4), k = item - pair * (N / 4);
+                const uint32_t mask = masks[pair];
+                if (mask == 0u) continue;
+                const int t = e1 + 2 * pair;
+                uint4 *X = reinterpret_cast<uint4 *>(S + t * N) + k;
+                uint4 *Y = reinterpret_cast<uint4 *>(S + (t + 1) * N) + k;
+                uint4 xv = *X, yv = *Y;
+                uint32_t dd;
+                dd = (xv.x ^ yv.x) & mask; xv.x ^= dd; yv.x ^= dd;
+                dd = (xv.y ^ yv.y) & mask; xv.y ^= dd; yv.y ^= dd;
+                dd = (xv.z ^ yv.z) & mask; xv.z ^= dd; yv.z ^= dd;
+                dd = (xv.w ^ yv.w) & mask; xv.w ^= dd; yv.w ^= dd;
+                *X = xv;
+                *Y = yv;
+            }
+            exchange += 1;
             __syncthreads();
         }
     }
@@ -248,7 +375,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
 size_t ladder_smem_bytes(int L, int NT)
 {
     const size_t N = (size_t)L * L * L;
-    return (size_t)NT * N * 4 + 3 * N * 4 + (size_t)NT * 8 * sizeof(uint2);
+    return (size_t)NT * N * 4 + 3 * N * 4 + (size_t)NT * 8 * sizeof(uint2) + (size_t)NT * 32 * 8 + (size_t)(NT / 2 + 1) * 4;
 }
 
 bool ladder_supported(const sg_ctx *c)
@@ -272,8 +399,9 @@ static cudaError_t launch_l(const LadderArgs &A, int threads, size_t smem, cudaS
     return cudaGetLastError();
 }
 
-// n_sweeps consecutive sweeps starting at global sweep index `sweep0`; returns kernels launched (or -1)
-int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps)
+// n_sweeps consecutive sweeps starting at global sweep index `sweep0`, with the exchanges that fall due fused in
+// (pt_every > 0; first exchange index exchange0); returns kernels launched (or -1)
+int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0, int pt_every)
 {
     const Dims &d = c->d;
     LadderArgs A;
@@ -288,6 +416,10 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps)
     A.pad0 = 0;
     A.sweep0 = (uint32_t)sweep0;
     A.n_sweeps = n_sweeps;
+    A.pt_every = pt_every;
+    A.exchange0 = exchange0;
+    A.exp_tab = c->exp64_tab;
+    A.h = c->h;
     const int Q = d.N / 8;
     // groups: as many as fit in <= 512 threads, at most NT, preferring a divisor of NT
     const int maxt = d.L == 8 ? 320 : 512;

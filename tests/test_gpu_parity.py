@@ -274,3 +274,28 @@ def test_estimators_on_device_moments_high_temperature(sg):
         assert np.all(np.abs(out[name] - 1.0) < 0.03 + 5 * out[name + "_err"]), (name, out[name], out[name + "_err"])
     assert np.all(np.abs(out["g_std"]) < 0.01 + 5 * out["g_std_err"])
     sim.close()
+
+
+@pytest.mark.parametrize("L,h,NT,R,pt_every,n_samples", [(4, 0.3, 8, 4, 1, 1), (6, 0.1, 7, 2, 1, 40), (10, -0.2, 4, 4, 3, 33),
+                                                       (12, 0.1, 5, 4, 1, 32), (16, 0.2, 3, 2, 2, 32)])
+def test_generic_ladder_with_fused_pt(sg, O, L, h, NT, R, pt_every, n_samples):
+    """k_ladder_pmj<L> with the exchange step fused in (one warp per system recounts U, M from shared memory,
+    one thread per (pair, lane) decides, masked swap) vs the oracle, across a measurement boundary, then
+    primitives from the same state."""
+    temps = W.ladder(0.5, 1.9, NT)
+    samples = sorted({0, n_samples - 1, n_samples // 2})
+    sim, orc = make_pair(sg, O, L, h, n_samples, R, temps, 0, 31, samples)
+    sim.sg_run(21, pt_every, 8)
+    for o in orc.values():
+        o.run(21, pt_every, 8)
+    check_state(sim, orc, "fused generic ladder")
+    assert sim.sg_get_counters() == (21, 21 // pt_every)
+    mom, n = sim.sg_get_moments()
+    assert n == 2
+    for s, o in orc.items():
+        assert close(mom[s], o.moments()[0])
+    sim.sg_sweep(2); sim.sg_pt_exchange(); sim.sg_run(4, pt_every, 0)
+    for o in orc.values():
+        o.sweep(2); o.pt_exchange(); o.run(4, pt_every, 0)
+    check_state(sim, orc, "fused generic ladder + primitives")
+    sim.close()
