@@ -1,8 +1,9 @@
 // sg_res32.cu — L = 32 (+-J) sweep kernel: ONE system (32768 word-sites = 128 KB) is resident in the
 // shared memory of one SM for all sweeps of a launch (BASELINE.json config 5: 4 sweeps between exchanges),
 // so the spin state crosses HBM once per launch (2 B per word-site and sweep at 4 sweeps) instead of
-// once per half sweep.  The couplings of the packed word (384 KB, shared by its R * NT = 128 systems,
-// which are consecutive CTAs) are streamed from L2 through registers, one quad ahead.
+// once per half sweep; it arrives by eight 16 KB bulk-async copies (TMA) on one mbarrier.  The couplings of
+// the packed word (shared by its R * NT = 128 systems, which are consecutive CTAs, so they stay in L2) stream
+// through per-warp two-stage rings in shared memory, filled by bulk-async copies two warp steps ahead.
 //
 // Layout in shared memory = the canonical colour-compacted layout of global memory
 // ([colour][z][y][16 words], one row = 64 B).  A warp owns 4 "diagonal pairs" of rows
@@ -186,7 +187,8 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
     uint4 *S4 = reinterpret_cast<uint4 *>(smem);                           // [2][RQ]                  128 KB
     uint4 *ring = S4 + 2 * RQ;                                             // [16 warps][2 stages][6][32] 96 KB
     uint64_t *bars = reinterpret_cast<uint64_t *>(ring + R_WARPS * N_STAGES * CHUNK_U4);   // [16][2]
-    int *sUM = reinterpret_cast<int *>(bars + R_WARPS * N_STAGES);         // [2][32]
+    uint64_t *sysbar_p = bars + R_WARPS * N_STAGES;                        // load barrier of the system
+    int *sUM = reinterpret_cast<int *>(sysbar_p + 1);                      // [2][32]
     const Dims &d = A.d;
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);        // warp-uniform for the compiler: uniform datapath
@@ -213,9 +215,19 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
         issue(0, 1);
     }
 
-    // ---- load the system (contiguous 128 KB)
-#pragma unroll 8
-    for (int i = 0; i < 2 * RQ / R_THREADS; ++i) S4[i * R_THREADS + tid] = gS[i * R_THREADS + tid];
+    // ---- load the system (contiguous 128 KB): eight 16 KB bulk-async copies on one mbarrier
+    const uint32_t sysbar = smem_u32(sysbar_p);
+    if (tid == 0) {
+        mbar_init(sysbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(sysbar), "r"(RN * 4) : "memory");
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                             S_s + i * 16384),
+                         "l"(reinterpret_cast<const char *>(gS) + i * 16384), "r"(16384), "r"(sysbar)
+                         : "memory");
+    }
     if (tid < 64) sUM[tid] = 0;
 
     SlotK K;                                                // block-uniform: stays in uniform registers / the constant bank
@@ -229,7 +241,8 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
     const uint32_t c3 = ctr3(3, a, t);
     const Geo32 geo = geo_of(wj, lane);
     const int pi = (wj >> 2) & 1;
-    __syncthreads();
+    __syncthreads();                                        // sysbar initialised, sUM zeroed
+    mbar_wait(sysbar, 0u);                                  // the system has landed (async-proxy writes visible)
 
     auto half_sweep = [&](auto P_tag, auto E_tag, int hs) {
         constexpr int P = decltype(P_tag)::value;
@@ -293,7 +306,7 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
         }
     }
 
-    // ---- write back
+    // ---- write back (plain vector stores: a bulk-async store would hold the CTA until its completion — measured slower)
 #pragma unroll 8
     for (int i = 0; i < 2 * RQ / R_THREADS; ++i) gS[i * R_THREADS + tid] = S4[i * R_THREADS + tid];
 }
@@ -332,7 +345,7 @@ __global__ void __launch_bounds__(256) k_pack_J_res32(Dims d, const uint32_t *__
     Jp[idx] = make_uint4(v[0], v[1], v[2], v[3]);
 }
 
-constexpr size_t RES32_SMEM = (size_t)RN * 4 + (size_t)R_WARPS * N_STAGES * CHUNK_BYTES + R_WARPS * N_STAGES * 8 + 64 * 4;
+constexpr size_t RES32_SMEM = (size_t)RN * 4 + (size_t)R_WARPS * N_STAGES * CHUNK_BYTES + R_WARPS * N_STAGES * 8 + 8 + 64 * 4;
 
 }  // namespace
 
