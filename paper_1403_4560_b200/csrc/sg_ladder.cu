@@ -7,6 +7,7 @@
 // of its quad live in registers across those systems.  Bit-sliced arithmetic as in sg_pmj.cu:
 // per word-site 6 XOR3 + 8 (count) + 8 (accept/flip) + 5 (Philox share) = 27 ALU-pipe lane-ops; the
 // seven "r < thr" masks and the Philox products are IMAD.WIDE on the FMA pipe.
+#include "sg_accept.cuh"
 #include "sg_device.cuh"
 #include "sg_internal.h"
 
@@ -28,6 +29,7 @@ struct LadderArgs {
     uint64_t exchange0;       // global index of the first exchange of this launch
     const double *exp_tab;    // dexp64 table (R12)
     double h;
+    uint32_t one, mone;       // run-time 1 and 0xFFFFFFFF (sg_accept.cuh)
 };
 
 __device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -169,9 +171,17 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
         const uint4 *js = reinterpret_cast<const uint4 *>(gJ);
         uint4 *jd = reinterpret_cast<uint4 *>(Jsm);
         for (int i = tid; i < 3 * N / 4; i += nthr) jd[i] = js[i];
-        for (int i = tid; i < NT * 8; i += nthr) {
-            const int t = i >> 3, c = i & 7;
-            thr[i] = c < 7 ? A.tab[t].c64[c] : make_uint2(0u, 0u);
+        for (int t = tid; t < NT; t += nthr) {                 // acceptance constants (SlotK of sg_accept.cuh)
+            uint32_t lo[7], zc[7];
+            for (int c = 0; c < 7; ++c) {
+                const uint2 v = A.tab[t].c64[c];               // (0 - thr) as 64 bits: hi = 0 only for thr = 0
+                lo[c] = v.x;
+                zc[c] = v.y == 0u ? 1u : 0u;
+            }
+            uint4 *k4 = reinterpret_cast<uint4 *>(thr + t * 8);
+            k4[0] = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+            k4[1] = make_uint4(lo[4], lo[5], lo[6], zc[3] - 1u);
+            k4[2] = make_uint4(zc[1] + zc[5] - 1u, zc[0] + zc[2] + zc[4] + zc[6] - 2u, 0u, 0u);
         }
     }
     __syncthreads();
@@ -238,9 +248,14 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         const uint4 ozm = reinterpret_cast<const uint4 *>(So)[q_zm];
                         const uint32_t os[4] = {So[side[0]], So[side[1]], So[side[2]], So[side[3]]};
                         const uint4 r4 = philox_rk((uint32_t)q, time, wglob, ctr3(3, a, t), A.rk);
-                        uint2 c64[7];
-#pragma unroll
-                        for (int c = 0; c < 7; ++c) c64[c] = thr[t * 8 + c];
+                        SlotK K;
+                        {
+                            const uint4 *k4 = reinterpret_cast<const uint4 *>(thr + t * 8);
+                            const uint4 k0 = k4[0], k1 = k4[1], k2 = k4[2];
+                            K.lo[0] = k0.x; K.lo[1] = k0.y; K.lo[2] = k0.z; K.lo[3] = k0.w;
+                            K.lo[4] = k1.x; K.lo[5] = k1.y; K.lo[6] = k1.z; K.b3c = k1.w;
+                            K.nc = k2.x; K.ec = k2.y;
+                        }
                         const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
                         const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
                         const uint32_t v0[4] = {o0.x, o0.y, o0.z, o0.w}, vyp[4] = {oyp.x, oyp.y, oyp.z, oyp.w};
@@ -248,15 +263,11 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         const uint32_t vzm[4] = {ozm.x, ozm.y, ozm.z, ozm.w};
                         uint32_t out[4];
 #pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            uint32_t B[7];
-#pragma unroll
-                            for (int c = 0; c < 7; ++c) B[c] = lt_mask64(rr[e], c64[c]);
-                            out[e] = flip_word(s[e], xor3(s[e], v0[e], JA[e]), xor3(s[e], os[e], JB[e]),
-                                               xor3(s[e], vyp[e], Jyp[e]), xor3(s[e], vym[e], Jym[e]),
-                                               xor3(s[e], vzp[e], Jzp[e]), xor3(s[e], vzm[e], Jzm[e]),
-                                               ~(s[e] ^ amask), B);
-                        }
+                        for (int e = 0; e < 4; ++e)
+                            out[e] = flip_word_k(s[e], amask, xor3(s[e], v0[e], JA[e]), xor3(s[e], os[e], JB[e]),
+                                                 xor3(s[e], vyp[e], Jyp[e]), xor3(s[e], vym[e], Jym[e]),
+                                                 xor3(s[e], vzp[e], Jzp[e]), xor3(s[e], vzm[e], Jzm[e]), rr[e], K, A.one,
+                                                 A.mone);
                         reinterpret_cast<uint4 *>(Sa)[q] = make_uint4(out[0], out[1], out[2], out[3]);
                     }
                 } else {
@@ -272,13 +283,15 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         const int z = row / L, y = row - z * L;
                         const int p = (colour + y + z) & 1;
                         const int sd = row * Lh + (p ? (m + 1 == Lh ? 0 : m + 1) : (m == 0 ? Lh - 1 : m - 1));
-                        const int xp = p ? sd : n, xm = p ? n : sd;
                         const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m;
                         const int ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
                         const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m;
                         const int zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
-                        ix[e][0] = xp; ix[e][1] = xm; ix[e][2] = yp; ix[e][3] = ym; ix[e][4] = zp; ix[e][5] = zm;
-                        Jq[e][0] = Jown[n];          Jq[e][1] = Joth[xm];
+                        // slot 0: the x-neighbour at the same compact index (its bond if p, own bond else); slot 1: the one
+                        // at the side index (own bond if p, its bond else)
+                        ix[e][0] = n; ix[e][1] = sd; ix[e][2] = yp; ix[e][3] = ym; ix[e][4] = zp; ix[e][5] = zm;
+                        Jq[e][0] = p ? Joth[n] : Jown[n];
+                        Jq[e][1] = p ? Jown[n] : Joth[sd];
                         Jq[e][2] = Jown[H + n];      Jq[e][3] = Joth[H + ym];
                         Jq[e][4] = Jown[2 * H + n];  Jq[e][5] = Joth[2 * H + zm];
                     }
@@ -288,27 +301,47 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         const uint32_t *So = S + t * N + (1 - colour) * H;
                         const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[q];
                         uint32_t v[4][6];
+                        if constexpr (Lh % 2 == 0) {
+                            // even rows: elements (0,1) and (2,3) sit in one row at an even index, so every neighbour
+                            // except the side one is an aligned 64-bit pair
 #pragma unroll
-                        for (int e = 0; e < 4; ++e)
+                            for (int e = 0; e < 4; e += 2) {
 #pragma unroll
-                            for (int k = 0; k < 6; ++k) v[e][k] = So[ix[e][k]];
+                                for (int k = 0; k < 6; ++k) {
+                                    if (k == 1) {
+                                        v[e][1] = So[ix[e][1]];
+                                        v[e + 1][1] = So[ix[e + 1][1]];
+                                    } else {
+                                        const uint2 pr = *reinterpret_cast<const uint2 *>(So + ix[e][k]);
+                                        v[e][k] = pr.x;
+                                        v[e + 1][k] = pr.y;
+                                    }
+                                }
+                            }
+                        } else {
+#pragma unroll
+                            for (int e = 0; e < 4; ++e)
+#pragma unroll
+                                for (int k = 0; k < 6; ++k) v[e][k] = So[ix[e][k]];
+                        }
                         const uint4 r4 = philox_rk((uint32_t)q, time, wglob, ctr3(3, a, t), A.rk);
-                        uint2 c64[7];
-#pragma unroll
-                        for (int c = 0; c < 7; ++c) c64[c] = thr[t * 8 + c];
+                        SlotK K;
+                        {
+                            const uint4 *k4 = reinterpret_cast<const uint4 *>(thr + t * 8);
+                            const uint4 k0 = k4[0], k1 = k4[1], k2 = k4[2];
+                            K.lo[0] = k0.x; K.lo[1] = k0.y; K.lo[2] = k0.z; K.lo[3] = k0.w;
+                            K.lo[4] = k1.x; K.lo[5] = k1.y; K.lo[6] = k1.z; K.b3c = k1.w;
+                            K.nc = k2.x; K.ec = k2.y;
+                        }
                         const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
                         const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
                         uint32_t out[4];
 #pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            uint32_t B[7];
-#pragma unroll
-                            for (int c = 0; c < 7; ++c) B[c] = lt_mask64(rr[e], c64[c]);
-                            out[e] = flip_word(s[e], xor3(s[e], v[e][0], Jq[e][0]), xor3(s[e], v[e][1], Jq[e][1]),
-                                               xor3(s[e], v[e][2], Jq[e][2]), xor3(s[e], v[e][3], Jq[e][3]),
-                                               xor3(s[e], v[e][4], Jq[e][4]), xor3(s[e], v[e][5], Jq[e][5]),
-                                               ~(s[e] ^ amask), B);
-                        }
+                        for (int e = 0; e < 4; ++e)
+                            out[e] = flip_word_k(s[e], amask, xor3(s[e], v[e][0], Jq[e][0]), xor3(s[e], v[e][1], Jq[e][1]),
+                                                 xor3(s[e], v[e][2], Jq[e][2]), xor3(s[e], v[e][3], Jq[e][3]),
+                                                 xor3(s[e], v[e][4], Jq[e][4]), xor3(s[e], v[e][5], Jq[e][5]), rr[e], K, A.one,
+                                                 A.mone);
                         reinterpret_cast<uint4 *>(Sa)[q] = make_uint4(out[0], out[1], out[2], out[3]);
                     }
                 }
@@ -420,6 +453,8 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchang
     A.exchange0 = exchange0;
     A.exp_tab = c->exp64_tab;
     A.h = c->h;
+    A.one = 1u;
+    A.mone = 0xffffffffu;
     const int Q = d.N / 8;
     // groups: as many as fit in <= 512 threads, at most NT, preferring a divisor of NT
     const int maxt = d.L == 8 ? 320 : 512;
