@@ -267,14 +267,17 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
             Jq.ym = lds128(jc + 1536);
             Jq.zp = lds128(jc + 2048);
             Jq.zm = lds128(jc + 2560);
-            __syncwarp();                                   // every lane has read the stage: refill it two steps ahead
+            const uint32_t qb = geo.tb + 4096u * (uint32_t)(2 * it + zhalf);
+            quad_update<P, ENERGY>(sa, so, qb, geo, Jq, philox_rk8(qb >> 4, time, wglob, c3, A.rk), K, amask, A.one,
+                                   A.mone, lane, accU, accM);
+            // Refill the stage two steps ahead only now: every lane has CONSUMED its coupling registers, so the
+            // shared-memory loads of the stage have completed (a load that is merely issued could still be in the
+            // LSU queue when the bulk copy, which runs on a different engine, overwrites the stage).
+            __syncwarp();
             if (lane == 0) {
                 if (it + 2 < R_ITERS) issue(hs, it + 2);
                 else if (hs + 1 < n_half) issue(hs + 1, it + 2 - R_ITERS);
             }
-            const uint32_t qb = geo.tb + 4096u * (uint32_t)(2 * it + zhalf);
-            quad_update<P, ENERGY>(sa, so, qb, geo, Jq, philox_rk8(qb >> 4, time, wglob, c3, A.rk), K, amask, A.one,
-                                   A.mone, lane, accU, accM);
         }
         if constexpr (ENERGY) {                             // per-lane totals of this warp -> CTA totals
             const uint32_t totU = bs_warp_total(accU, 8, lane);
