@@ -31,8 +31,8 @@ ALU_OPS_PER_WORDSITE = 30     # algorithmic ALU-pipe lane-ops per 32-sample word
 #                               6 bond XOR3 + 8 count + 7 threshold carries + 4 compare/flip + 5 Philox share
 HBM_BYTES_PER_WORDSITE_LAUNCH = 8   # spin word read once + written once per LAUNCH of a resident kernel
 # dram__bytes_read.sum + dram__bytes_write.sum of the roofline launch below, from the ncu --set full captures
-# summarised in profiles/r01_v3_resident_kernels.md (same command line as the default run of this file)
-NCU_TRAFFIC_BYTES = {"C2": 10.92e6, "C5": 8.747e9}
+# summarised in profiles/r01_v3_resident_kernels.md (C2) and profiles/r01_v4_final_kernels.md (C3, C5)
+NCU_TRAFFIC_BYTES = {"C2": 10.92e6, "C3": 114.6e6, "C5": 8.746e9}
 ALU_LANES_PER_SM = 64         # INT/LOP3 lanes per SM per clock (16 per SMSP x 4; B300_MICROARCH pipe table)
 N_SM = 148
 
