@@ -232,6 +232,13 @@ int do_sweeps(sg_ctx *c, int n, bool energy_after = false, bool *fresh = nullptr
         c->sweeps += n;
         return SG_OK;
     }
+    if (gladder_supported(c)) {
+        const int k = launch_gladder(c, c->sweeps, n);
+        if (k < 0) return check_launch(c, "gauss ladder kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "gauss ladder kernel launch failed");
+        c->launches += k;
+        c->sweeps += n;
+        return SG_OK;
+    }
     if (ladder_supported(c)) {
         const int k = launch_ladder_pmj(c, c->sweeps, n);
         if (k < 0) return check_launch(c, "ladder kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "ladder kernel launch failed");
@@ -373,13 +380,14 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
     if (!c) return SG_EINVAL;
     if (n_sweeps < 0 || pt_every < 0 || meas_every < 0) return fail(c, SG_EINVAL, "sg_run: negative argument");
     int left = n_sweeps;
-    if (ladder8_supported(c) || ladder_supported(c)) {
+    if (ladder8_supported(c) || ladder_supported(c) || gladder_supported(c)) {
         // sweeps and the exchanges between them are fused in one launch; launches end at measurements
         while (left > 0) {
             uint64_t run = (uint64_t)left;
             if (meas_every > 0) run = std::min<uint64_t>(run, (uint64_t)meas_every - c->sweeps % (uint64_t)meas_every);
             const int k = ladder8_supported(c) ? launch_ladder8_pmj(c, c->sweeps, c->exchanges, (int)run, pt_every)
-                                               : launch_ladder_pmj(c, c->sweeps, (int)run, c->exchanges, pt_every);
+                          : gladder_supported(c) ? launch_gladder(c, c->sweeps, (int)run, c->exchanges, pt_every)
+                                                 : launch_ladder_pmj(c, c->sweeps, (int)run, c->exchanges, pt_every);
             if (k < 0) return check_launch(c, "ladder kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "ladder kernel launch failed");
             c->launches += k;
             if (pt_every > 0) c->exchanges += (c->sweeps + run) / (uint64_t)pt_every - c->sweeps / (uint64_t)pt_every;

@@ -81,6 +81,8 @@ int launch_sweep_pmj(sg_ctx *c, uint64_t sweep);            // both colours
 int launch_sweep_gauss(sg_ctx *c, uint64_t sweep);
 bool ladder_supported(const sg_ctx *c);                    // shared-memory-resident ladder kernel usable?
 int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0 = 0, int pt_every = 0);   // 1 launch (-1 on error)
+bool gladder_supported(const sg_ctx *c);                   // Gaussian ladder kernel (L = 8, 16) with fused exchanges
+int launch_gladder(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0 = 0, int pt_every = 0);   // 1 launch (-1 on error)
 bool ladder8_supported(const sg_ctx *c);                   // L = 8 kernel with fused parallel tempering
 int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_sweeps, int pt_every);
 bool res32_supported(const sg_ctx *c);                     // L = 32: one system resident per SM, couplings streamed from L2

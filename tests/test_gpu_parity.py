@@ -299,3 +299,27 @@ def test_generic_ladder_with_fused_pt(sg, O, L, h, NT, R, pt_every, n_samples):
         o.sweep(2); o.pt_exchange(); o.run(4, pt_every, 0)
     check_state(sim, orc, "fused generic ladder + primitives")
     sim.close()
+
+
+@pytest.mark.parametrize("L,h,NT,R,pt_every,n_samples", [(8, 0.3, 8, 4, 1, 3), (8, -0.2, 5, 2, 2, 2), (16, 0.3, 6, 2, 1, 2)])
+def test_gaussian_ladder_with_fused_pt(sg, O, L, h, NT, R, pt_every, n_samples):
+    """k_gladder<L>: the Gaussian fp32 ladder resident in shared memory with the exchange step fused in
+    (fixed-point energies, R14) vs the oracle — spins and E_fix bit-exact, moments to 1e-12 — across a
+    measurement boundary, then primitives from the same state."""
+    temps = W.ladder(0.2, 1.5, NT)
+    samples = list(range(n_samples))
+    sim, orc = make_pair(sg, O, L, h, n_samples, R, temps, 1, 41, samples)
+    sim.sg_run(13, pt_every, 4)
+    for o in orc.values():
+        o.run(13, pt_every, 4)
+    check_state(sim, orc, "fused Gaussian ladder")
+    assert sim.sg_get_counters() == (13, 13 // pt_every)
+    mom, n = sim.sg_get_moments()
+    assert n == 3
+    for s, o in orc.items():
+        assert close(mom[s], o.moments()[0])
+    sim.sg_sweep(2); sim.sg_pt_exchange(); sim.sg_run(3, pt_every, 0)
+    for o in orc.values():
+        o.sweep(2); o.pt_exchange(); o.run(3, pt_every, 0)
+    check_state(sim, orc, "fused Gaussian ladder + primitives")
+    sim.close()
