@@ -154,36 +154,66 @@ __global__ void __launch_bounds__(512, 1) k_gladder(const __grid_constant__ GLad
         }
         // ---- exchange step (R12, R14), all in shared memory
         if (A.pt_every > 0 && ((uint64_t)A.sweep0 + (uint64_t)sw + 1) % (uint64_t)A.pt_every == 0) {
-            const int lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
+            // Energies: threads stride over the colour-0 sites (their six bonds cover every bond once); the six
+            // fixed-point couplings of a site are converted once and used for a chunk of 16 systems, whose partial
+            // sums live in registers; warp shuffle + one shared-memory atomic per (warp, system) finish the sums.
+            const int lane = tid & 31;
             const float *J0 = Jsm, *J1 = Jsm + 3 * H;
-            for (int t = warp; t < NT; t += nwarp) {
-                const int8_t *s0 = S + (size_t)t * N, *s1 = s0 + H;
-                long long e = 0;
-                int m = 0;
-                for (int n = lane; n < H; n += 32) {
-                    const int row = n / Lh, mm = n - row * Lh;
+            for (int t = tid; t < NT; t += nthr) { Efix[t] = 0; Msum[t] = 0; }
+            __syncthreads();
+            constexpr int TCH = 16;
+            for (int t0 = 0; t0 < NT; t0 += TCH) {
+                long long acc[TCH];
+                int mm[TCH];
+#pragma unroll
+                for (int k = 0; k < TCH; ++k) { acc[k] = 0; mm[k] = 0; }
+                for (int n = tid; n < H; n += nthr) {
+                    const int row = n / Lh, mi = n - row * Lh;
                     const int z = row / L, y = row - z * L;
                     const int p = (y + z) & 1;
-                    const int sd = row * Lh + (p ? (mm + 1 == Lh ? 0 : mm + 1) : (mm == 0 ? Lh - 1 : mm - 1));
+                    const int sd = row * Lh + (p ? (mi + 1 == Lh ? 0 : mi + 1) : (mi == 0 ? Lh - 1 : mi - 1));
                     const int xp = p ? sd : n, xm = p ? n : sd;
-                    const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + mm, ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + mm;
-                    const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + mm, zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + mm;
-                    const int si = s0[n];
-                    m += si + s1[n];
-                    long long acc = 0;
-                    acc += __double2ll_rz(__dmul_rn((double)J0[n], 4294967296.0)) * (long long)(si * s1[xp]);
-                    acc += __double2ll_rz(__dmul_rn((double)J1[xm], 4294967296.0)) * (long long)(si * s1[xm]);
-                    acc += __double2ll_rz(__dmul_rn((double)J0[H + n], 4294967296.0)) * (long long)(si * s1[yp]);
-                    acc += __double2ll_rz(__dmul_rn((double)J1[H + ym], 4294967296.0)) * (long long)(si * s1[ym]);
-                    acc += __double2ll_rz(__dmul_rn((double)J0[2 * H + n], 4294967296.0)) * (long long)(si * s1[zp]);
-                    acc += __double2ll_rz(__dmul_rn((double)J1[2 * H + zm], 4294967296.0)) * (long long)(si * s1[zm]);
-                    e -= acc;
+                    const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + mi, ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + mi;
+                    const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + mi, zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + mi;
+                    const long long jf0 = __double2ll_rz(__dmul_rn((double)J0[n], 4294967296.0));
+                    const long long jf1 = __double2ll_rz(__dmul_rn((double)J1[xm], 4294967296.0));
+                    const long long jf2 = __double2ll_rz(__dmul_rn((double)J0[H + n], 4294967296.0));
+                    const long long jf3 = __double2ll_rz(__dmul_rn((double)J1[H + ym], 4294967296.0));
+                    const long long jf4 = __double2ll_rz(__dmul_rn((double)J0[2 * H + n], 4294967296.0));
+                    const long long jf5 = __double2ll_rz(__dmul_rn((double)J1[2 * H + zm], 4294967296.0));
+#pragma unroll
+                    for (int k = 0; k < TCH; ++k) {
+                        const int t = t0 + k;
+                        if (t < NT) {
+                            const int8_t *s0 = S + (size_t)t * N, *s1 = s0 + H;
+                            const int si = s0[n];
+                            mm[k] += si + s1[n];
+                            long long a8 = 0;
+                            a8 += (si ^ s1[xp]) < 0 ? -jf0 : jf0;          // J_fix * S_i * S_j, S = +-1
+                            a8 += (si ^ s1[xm]) < 0 ? -jf1 : jf1;
+                            a8 += (si ^ s1[yp]) < 0 ? -jf2 : jf2;
+                            a8 += (si ^ s1[ym]) < 0 ? -jf3 : jf3;
+                            a8 += (si ^ s1[zp]) < 0 ? -jf4 : jf4;
+                            a8 += (si ^ s1[zm]) < 0 ? -jf5 : jf5;
+                            acc[k] -= a8;
+                        }
+                    }
                 }
-                for (int o = 16; o; o >>= 1) {
-                    e += __shfl_xor_sync(0xffffffffu, e, o);
-                    m += __shfl_xor_sync(0xffffffffu, m, o);
+#pragma unroll
+                for (int k = 0; k < TCH; ++k) {
+                    if (t0 + k < NT) {                                     // uniform
+                        long long e = acc[k];
+                        int m = mm[k];
+                        for (int o = 16; o; o >>= 1) {
+                            e += __shfl_xor_sync(0xffffffffu, e, o);
+                            m += __shfl_xor_sync(0xffffffffu, m, o);
+                        }
+                        if (lane == 0) {
+                            atomicAdd(reinterpret_cast<unsigned long long *>(&Efix[t0 + k]), (unsigned long long)e);
+                            atomicAdd(&Msum[t0 + k], m);
+                        }
+                    }
                 }
-                if (lane == 0) { Efix[t] = e; Msum[t] = m; }
             }
             __syncthreads();
             const int e1 = (int)(exchange & 1u);
