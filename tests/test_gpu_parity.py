@@ -323,3 +323,23 @@ def test_gaussian_ladder_with_fused_pt(sg, O, L, h, NT, R, pt_every, n_samples):
         o.sweep(2); o.pt_exchange(); o.run(3, pt_every, 0)
     check_state(sim, orc, "fused Gaussian ladder + primitives")
     sim.close()
+
+
+@pytest.mark.parametrize("L,n_samples", [(6, 33), (8, 32), (10, 32)])
+def test_paper_shapes_56_temperatures_two_replicas(sg, O, L, n_samples):
+    """The paper's own run shape (Table I): N_T = 56 temperatures geometric in beta in [0.1, 1.8],
+    h = 0.1, 2 replicas, PT every sweep — bit-exact vs the oracle on a few samples, moments to 1e-12."""
+    temps = W.ladder(1.0 / 1.8, 1.0 / 0.1, 56)
+    samples = [0, n_samples - 1]
+    sim, orc = make_pair(sg, O, L, 0.1, n_samples, 2, temps, 0, 1403, samples)
+    sim.sg_run(10, 1, 0)
+    sim.sg_run(10, 1, 5)
+    for o in orc.values():
+        o.run(10, 1, 0)
+        o.run(10, 1, 5)
+    check_state(sim, orc, "paper shape L=%d" % L)
+    mom, n = sim.sg_get_moments()
+    assert n == 2
+    for s, o in orc.items():
+        assert close(mom[s], o.moments()[0])
+    sim.close()
