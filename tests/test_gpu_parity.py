@@ -343,3 +343,42 @@ def test_paper_shapes_56_temperatures_two_replicas(sg, O, L, n_samples):
     for s, o in orc.items():
         assert close(mom[s], o.moments()[0])
     sim.close()
+
+
+def _fuzz_cases():
+    rng = np.random.default_rng(4560)
+    cases = []
+    for i in range(14):
+        kind = 1 if i % 5 == 4 else 0
+        L = int(rng.choice([4, 6, 8] if kind else [4, 6, 8, 10, 12, 16]))
+        NT = int(rng.integers(2, 10))
+        R = int(rng.choice([2, 4]))
+        h = float(rng.choice([0.0, 0.1, -0.25, 0.7, 1.0, -1.0, 1.3]))
+        pt_every = int(rng.choice([0, 1, 1, 2, 3]))
+        meas_every = int(rng.choice([0, 3, 4]))
+        ns = int(rng.integers(1, 5)) if kind else int(rng.choice([1, 31, 32, 33, 64, 70]))
+        n1, n2 = int(rng.integers(1, 8)), int(rng.integers(1, 8))
+        cases.append((L, h, ns, R, NT, kind, 100 + i, pt_every, meas_every, n1, n2))
+    return cases
+
+
+@pytest.mark.parametrize("case", _fuzz_cases(), ids=lambda c: "L%d-h%g-ns%d-R%d-NT%d-k%d-pt%d-m%d" % (c[0], c[1], c[2], c[3], c[4], c[5], c[7], c[8]))
+def test_fuzzed_shapes_run_vs_oracle(sg, O, case):
+    """Seeded random shapes through sg_run (every fused / fallback kernel path, ragged sample counts, odd ladders,
+    both signs of h, |h| > 1 general acceptance): two consecutive runs vs the oracle, bit-exact."""
+    L, h, ns, R, NT, kind, seed, pt_every, meas_every, n1, n2 = case
+    temps = W.ladder(0.45, 2.2, NT)
+    samples = sorted({0, ns - 1, ns // 2})
+    sim, orc = make_pair(sg, O, L, h, ns, R, temps, kind, seed, samples)
+    for n in (n1, n2):
+        sim.sg_run(n, pt_every, meas_every)
+        for o in orc.values():
+            o.run(n, pt_every, meas_every)
+        check_state(sim, orc, "fuzz after %d sweeps" % n)
+    mom, nm = sim.sg_get_moments()
+    for s, o in orc.items():
+        want, no = o.moments()
+        assert no == nm
+        assert close(mom[s], want)
+    assert sim.sg_get_counters()[0] == n1 + n2
+    sim.close()
