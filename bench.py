@@ -311,7 +311,7 @@ def run_ours(args, w):
             cores = os.cpu_count() or 1
             threads = min(cores, 32)
             per_sweep = w.N * w.n_replicas * w.n_temps * 40e-9
-            n_sw = int(max(32, min(w.n_sweeps, 12.0 / per_sweep)))
+            n_sw = int(max(32, min(w.n_sweeps, 45.0 / per_sweep)))        # ~10-20 s of CPU work (the oracle runs ~12 ns per attempt)
             n_sw -= n_sw % 32
             r, dt = oracle_rate(w, threads, n_sw, threads)
             out["cpu_baseline"] = {"value": r, "unit": "flips/ns", "cores": threads, "kind": "oracle",
