@@ -21,7 +21,8 @@
  * Pins (tests/test_oracle_*.py): Philox known answers; threshold-table worked example;
  * exact enumeration on 2x2x2 and 2x2x3; tracked energy == recomputed energy; gauge
  * covariance; (h,S)->(-h,-S) covariance; beta=0 and beta=inf limits; stripe closed form
- * and Parseval for q(k); dexp/dlog/dsincos vs libm; Gaussian moments.
+ * and Parseval for q(k); dexp/dlog/dsincos vs libm; Gaussian moments; the draw <-> site
+ * keying of sweep_once and the PT draw keying followed by hand (tests/test_oracle_keying.py).
  * Parity unpinned (conventions, not results): choice of random initial state, PT pair
  * schedule, measurement cadence — see DESIGN.md §3.
  *
@@ -76,7 +77,7 @@ static void draw4(const uint32_t key[2], uint32_t index, uint32_t time, uint32_t
 /* DESIGN.md R12: written sequences of IEEE-754 operations (every multiply and add rounded
  * separately; this file is compiled with -ffp-contract=off).  They define the method's
  * exponentials / Box-Muller transcendentals so that a second implementation can reproduce
- * them bit for bit; accuracy vs libm is pinned in tests/test_oracle_math.py. */
+ * them bit for bit; accuracy vs libm is pinned in tests/test_oracle_rng_math.py. */
 
 /* 2^32 * exp(-y) rounded down, for y > 0; table[i] = exp(-i/256) from libm. */
 static uint64_t dexp64_tab(const double *table, double y)
@@ -623,7 +624,7 @@ void ea_get_pt_stats(const ea_oracle *o, uint64_t *proposed, uint64_t *accepted)
     *proposed = o->n_pt_prop; *accepted = o->n_pt_acc;
 }
 
-/* time series for the equilibrium pins (tests/test_oracle_enumeration.py): after every sweep
+/* time series for the equilibrium pins (tests/test_oracle_equilibrium.py): after every sweep
  * (and PT step, if due) record the literal Eq.-1 energy inputs (U, M) of every system and the
  * integer overlap Q_t = sum_j S^0_j S^1_j of replicas 0 and 1 at every slot. */
 void ea_run_series(ea_oracle *o, int n_sweeps, int pt_every, int64_t *U_out, int32_t *M_out, int32_t *Q_out)
