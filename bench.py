@@ -37,6 +37,21 @@ ALU_LANES_PER_SM = 64         # INT/LOP3 lanes per SM per clock (16 per SMSP x 4
 N_SM = 148
 
 
+def probe_alu_peak(stream):
+    """Measured ALU-pipe (LOP3) peak in lane-ops/s: bench-only micro-benchmark (csrc/probe/alu_probe.cu),
+    a library of its own, not part of the product ABI."""
+    import ctypes as C
+    from paper_1403_4560_b200 import build
+    lib = C.CDLL(build.build_probe())
+    lib.sgprobe_alu_peak.restype = C.c_int
+    lib.sgprobe_alu_peak.argtypes = [C.c_void_p, C.c_void_p]
+    v = C.c_double()
+    rc = lib.sgprobe_alu_peak(C.c_void_p(stream.cuda_stream), C.byref(v))
+    if rc != 0:
+        raise RuntimeError("sgprobe_alu_peak failed: %d" % rc)
+    return v.value
+
+
 def peaks():
     p = {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback"}
     try:
@@ -236,7 +251,7 @@ def run_ours(args, w):
     sweep_launches = sim.sg_get_launch_count() - l0
     sweep_ms = float(sum(a.elapsed_time(b) for a, b in kev)) / reps          # per n_k sweeps
     sweep_launches //= reps
-    alu_peak_measured = sg.sg_probe_alu_peak(stream) / 1e12                  # T lane-ops/s, LOP3 micro-benchmark
+    alu_peak_measured = probe_alu_peak(stream) / 1e12                  # T lane-ops/s, LOP3 micro-benchmark
     sampler.stop_flag = True
     sampler.join()
 
@@ -286,7 +301,7 @@ def run_ours(args, w):
         hbm_ach = HBM_BYTES_PER_WORDSITE_LAUNCH * wordsites_per_sweep / launch_s / 1e9 if w.kind == W.PMJ else None
         roofline = {"bound": "alu", "kernel": "sweep (+-J multispin)", "achieved": ach, "peak": peak, "unit": "Tlaneop/s",
                     "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(w.name),
-                    "peak_source": "measured in this run: dependency-free LOP3 micro-benchmark (sg_probe_alu_peak); "
+                    "peak_source": "measured in this run: dependency-free LOP3 micro-benchmark (csrc/probe/alu_probe.cu); "
                                    "nominal 64 INT lanes/SM/clk x 148 SMs x %.0f MHz = %.2f" % (pk["sm_max_mhz"], nominal),
                     "peak_nominal": nominal, "frac_of_nominal": ach / nominal,
                     "alu_ops_per_wordsite": ALU_OPS_PER_WORDSITE, "launch_us": 1e6 * launch_s,

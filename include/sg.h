@@ -62,7 +62,8 @@ size_t sg_workspace_bytes(int L, int n_samples, int n_replicas, int n_temps, int
  *   h             external field, any finite double
  *   n_samples     >= 1 disorder samples; the +-J path packs 32 per uint32 (idle lanes are ignored)
  *   n_replicas    2 or 4 replicas per (sample, temperature) (R9)
- *   temps         host ptr, n_temps temperatures T > 0, non-decreasing (slot 0 coldest); copied
+ *   temps         host ptr, n_temps temperatures T > 0, non-decreasing (slot 0 coldest; equal neighbours
+ *                 are allowed: every proposed swap between them is accepted); copied
  *   n_temps       1 <= n_temps <= 64
  *   coupling_kind SG_PMJ or SG_GAUSS
  *   workspace     device ptr, 256-byte aligned, >= sg_workspace_bytes(...) bytes, must outlive the
@@ -85,7 +86,8 @@ int sg_set_first_sample(sg_ctx *ctx, int64_t first_sample);
 int sg_reset(sg_ctx *ctx);
 
 /* n >= 0 full checkerboard Metropolis sweeps of every system, colour 0 then colour 1 (R2, R3),
- * no exchange, no measurement.  Asynchronous. */
+ * no exchange, no measurement.  Asynchronous.  The global sweep counter must stay below 2^31
+ * (the Philox time word is 2 * sweep + colour, R6): SG_EINVAL beyond that (also for sg_run). */
 int sg_sweep(sg_ctx *ctx, int n);
 
 /* One parallel-tempering exchange step: pairs (t, t+1) with t = e mod 2 for the e-th call (R12),
@@ -135,11 +137,34 @@ int sg_get_counters(sg_ctx *ctx, uint64_t *sweeps_done, uint64_t *exchanges_done
 /* number of kernels this context has launched so far (for bench.py's gpu_launches) */
 int sg_get_launch_count(sg_ctx *ctx, uint64_t *launches);
 
-/* Measured peak of the ALU (INT/LOP3) pipe of the current device: a dependency-free LOP3 micro-benchmark
- * (8 independent chains per thread, 2 x 1024 threads per SM, no memory traffic; best of 5 launches, ~10 ms
- * each) on `cuda_stream` (NULL = default stream).  *lane_ops_per_s = 32-bit lane operations per second.
- * This is the denominator of bench.py's "alu" roofline.  Synchronous. */
-int sg_probe_alu_peak(void *cuda_stream, double *lane_ops_per_s);
+/* ---- cross-checks and diagnostics of the exchange step ---- */
+
+/* Kernel-path selection.  SG_PATH_AUTO (default) picks the fastest kernels for the shape (ladders or
+ * systems resident in shared memory, exchanges fused in); SG_PATH_GENERIC forces the plain
+ * global-memory kernels (one launch per half sweep, separate energy / decision / swap / histogram
+ * kernels).  Both paths compute the same trajectory bit for bit; the GPU tests compare them over the
+ * whole pool through sg_get_state_hash.  May be changed at any time between calls. */
+enum { SG_PATH_AUTO = 0, SG_PATH_GENERIC = 1 };
+int sg_set_kernel_path(sg_ctx *ctx, int path);
+
+/* One 64-bit hash per system (spin configuration of one packed word / sample, replica, slot):
+ * the sum over the system's 32-bit words of mix64(index, word) — independent of the order in which
+ * the words are visited.  out: HOST ptr, [n_words][n_replicas][n_temps] with n_words =
+ * ceil(n_samples / 32) for SG_PMJ (all 32 lanes of a word, idle lanes included) and n_samples for
+ * SG_GAUSS.  Synchronous. */
+int sg_get_state_hash(sg_ctx *ctx, uint64_t *out);
+
+/* The energies the sweep / exchange kernels computed for themselves (what the swap decisions of R12
+ * actually used), permuted like the configurations by the exchanges since: same layout as
+ * sg_get_energies, which always recounts with a separate kernel.  SG_ESTATE if the kernels' own
+ * values are not up to date with the current state (the last operation was a sweep without a
+ * following exchange, sg_set_spins, sg_reset). */
+int sg_get_energies_cached(sg_ctx *ctx, int64_t *U, int32_t *M);
+
+/* Parallel-tempering statistics since sg_create / sg_reset, per adjacent slot pair (t, t+1),
+ * t = 0 .. n_temps-2, summed over samples and replicas: swaps proposed and accepted (R12).
+ * HOST ptrs to n_temps-1 values each; either may be NULL.  Synchronous. */
+int sg_get_pt_stats(sg_ctx *ctx, uint64_t *proposed, uint64_t *accepted);
 
 /* Description of the last error of this context (or of the last failed sg_create if ctx is NULL).
  * The string is owned by the library and valid until the next call on the same context. */

@@ -11,32 +11,58 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libsg_b200.so")
+PROBE_SRC = os.path.join(CSRC, "probe", "alu_probe.cu")
+PROBE_LIB = os.path.join(CSRC, "probe", "libsg_probe.so")     # bench-only micro-benchmark, not the product ABI
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",
          "-Xcompiler", "-fPIC,-O2,-Wall", "-shared"]
+
+
+OBJ_DIR = os.path.join(CSRC, "build")
 
 
 def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")))
 
 
-def needs_build():
-    if not os.path.exists(LIB):
-        return True
-    t = os.path.getmtime(LIB)
-    deps = sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) + \
+def headers():
+    return glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) + \
         [os.path.join(HERE, "..", "include", "sg.h")]
-    return any(os.path.getmtime(p) > t for p in deps)
+
+
+def build_probe(force=False):
+    if force or not os.path.exists(PROBE_LIB) or os.path.getmtime(PROBE_LIB) < os.path.getmtime(PROBE_SRC):
+        tmp = PROBE_LIB + ".tmp.%d" % os.getpid()
+        subprocess.run([NVCC, *FLAGS, "-o", tmp, PROBE_SRC], check=True)
+        os.replace(tmp, PROBE_LIB)
+    return PROBE_LIB
 
 
 def build(force=False, verbose=False, extra=()):
-    if not (force or needs_build()):
+    """Compile every csrc/*.cu to an object (in parallel, only the stale ones) and link libsg_b200.so."""
+    from concurrent.futures import ThreadPoolExecutor
+    build_probe(force)
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    hdr_t = max(os.path.getmtime(p) for p in headers())
+    compile_flags = [f for f in FLAGS if f != "-shared"]
+    jobs, objs = [], []
+    for src in sources():
+        obj = os.path.join(OBJ_DIR, os.path.basename(src)[:-3] + ".o")
+        objs.append(obj)
+        if force or extra or not os.path.exists(obj) or os.path.getmtime(obj) < max(hdr_t, os.path.getmtime(src)):
+            jobs.append([NVCC, *compile_flags, *extra, "-c", "-o", obj, src])
+    if not jobs and os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(o) for o in objs):
         return LIB
+
+    def run(cmd):
+        if verbose:
+            print(" ".join(cmd))
+        subprocess.run(cmd, check=True)
+
+    with ThreadPoolExecutor(max_workers=max(1, min(len(jobs), os.cpu_count() or 1))) as ex:
+        list(ex.map(run, jobs))
     tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [NVCC, *FLAGS, *extra, "-o", tmp, *sources()]
-    if verbose:
-        print(" ".join(cmd))
-    subprocess.run(cmd, check=True)
+    run([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *objs])
     os.replace(tmp, LIB)
     return LIB
 

@@ -1,4 +1,5 @@
-// sg_probe.cu — micro-benchmark of the ALU pipe: the measured denominator of the "alu" roofline
+// alu_probe.cu — micro-benchmark of the ALU pipe: the measured denominator of the "alu" roofline.
+// NOT part of the product ABI: built into its own libsg_probe.so, loaded by bench.py only.
 // ("verify SM count, pipe width and sustained clock with a dependent-free LOP3
 // micro-benchmark; that measured number is the denominator").
 //
@@ -7,7 +8,6 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "../../include/sg.h"
 
 namespace {
 
@@ -34,15 +34,18 @@ __global__ void __launch_bounds__(1024) k_probe_lop3(uint32_t *out, uint32_t a0,
 
 }  // namespace
 
-extern "C" int sg_probe_alu_peak(void *cuda_stream, double *lane_ops_per_s)
+// Measured peak of the ALU (INT/LOP3) pipe of the current device on `cuda_stream` (NULL = default
+// stream); best of 5 launches of ~10 ms.  *lane_ops_per_s = 32-bit lane operations per second.
+// Returns 0, or -1 bad argument, -2 allocation failure, -3 CUDA error.  Synchronous.
+extern "C" int sgprobe_alu_peak(void *cuda_stream, double *lane_ops_per_s)
 {
-    if (!lane_ops_per_s) return SG_EINVAL;
+    if (!lane_ops_per_s) return -1;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return SG_ECUDA;
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return SG_ECUDA;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -3;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
     uint32_t *out = nullptr;
-    if (cudaMalloc(&out, 256) != cudaSuccess) return SG_ENOMEM;
+    if (cudaMalloc(&out, 256) != cudaSuccess) return -2;
     const int grid = 2 * sms, threads = 1024, iters = 4096, reps = 5;
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
@@ -53,7 +56,7 @@ extern "C" int sg_probe_alu_peak(void *cuda_stream, double *lane_ops_per_s)
         cudaEventRecord(e0, st);
         k_probe_lop3<<<grid, threads, 0, st>>>(out, 1u, 2u, iters);
         cudaEventRecord(e1, st);
-        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(out); return SG_ECUDA; }
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(out); return -3; }
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
         const double ops = (double)grid * threads * 64.0 * iters;
@@ -62,7 +65,7 @@ extern "C" int sg_probe_alu_peak(void *cuda_stream, double *lane_ops_per_s)
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     cudaFree(out);
-    if (cudaGetLastError() != cudaSuccess) return SG_ECUDA;
+    if (cudaGetLastError() != cudaSuccess) return -3;
     *lane_ops_per_s = best;
-    return SG_OK;
+    return 0;
 }

@@ -22,7 +22,7 @@ constexpr int DEXP64_N = 5761, DEXP32_N = 1441;
 inline size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-    size_t spins, J, Jp, tab, exp64, exp32, tw, U, M, swap, acc, hist, rec, stage, total;
+    size_t spins, spins_alt, J, Jp, tab, exp64, exp32, tw, U, M, U_alt, M_alt, swap, pt_acc, hashes, acc, hist, rec, stage, total;
     int chunk_meas, chunk_stage, S_pad;
 };
 
@@ -47,10 +47,12 @@ Layout make_layout(int L, int n_samples, int R, int NT, int kind)
     auto take = [&](size_t bytes) { size_t o = off; off += up(bytes); return o; };
     if (kind == SG_PMJ) {
         lo.spins = take((size_t)W * R * NT * N * 4);
+        lo.spins_alt = L == 32 ? take((size_t)W * R * NT * N * 4) : 0;     // k_res32_pmj reads one buffer, writes the other
         lo.J = take((size_t)W * 3 * N * 4);
         lo.Jp = L == 32 ? take(res32_packed_bytes(W)) : 0;
     } else {
         lo.Jp = 0;
+        lo.spins_alt = 0;
         lo.spins = take((size_t)n_samples * R * NT * N);
         lo.J = take((size_t)n_samples * 3 * N * 4);
     }
@@ -60,6 +62,10 @@ Layout make_layout(int L, int n_samples, int R, int NT, int kind)
     lo.tw = take(sizeof(double) * 2 * L);
     lo.U = take(sizeof(int64_t) * (size_t)lo.S_pad * R * NT);
     lo.M = take(sizeof(int32_t) * (size_t)lo.S_pad * R * NT);
+    lo.U_alt = take(sizeof(int64_t) * (size_t)lo.S_pad * R * NT);
+    lo.M_alt = take(sizeof(int32_t) * (size_t)lo.S_pad * R * NT);
+    lo.pt_acc = take(sizeof(unsigned long long) * MAX_NT);
+    lo.hashes = take(sizeof(uint64_t) * (size_t)(kind == SG_PMJ ? W : n_samples) * R * NT);
     lo.swap = take(sizeof(uint32_t) * (size_t)lo.S_pad * R * (NT / 2 + 1));
     lo.acc = take(sizeof(double) * (size_t)n_samples * NT * SG_NMOM);
     // measurement scratch, chunked over samples (multiples of 32)
@@ -163,22 +169,36 @@ int do_reset(sg_ctx *c)
     const Dims &d = c->d;
     int rc;
     if ((rc = check_cuda(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * (size_t)d.n_samples * d.NT * SG_NMOM, c->stream), "zero acc"))) return rc;
+    if ((rc = check_cuda(c, cudaMemsetAsync(c->pt_acc, 0, sizeof(unsigned long long) * MAX_NT, c->stream), "zero pt counters"))) return rc;
     c->launches += c->kind == SG_PMJ ? launch_init_pmj(c) : launch_init_gauss(c);
-    if (res32_supported(c)) c->launches += launch_pack_J_res32(c);
+    if (c->Jp) c->launches += launch_pack_J_res32(c);
     c->sweeps = c->exchanges = 0;
     c->n_meas = 0;
+    c->um_fresh = false;
+    c->pending_exchange = false;
     return check_launch(c, "init kernels");
 }
 
-int do_exchange(sg_ctx *c, bool energies_fresh = false)
+// The L = 32 resident path leaves the exchange that follows its last sweep to the NEXT launch (decision and
+// masked swap happen while that launch loads its system).  Anything else that looks at the state first
+// materialises it here: decision kernel from the kernels' own U, M, then the masked swap of spins and U, M.
+int flush_pending(sg_ctx *c)
 {
-    if (c->kind == SG_PMJ) {
-        if (!energies_fresh) c->launches += launch_energy_pmj(c);
-        c->launches += launch_pt_pmj(c, c->exchanges);
-    } else {
-        c->launches += launch_energy_gauss(c);
-        c->launches += launch_pt_gauss(c, c->exchanges);
-    }
+    if (!c->pending_exchange) return SG_OK;
+    c->pending_exchange = false;
+    c->launches += launch_pt_pmj(c, c->exchanges - 1);
+    return check_launch(c, "pending exchange");
+}
+
+// one exchange step on the current state; the swap kernels permute U, M with the configurations, so the
+// energies stay valid afterwards
+int do_exchange(sg_ctx *c)
+{
+    int rc;
+    if ((rc = flush_pending(c))) return rc;
+    if (!c->um_fresh) c->launches += c->kind == SG_PMJ ? launch_energy_pmj(c) : launch_energy_gauss(c);
+    c->um_fresh = true;
+    c->launches += c->kind == SG_PMJ ? launch_pt_pmj(c, c->exchanges) : launch_pt_gauss(c, c->exchanges);
     c->exchanges += 1;
     return check_launch(c, "pt kernels");
 }
@@ -186,6 +206,10 @@ int do_exchange(sg_ctx *c, bool energies_fresh = false)
 int do_measure(sg_ctx *c, double *out)
 {
     const Dims &d = c->d;
+    {
+        const int rc = flush_pending(c);
+        if (rc) return rc;
+    }
     for (int s0 = 0; s0 < d.n_samples; s0 += c->chunk_samples) {
         const int ns = std::min(c->chunk_samples, d.n_samples - s0);
         if (measure_fused_supported(c)) {
@@ -211,20 +235,34 @@ int do_measure(sg_ctx *c, double *out)
     return SG_OK;
 }
 
-// n consecutive sweeps with nothing in between
-// (energy_after: the caller runs an exchange next; *fresh is set if the kernel left U, M up to date)
-int do_sweeps(sg_ctx *c, int n, bool energy_after = false, bool *fresh = nullptr)
+// L = 32 resident kernel: n sweeps; applies the pending exchange on load; if `energy_after`, leaves the
+// exchange that follows these sweeps pending (its decision needs the energies this launch writes)
+int res32_step(sg_ctx *c, int n, bool energy_after)
 {
-    if (fresh) *fresh = false;
-    if (n <= 0) return SG_OK;
-    if (res32_supported(c)) {
-        const int k = launch_res32_pmj(c, c->sweeps, n, energy_after);
-        if (k < 0) return check_launch(c, "res32 kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "res32 kernel launch failed");
-        c->launches += k;
-        c->sweeps += n;
-        if (fresh) *fresh = energy_after;
-        return SG_OK;
+    const int k = launch_res32_pmj(c, c->sweeps, n, energy_after, c->pending_exchange, c->exchanges - 1);
+    if (k < 0) return check_launch(c, "res32 kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "res32 kernel launch failed");
+    c->launches += k;
+    c->sweeps += n;
+    std::swap(c->spins, c->spins_alt);
+    c->pending_exchange = false;
+    c->um_fresh = energy_after;
+    if (energy_after) {
+        std::swap(c->U, c->U_alt);
+        std::swap(c->M, c->M_alt);
+        c->pending_exchange = true;
+        c->exchanges += 1;
     }
+    return SG_OK;
+}
+
+// n consecutive sweeps with nothing in between
+int do_sweeps(sg_ctx *c, int n)
+{
+    if (n <= 0) return SG_OK;
+    int rc;
+    if (res32_supported(c)) return res32_step(c, n, false);
+    if ((rc = flush_pending(c))) return rc;
+    c->um_fresh = false;
     if (ladder8_supported(c)) {
         const int k = launch_ladder8_pmj(c, c->sweeps, c->exchanges, n, 0);
         if (k < 0) return check_launch(c, "ladder8 kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "ladder8 kernel launch failed");
@@ -252,6 +290,8 @@ int do_sweeps(sg_ctx *c, int n, bool energy_after = false, bool *fresh = nullptr
     }
     return SG_OK;
 }
+
+bool sweeps_overflow(const sg_ctx *c, int n) { return c->sweeps + (uint64_t)n >= (1ull << 31); }
 
 }  // namespace
 
@@ -289,6 +329,10 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     c->temps.assign(temps, temps + n_temps);
     c->sweeps = c->exchanges = c->launches = 0;
     c->n_meas = 0;
+    c->path = SG_PATH_AUTO;
+    c->um_fresh = false;
+    c->pending_exchange = false;
+    c->attr_done = 0;
     Dims &d = c->d;
     d.L = L; d.Lh = L / 2; d.N = L * L * L; d.H = d.N / 2;
     d.R = n_replicas; d.NT = n_temps; d.P = n_replicas * (n_replicas - 1) / 2;
@@ -312,6 +356,7 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     char *b = (char *)c->ws;
     c->spins = (uint32_t *)(b + lo.spins);
     c->spins8 = (int8_t *)(b + lo.spins);
+    c->spins_alt = (coupling_kind == SG_PMJ && L == 32) ? (uint32_t *)(b + lo.spins_alt) : nullptr;
     c->J = (uint32_t *)(b + lo.J);
     c->Jg = (float *)(b + lo.J);
     c->Jp = (coupling_kind == SG_PMJ && L == 32) ? (uint4 *)(b + lo.Jp) : nullptr;
@@ -321,7 +366,11 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     c->twiddle = (double *)(b + lo.tw);
     c->U = (int64_t *)(b + lo.U);
     c->M = (int32_t *)(b + lo.M);
+    c->U_alt = (int64_t *)(b + lo.U_alt);
+    c->M_alt = (int32_t *)(b + lo.M_alt);
     c->swapmask = (uint32_t *)(b + lo.swap);
+    c->pt_acc = (unsigned long long *)(b + lo.pt_acc);
+    c->hashes = (uint64_t *)(b + lo.hashes);
     c->acc = (double *)(b + lo.acc);
     c->hist = (uint16_t *)(b + lo.hist);
     c->rec = (double *)(b + lo.rec);
@@ -358,7 +407,9 @@ int sg_sweep(sg_ctx *c, int n)
 {
     if (!c) return SG_EINVAL;
     if (n < 0) return fail(c, SG_EINVAL, "sg_sweep: n < 0");
-    int rc = do_sweeps(c, n);
+    if (sweeps_overflow(c, n)) return fail(c, SG_EINVAL, "sg_sweep: the global sweep counter must stay below 2^31");
+    int rc = flush_pending(c);
+    if (!rc) rc = do_sweeps(c, n);
     if (rc) return rc;
     return check_launch(c, "sweep kernels");
 }
@@ -379,7 +430,8 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
 {
     if (!c) return SG_EINVAL;
     if (n_sweeps < 0 || pt_every < 0 || meas_every < 0) return fail(c, SG_EINVAL, "sg_run: negative argument");
-    int left = n_sweeps;
+    if (sweeps_overflow(c, n_sweeps)) return fail(c, SG_EINVAL, "sg_run: the global sweep counter must stay below 2^31");
+    int left = n_sweeps, rc;
     if (ladder8_supported(c) || ladder_supported(c) || gladder_supported(c)) {
         // sweeps and the exchanges between them are fused in one launch; launches end at measurements
         while (left > 0) {
@@ -392,8 +444,9 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
             c->launches += k;
             if (pt_every > 0) c->exchanges += (c->sweeps + run) / (uint64_t)pt_every - c->sweeps / (uint64_t)pt_every;
             c->sweeps += run;
+            // the kernel publishes its own energies when an exchange follows its last sweep
+            c->um_fresh = pt_every > 0 && c->sweeps % (uint64_t)pt_every == 0;
             left -= (int)run;
-            int rc;
             if (meas_every > 0 && c->sweeps % (uint64_t)meas_every == 0)
                 if ((rc = do_measure(c, nullptr))) return rc;
         }
@@ -404,16 +457,19 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
         uint64_t run = (uint64_t)left;
         if (pt_every > 0) run = std::min<uint64_t>(run, (uint64_t)pt_every - c->sweeps % (uint64_t)pt_every);
         if (meas_every > 0) run = std::min<uint64_t>(run, (uint64_t)meas_every - c->sweeps % (uint64_t)meas_every);
-        int rc;
         const bool pt_due = pt_every > 0 && (c->sweeps + run) % (uint64_t)pt_every == 0;
-        bool fresh = false;
-        if ((rc = do_sweeps(c, (int)run, pt_due, &fresh))) return rc;
+        if (res32_supported(c)) {
+            if ((rc = res32_step(c, (int)run, pt_due))) return rc;      // the exchange stays pending for the next launch
+        } else {
+            if ((rc = do_sweeps(c, (int)run))) return rc;
+            if (pt_due)
+                if ((rc = do_exchange(c))) return rc;
+        }
         left -= (int)run;
-        if (pt_due)
-            if ((rc = do_exchange(c, fresh))) return rc;
         if (meas_every > 0 && c->sweeps % (uint64_t)meas_every == 0)
             if ((rc = do_measure(c, nullptr))) return rc;
     }
+    if ((rc = flush_pending(c))) return rc;
     return check_launch(c, "run kernels");
 }
 
@@ -439,6 +495,11 @@ static int spins_range(sg_ctx *c, int s0, int ns, int8_t *out, const int8_t *in)
     const Dims &d = c->d;
     const size_t per = (size_t)d.R * d.NT * d.N;
     const Layout lo = make_layout(d.L, d.n_samples, d.R, d.NT, c->kind);
+    {
+        const int rc = flush_pending(c);
+        if (rc) return rc;
+    }
+    if (in) c->um_fresh = false;
     for (int a = s0; a < s0 + ns; a += lo.chunk_stage) {
         const int n = std::min(lo.chunk_stage, s0 + ns - a);
         int rc;
@@ -482,16 +543,75 @@ int sg_get_couplings_range(sg_ctx *c, int s0, int ns, float *out)
 
 int sg_get_couplings(sg_ctx *c, float *out) { return c ? sg_get_couplings_range(c, 0, c->d.n_samples, out) : SG_EINVAL; }
 
-int sg_get_energies(sg_ctx *c, int64_t *U, int32_t *M)
+static int copy_energies(sg_ctx *c, int64_t *U, int32_t *M)
 {
-    if (!c) return SG_EINVAL;
-    c->launches += c->kind == SG_PMJ ? launch_energy_pmj(c) : launch_energy_gauss(c);
     int rc;
-    if ((rc = check_launch(c, "energy kernel"))) return rc;
     const size_t n = (size_t)c->d.n_samples * c->d.R * c->d.NT;
     if (U && (rc = check_cuda(c, cudaMemcpyAsync(U, c->U, sizeof(int64_t) * n, cudaMemcpyDeviceToHost, c->stream), "copy U"))) return rc;
     if (M && (rc = check_cuda(c, cudaMemcpyAsync(M, c->M, sizeof(int32_t) * n, cudaMemcpyDeviceToHost, c->stream), "copy M"))) return rc;
     return check_cuda(c, cudaStreamSynchronize(c->stream), "sync energies");
+}
+
+int sg_get_energies(sg_ctx *c, int64_t *U, int32_t *M)
+{
+    if (!c) return SG_EINVAL;
+    int rc;
+    if ((rc = flush_pending(c))) return rc;
+    c->launches += c->kind == SG_PMJ ? launch_energy_pmj(c) : launch_energy_gauss(c);     // always a recount
+    if ((rc = check_launch(c, "energy kernel"))) return rc;
+    c->um_fresh = true;
+    return copy_energies(c, U, M);
+}
+
+int sg_get_energies_cached(sg_ctx *c, int64_t *U, int32_t *M)
+{
+    if (!c) return SG_EINVAL;
+    if (!c->um_fresh) return fail(c, SG_ESTATE, "sg_get_energies_cached: the kernels' own energies are not up to date with the state");
+    int rc;
+    if ((rc = flush_pending(c))) return rc;
+    return copy_energies(c, U, M);
+}
+
+int sg_set_kernel_path(sg_ctx *c, int path)
+{
+    if (!c) return SG_EINVAL;
+    if (path != SG_PATH_AUTO && path != SG_PATH_GENERIC) return fail(c, SG_EINVAL, "sg_set_kernel_path: unknown path");
+    const int rc = flush_pending(c);
+    if (rc) return rc;
+    c->path = path;
+    return SG_OK;
+}
+
+int sg_get_state_hash(sg_ctx *c, uint64_t *out)
+{
+    if (!c || !out) return SG_EINVAL;
+    int rc;
+    if ((rc = flush_pending(c))) return rc;
+    c->launches += launch_hash(c, c->hashes);
+    if ((rc = check_launch(c, "hash kernel"))) return rc;
+    const size_t n = (size_t)c->d.W * c->d.R * c->d.NT;
+    if ((rc = check_cuda(c, cudaMemcpyAsync(out, c->hashes, sizeof(uint64_t) * n, cudaMemcpyDeviceToHost, c->stream), "copy hashes"))) return rc;
+    return check_cuda(c, cudaStreamSynchronize(c->stream), "sync hashes");
+}
+
+int sg_get_pt_stats(sg_ctx *c, uint64_t *proposed, uint64_t *accepted)
+{
+    if (!c) return SG_EINVAL;
+    const int NT = c->d.NT;
+    int rc;
+    if ((rc = flush_pending(c))) return rc;
+    if (accepted && NT > 1) {
+        unsigned long long tmp[MAX_NT];
+        if ((rc = check_cuda(c, cudaMemcpyAsync(tmp, c->pt_acc, sizeof(unsigned long long) * MAX_NT, cudaMemcpyDeviceToHost, c->stream), "copy pt counters"))) return rc;
+        if ((rc = check_cuda(c, cudaStreamSynchronize(c->stream), "sync pt counters"))) return rc;
+        for (int t = 0; t + 1 < NT; ++t) accepted[t] = tmp[t];
+    }
+    if (proposed) {
+        // exchange e proposes the pairs (t, t+1) with t = e mod 2 (R12), once per (sample, replica)
+        const uint64_t even = (c->exchanges + 1) / 2, odd = c->exchanges / 2;
+        for (int t = 0; t + 1 < NT; ++t) proposed[t] = ((t & 1) ? odd : even) * (uint64_t)c->d.n_samples * (uint64_t)c->d.R;
+    }
+    return SG_OK;
 }
 
 int sg_get_thresholds(sg_ctx *c, uint64_t *out)

@@ -177,7 +177,8 @@ k_energy_gauss(Dims d, const int8_t *__restrict__ spins, const float *__restrict
 __global__ void __launch_bounds__(128)
 k_pt_decide_gauss(Dims d, const int64_t *__restrict__ U, const int32_t *__restrict__ M,
                   const SlotTab *__restrict__ tab, const double *__restrict__ exp_tab, double h,
-                  uint32_t exchange, int npairs, uint32_t *__restrict__ swapmask)
+                  uint32_t exchange, int npairs, uint32_t *__restrict__ swapmask,
+                  unsigned long long *__restrict__ pt_acc)
 {
     const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= (long long)d.n_samples * d.R * npairs) return;
@@ -190,26 +191,30 @@ k_pt_decide_gauss(Dims d, const int64_t *__restrict__ U, const int32_t *__restri
     const uint4 r = philox4x32_10(0u, exchange, (uint32_t)(s + d.s_first), ctr3(4, a, t), d.k0, d.k1);
     const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(exp_tab, -x));
     swapmask[((size_t)s * d.R + a) * (d.NT / 2) + pair] = accept ? 1u : 0u;
+    if (accept) atomicAdd(&pt_acc[t], 1ULL);
 }
 
+// One CTA per (pair, replica, sample): leaves at once if the pair does not swap; otherwise trades the two
+// configurations and their E_fix, M.
 __global__ void __launch_bounds__(256)
 k_pt_swap_gauss(Dims d, int8_t *__restrict__ spins, const uint32_t *__restrict__ swapmask,
-                uint32_t exchange, int npairs)
+                uint32_t exchange, int npairs, int64_t *__restrict__ U, int32_t *__restrict__ M)
 {
-    const int NQ = d.N >> 2;                   // 4-byte chunks per system (N is a multiple of 8)
-    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (tid >= (long long)d.n_samples * d.R * npairs * NQ) return;
-    const int j = (int)(tid % NQ);
-    const long long g = tid / NQ;
-    const int pair = (int)(g % npairs), a = (int)((g / npairs) % d.R), s = (int)(g / (npairs * d.R));
+    const int pair = blockIdx.x, a = blockIdx.y, s = blockIdx.z;
     if (!swapmask[((size_t)s * d.R + a) * (d.NT / 2) + pair]) return;
     const int t = (int)(exchange & 1u) + 2 * pair;
     const size_t sys = ((size_t)s * d.R + a) * d.NT + t;
-    uint32_t *A = reinterpret_cast<uint32_t *>(spins + sys * d.N) + j;
-    uint32_t *B = reinterpret_cast<uint32_t *>(spins + (sys + 1) * d.N) + j;
-    const uint32_t x = *A, y = *B;
-    *A = y;
-    *B = x;
+    uint32_t *A = reinterpret_cast<uint32_t *>(spins + sys * d.N);
+    uint32_t *B = reinterpret_cast<uint32_t *>(spins + (sys + 1) * d.N);
+    for (int j = threadIdx.x; j < (d.N >> 2); j += blockDim.x) {      // N is a multiple of 8
+        const uint32_t x = A[j], y = B[j];
+        A[j] = y;
+        B[j] = x;
+    }
+    if (threadIdx.x == 0) {
+        const int64_t u = U[sys]; U[sys] = U[sys + 1]; U[sys + 1] = u;
+        const int32_t m = M[sys]; M[sys] = M[sys + 1]; M[sys + 1] = m;
+    }
 }
 
 // ------------------------------------------------------------------------------- measurement
@@ -339,9 +344,9 @@ int launch_pt_gauss(sg_ctx *c, uint64_t exchange)
     const int npairs = (d.NT - (int)(exchange & 1)) / 2;
     if (npairs <= 0) return 0;
     k_pt_decide_gauss<<<blocks_for((long long)d.n_samples * d.R * npairs, 128), 128, 0, c->stream>>>(
-        d, c->U, c->M, c->tab, c->exp64_tab, c->h, (uint32_t)exchange, npairs, c->swapmask);
-    k_pt_swap_gauss<<<blocks_for((long long)d.n_samples * d.R * npairs * (d.N >> 2), 256), 256, 0, c->stream>>>(
-        d, c->spins8, c->swapmask, (uint32_t)exchange, npairs);
+        d, c->U, c->M, c->tab, c->exp64_tab, c->h, (uint32_t)exchange, npairs, c->swapmask, c->pt_acc);
+    k_pt_swap_gauss<<<dim3(npairs, d.R, d.n_samples), 256, 0, c->stream>>>(d, c->spins8, c->swapmask, (uint32_t)exchange,
+                                                                           npairs, c->U, c->M);
     return 2;
 }
 

@@ -32,6 +32,9 @@ struct GLadderArgs {
     int G;
     int pt_every;
     uint64_t exchange0;
+    int64_t *U;               // [S][R][NT]: the kernel's own E_fix, M after the last exchange of the launch (post-swap)
+    int32_t *M;
+    unsigned long long *pt_acc;   // [NT] accepted swaps per lower slot of the pair
 };
 
 namespace {
@@ -58,6 +61,7 @@ __global__ void __launch_bounds__(512, 1) k_gladder(const __grid_constant__ GLad
     long long *Efix = reinterpret_cast<long long *>(betaf + ((NT + 3) & ~3)); // [NT]
     int *Msum = reinterpret_cast<int *>(Efix + NT);                           // [NT]
     int *flags = Msum + NT;                                                   // [NT / 2 + 1]
+    int *accs = flags + (NT / 2 + 1);                                         // [NT]
 
     const int s = blockIdx.x / d.R, a = blockIdx.x % d.R;
     const int tid = threadIdx.x, nthr = blockDim.x;
@@ -72,7 +76,7 @@ __global__ void __launch_bounds__(512, 1) k_gladder(const __grid_constant__ GLad
         uint4 *jd = reinterpret_cast<uint4 *>(Jsm);
         for (int i = tid; i < 3 * N / 4; i += nthr) jd[i] = js[i];
         for (int i = tid; i < EXP32_N; i += nthr) etab[i] = A.exp32_tab[i];
-        for (int i = tid; i < NT; i += nthr) betaf[i] = A.tab[i].beta_f;
+        for (int i = tid; i < NT; i += nthr) { betaf[i] = A.tab[i].beta_f; accs[i] = 0; }
     }
     __syncthreads();
 
@@ -224,9 +228,19 @@ __global__ void __launch_bounds__(512, 1) k_gladder(const __grid_constant__ GLad
                 const double Eu = __dsub_rn(__dmul_rn((double)Efix[t + 1], 0x1p-32), __dmul_rn(A.h, (double)Msum[t + 1]));
                 const double x = __dmul_rn(__dsub_rn(A.tab[t].beta, A.tab[t + 1].beta), __dsub_rn(Et, Eu));
                 const uint4 r = philox_rk8(0u, (uint32_t)exchange, sglob, ctr3(4, a, t), A.rk);
-                flags[tid] = ((x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp64_tab, -x))) ? 1 : 0;
+                const int acc = ((x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp64_tab, -x))) ? 1 : 0;
+                flags[tid] = acc;
+                accs[t] += acc;
             }
             __syncthreads();
+            if (sw == A.n_sweeps - 1 && tid < NT) {           // publish the energies, permuted like the configurations
+                const int p = tid - e1;
+                int src = tid;
+                if (p >= 0 && (p >> 1) < npairs && flags[p >> 1]) src = (p & 1) ? tid - 1 : tid + 1;
+                const size_t o = ((size_t)s * d.R + a) * NT + tid;
+                A.U[o] = (int64_t)Efix[src];
+                A.M[o] = Msum[src];
+            }
             for (int item = tid; item < npairs * (N / 16); item += nthr) {
                 const int pair = item / (N / 16), k = item - pair * (N / 16);
                 if (!flags[pair]) continue;
@@ -242,6 +256,7 @@ __global__ void __launch_bounds__(512, 1) k_gladder(const __grid_constant__ GLad
         }
     }
 
+    if (tid < NT && accs[tid]) atomicAdd(&A.pt_acc[tid], (unsigned long long)accs[tid]);
     {
         uint4 *dst = reinterpret_cast<uint4 *>(gS);
         const uint4 *src = reinterpret_cast<const uint4 *>(S);
@@ -253,17 +268,15 @@ size_t gladder_smem(int L, int NT)
 {
     const size_t N = (size_t)L * L * L;
     return (size_t)NT * N + 3 * N * 4 + EXP32_PAD * 4 + (size_t)((NT + 3) & ~3) * 4 + (size_t)NT * 8 + (size_t)NT * 4 +
-           (size_t)(NT / 2 + 1) * 4 + 16;
+           (size_t)(NT / 2 + 1) * 4 + (size_t)NT * 4 + 16;
 }
 
 template <int L>
-cudaError_t launch_g(const GLadderArgs &A, int threads, size_t smem, cudaStream_t st, int grid)
+cudaError_t launch_g(sg_ctx *c, const GLadderArgs &A, int threads, size_t smem, cudaStream_t st, int grid)
 {
-    static bool configured = false;
-    if (!configured) {
+    if (attr_needed(c, ATTR_GLADDER + (L == 16))) {
         cudaError_t e = cudaFuncSetAttribute(k_gladder<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
-        configured = true;
     }
     k_gladder<L><<<grid, threads, smem, st>>>(A);
     return cudaGetLastError();
@@ -274,7 +287,7 @@ cudaError_t launch_g(const GLadderArgs &A, int threads, size_t smem, cudaStream_
 bool gladder_supported(const sg_ctx *c)
 {
     const Dims &d = c->d;
-    if (c->kind != SG_GAUSS) return false;
+    if (c->path != SG_PATH_AUTO || c->kind != SG_GAUSS) return false;
     if (d.L != 8 && d.L != 16) return false;
     return (size_t)d.NT * d.N % 16 == 0 && gladder_smem(d.L, d.NT) <= (size_t)227 * 1024;
 }
@@ -301,6 +314,9 @@ int launch_gladder(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0,
     A.n_sweeps = n_sweeps;
     A.pt_every = pt_every;
     A.exchange0 = exchange0;
+    A.U = c->U;
+    A.M = c->M;
+    A.pt_acc = c->pt_acc;
     const int Q = d.N / 8;
     int G = std::max(1, std::min(d.NT, 512 / Q));
     for (int gtry = G; gtry >= 1 && gtry * 2 > G; --gtry)
@@ -310,7 +326,7 @@ int launch_gladder(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0,
     if (threads > 512) return -1;
     const size_t smem = gladder_smem(d.L, d.NT);
     const int grid = d.n_samples * d.R;
-    const cudaError_t e = d.L == 8 ? launch_g<8>(A, threads, smem, c->stream, grid) : launch_g<16>(A, threads, smem, c->stream, grid);
+    const cudaError_t e = d.L == 8 ? launch_g<8>(c, A, threads, smem, c->stream, grid) : launch_g<16>(c, A, threads, smem, c->stream, grid);
     return e == cudaSuccess ? 1 : -1;
 }
 

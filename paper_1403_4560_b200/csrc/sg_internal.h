@@ -49,11 +49,17 @@ struct sg_ctx {
     std::string err;
     uint64_t sweeps, exchanges, launches;
     int64_t n_meas;
+    int path;                           // SG_PATH_AUTO / SG_PATH_GENERIC (sg_set_kernel_path)
+    bool um_fresh;                      // U, M below are the kernels' own energies of the CURRENT state
+    bool pending_exchange;              // L = 32 resident path: exchange `exchanges - 1` is decided and applied by the
+                                        // next k_res32_pmj launch on load (or by flush_pending), from U, M below
+    uint32_t attr_done;                 // bit k: cudaFuncSetAttribute done for kernel family k on this context's device
     // device memory
     void *ws;                           // base of the workspace
     size_t ws_bytes;
     bool own_ws;
-    uint32_t *spins;                    // PMJ: [W][R][NT][2][H] colour-compacted words
+    uint32_t *spins;                    // PMJ: [W][R][NT][2][H] colour-compacted words (the CURRENT state)
+    uint32_t *spins_alt;                // PMJ, L = 32: second state buffer; k_res32_pmj reads `spins`, writes `spins_alt`, then they swap
     uint32_t *J;                        // PMJ: [W][2][3][H]
     uint4 *Jp;                          // PMJ, L = 32: couplings repacked per warp step for k_res32_pmj (else NULL)
     int8_t *spins8;                     // GAUSS: [S][R][NT][2][H] colour-compacted bytes
@@ -64,7 +70,11 @@ struct sg_ctx {
     double *twiddle;                    // [2][L] cos, sin (2 pi m / L)
     int64_t *U;                         // [S_pad][R][NT]  (S_pad = 32 W for PMJ)
     int32_t *M;                         // [S_pad][R][NT]
+    int64_t *U_alt;                     // L = 32: ping-pong partners of U, M (same reason as spins_alt)
+    int32_t *M_alt;
     uint32_t *swapmask;                 // PMJ: [W][R][NT/2]; GAUSS: [S][R][NT/2] (0/1)
+    uint64_t *hashes;                   // [W][R][NT] scratch of sg_get_state_hash
+    unsigned long long *pt_acc;         // [MAX_NT] accepted swaps per lower slot t of the pair (t, t+1), all samples and replicas
     double *acc;                        // [n_samples][NT][SG_NMOM]
     uint16_t *hist;                     // scratch [chunk samples][NT][P][N_HIST][L]
     double *rec;                        // scratch [chunk samples][NT][P][SG_REC]
@@ -88,10 +98,12 @@ int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_swe
 bool res32_supported(const sg_ctx *c);                     // L = 32: one system resident per SM, couplings streamed from L2
 size_t res32_packed_bytes(int W);
 int launch_pack_J_res32(sg_ctx *c);                        // J -> Jp
-int launch_res32_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, bool want_energy);   // 1 launch (-1 on error)
+// 1 launch (-1 on error): reads c->spins (+ c->U, c->M if do_exchange: decides exchange `exchange` and applies it while
+// loading), writes c->spins_alt (+ c->U_alt, c->M_alt if want_energy); the caller swaps the pointers
+int launch_res32_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, bool want_energy, bool do_exchange, uint64_t exchange);
 int launch_energy_pmj(sg_ctx *c);
 int launch_energy_gauss(sg_ctx *c);
-int launch_pt_pmj(sg_ctx *c, uint64_t exchange);            // decide + swap (energies must be fresh)
+int launch_pt_pmj(sg_ctx *c, uint64_t exchange);            // decide + swap of spins and of U, M (energies must be fresh)
 int launch_pt_gauss(sg_ctx *c, uint64_t exchange);
 int launch_hist_pmj(sg_ctx *c, int s0, int ns);             // samples [s0, s0+ns) -> c->hist
 int launch_hist_gauss(sg_ctx *c, int s0, int ns);
@@ -104,5 +116,16 @@ int launch_unpack_gauss(sg_ctx *c, int s0, int ns);
 int launch_pack_gauss(sg_ctx *c, int s0, int ns);
 int launch_couplings_pmj(sg_ctx *c, int s0, int ns, float *dev_out);   // -> [ns][3][N] float
 int launch_couplings_gauss(sg_ctx *c, int s0, int ns, float *dev_out);
+int launch_hash(sg_ctx *c, uint64_t *dev_out);             // one 64-bit hash per system -> dev_out
+
+// kernel families for sg_ctx::attr_done
+enum { ATTR_LADDER8 = 0, ATTR_LADDER = 1, ATTR_GLADDER = 8, ATTR_RES32 = 10, ATTR_MEASURE = 11, ATTR_MEASURE32 = 18, ATTR_GMEASURE = 19, ATTR_TPACK = 24 };
+// true if the attribute still has to be set for family `id` on this context (and marks it done)
+inline bool attr_needed(sg_ctx *c, int id)
+{
+    if (c->attr_done & (1u << id)) return false;
+    c->attr_done |= 1u << id;
+    return true;
+}
 
 }  // namespace sg

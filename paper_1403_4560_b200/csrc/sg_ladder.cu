@@ -30,6 +30,9 @@ struct LadderArgs {
     const double *exp_tab;    // dexp64 table (R12)
     double h;
     uint32_t one, mone;       // run-time 1 and 0xFFFFFFFF (sg_accept.cuh)
+    int64_t *U;               // the kernel's own energies after the last exchange of the launch (see sg_ladder8.cu)
+    int32_t *M;
+    unsigned long long *pt_acc;
 };
 
 __device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -156,7 +159,8 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     uint2 *thr = reinterpret_cast<uint2 *>(Jsm + 3 * N);  // [NT][8]
     int *Uint = reinterpret_cast<int *>(thr + NT * 8);    // [NT][32]   exchange scratch (pt_every > 0 only)
     int *Mint = Uint + NT * 32;                           // [NT][32]
-    uint32_t *masks = reinterpret_cast<uint32_t *>(Mint + NT * 32);   // [NT / 2]
+    uint32_t *masks = reinterpret_cast<uint32_t *>(Mint + NT * 32);   // [NT / 2 + 1]
+    uint32_t *accs = masks + (NT / 2 + 1);                // [NT] accepted swaps of this CTA per lower slot
 
     const int w = blockIdx.x / d.R, a = blockIdx.x % d.R;
     const int tid = threadIdx.x, nthr = blockDim.x;
@@ -183,6 +187,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
             k4[1] = make_uint4(lo[4], lo[5], lo[6], zc[3] - 1u);
             k4[2] = make_uint4(zc[1] + zc[5] - 1u, zc[0] + zc[2] + zc[4] + zc[6] - 2u, 0u, 0u);
         }
+        for (int t = tid; t < NT; t += nthr) accs[t] = 0u;
     }
     __syncthreads();
 
@@ -372,9 +377,20 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                 const uint4 r = philox_rk(0u, (uint32_t)exchange, (uint32_t)(smp + d.s_first), ctr3(4, a, t), A.rk);
                 const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
                 const uint32_t mask = __ballot_sync(0xffffffffu, accept && smp < d.n_samples);
-                if (ln == 0) masks[pair] = mask;
+                if (ln == 0) { masks[pair] = mask; accs[t] += (uint32_t)__popc(mask); }
             }
             __syncthreads();
+            if (sw == A.n_sweeps - 1) {
+                for (int item = tid; item < NT * 32; item += nthr) {       // publish the energies, permuted like the configurations
+                    const int t = item >> 5, ln = item & 31;
+                    const int p = t - e1;
+                    int src = t;
+                    if (p >= 0 && (p >> 1) < npairs && ((masks[p >> 1] >> ln) & 1u)) src = (p & 1) ? t - 1 : t + 1;
+                    const size_t o = ((size_t)(w * 32 + ln) * d.R + a) * NT + t;
+                    A.U[o] = (int64_t)Uint[src * 32 + ln];
+                    A.M[o] = Mint[src * 32 + ln];
+                }
+            }
             for (int item = tid; item < npairs * (N / 4); item += nthr) {  // masked swap of the two configurations
                 const int pair = item / (N / 4), k = item - pair * (N / 4);
                 const uint32_t mask = masks[pair];
@@ -397,6 +413,8 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     }
 
     // ---- write the ladder back
+    for (int t = tid; t < NT; t += nthr)
+        if (accs[t]) atomicAdd(&A.pt_acc[t], (unsigned long long)accs[t]);
     {
         uint4 *dst = reinterpret_cast<uint4 *>(gS);
         const uint4 *src = reinterpret_cast<const uint4 *>(S);
@@ -408,25 +426,23 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
 size_t ladder_smem_bytes(int L, int NT)
 {
     const size_t N = (size_t)L * L * L;
-    return (size_t)NT * N * 4 + 3 * N * 4 + (size_t)NT * 8 * sizeof(uint2) + (size_t)NT * 32 * 8 + (size_t)(NT / 2 + 1) * 4;
+    return (size_t)NT * N * 4 + 3 * N * 4 + (size_t)NT * 8 * sizeof(uint2) + (size_t)NT * 32 * 8 + (size_t)(NT / 2 + 1) * 4 + (size_t)NT * 4;
 }
 
 bool ladder_supported(const sg_ctx *c)
 {
     const Dims &d = c->d;
-    if (c->kind != SG_PMJ || !d.fast_accept) return false;
+    if (c->path != SG_PATH_AUTO || c->kind != SG_PMJ || !d.fast_accept) return false;
     if (d.L != 4 && d.L != 6 && d.L != 8 && d.L != 10 && d.L != 12 && d.L != 16) return false;
     return ladder_smem_bytes(d.L, d.NT) <= (size_t)227 * 1024;
 }
 
 template <int L>
-static cudaError_t launch_l(const LadderArgs &A, int threads, size_t smem, cudaStream_t st, int grid)
+static cudaError_t launch_l(sg_ctx *c, const LadderArgs &A, int threads, size_t smem, cudaStream_t st, int grid)
 {
-    static bool configured = false;
-    if (!configured) {
+    if (attr_needed(c, ATTR_LADDER + L / 2 - 2)) {       // L = 4..16 -> ids 1..7
         cudaError_t e = cudaFuncSetAttribute(k_ladder_pmj<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
-        configured = true;
     }
     k_ladder_pmj<L><<<grid, threads, smem, st>>>(A);
     return cudaGetLastError();
@@ -455,6 +471,9 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchang
     A.h = c->h;
     A.one = 1u;
     A.mone = 0xffffffffu;
+    A.U = c->U;
+    A.M = c->M;
+    A.pt_acc = c->pt_acc;
     const int Q = d.N / 8;
     // groups: as many as fit in <= 512 threads, at most NT, preferring a divisor of NT
     const int maxt = d.L == 8 ? 320 : 512;
@@ -468,12 +487,12 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchang
     const int grid = d.W * d.R;
     cudaError_t e;
     switch (d.L) {
-    case 4: e = launch_l<4>(A, threads, smem, c->stream, grid); break;
-    case 6: e = launch_l<6>(A, threads, smem, c->stream, grid); break;
-    case 8: e = launch_l<8>(A, threads, smem, c->stream, grid); break;
-    case 10: e = launch_l<10>(A, threads, smem, c->stream, grid); break;
-    case 12: e = launch_l<12>(A, threads, smem, c->stream, grid); break;
-    case 16: e = launch_l<16>(A, threads, smem, c->stream, grid); break;
+    case 4: e = launch_l<4>(c, A, threads, smem, c->stream, grid); break;
+    case 6: e = launch_l<6>(c, A, threads, smem, c->stream, grid); break;
+    case 8: e = launch_l<8>(c, A, threads, smem, c->stream, grid); break;
+    case 10: e = launch_l<10>(c, A, threads, smem, c->stream, grid); break;
+    case 12: e = launch_l<12>(c, A, threads, smem, c->stream, grid); break;
+    case 16: e = launch_l<16>(c, A, threads, smem, c->stream, grid); break;
     default: return -1;
     }
     return e == cudaSuccess ? 1 : -1;

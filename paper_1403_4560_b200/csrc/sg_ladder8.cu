@@ -34,6 +34,9 @@ struct Ladder8Args {
     int pt_every;             // 0 = never
     int G;
     uint32_t one, mone;       // 1 and 0xFFFFFFFF as run-time values: mad.lo with them stays an IMAD (FMA pipe)
+    int64_t *U;               // [32 W][R][NT]: the kernel's own per-lane energies after the LAST exchange of the launch
+    int32_t *M;               //                (post-swap), written only if that exchange follows the last sweep
+    unsigned long long *pt_acc;   // [NT] accepted swaps per lower slot of the pair
 };
 
 __device__ __forceinline__ int slot_of_row(int y, int z) { return ((y + z) & 1) * 32 + z * 4 + (y >> 1); }
@@ -159,8 +162,9 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
     uint32_t *Jsm = S + NT * N;                            // [2][3][64 slots][4]
     uint4 *thr = reinterpret_cast<uint4 *>(Jsm + 3 * N);   // [NT][3] = SlotK: lo[7], b3c, nc, ec, 0, 0
     uint32_t *masks = reinterpret_cast<uint32_t *>(thr + NT * 3);     // [32]
+    uint32_t *accs = masks + 32;                           // [MAX_NT] accepted swaps of this CTA per lower slot
     // exchange scratch (allocated only when pt_every > 0); later stages alias dead earlier ones
-    uint32_t *red0 = masks + 32;                           // [NT][9][64]   stage-1 planes
+    uint32_t *red0 = accs + MAX_NT;                        // [NT][9][64]   stage-1 planes
     uint32_t *red1 = red0 + NT * PW1 * 64;                 // [NT][13][16]
     uint32_t *red2 = red0;                                 // [NT][17][4]   (red0 is dead after stage 2)
     uint32_t *red3 = red1;                                 // [NT][21][1]   (red1 is dead after stage 3)
@@ -192,6 +196,7 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
         thr[t * 3 + 1] = make_uint4(lo[4], lo[5], lo[6], zc[3] - 1u);
         thr[t * 3 + 2] = make_uint4(zc[1] + zc[5] - 1u, zc[0] + zc[2] + zc[4] + zc[6] - 2u, 0u, 0u);
     }
+    if (tid < MAX_NT) accs[tid] = 0u;
     __syncthreads();
 
     // ---- thread geometry (colour independent)
@@ -303,9 +308,21 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
                 const uint4 r = philox_rk8(0u, (uint32_t)exchange, (uint32_t)(s + d.s_first), ctr3(4, a, t), A.rk);
                 const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
                 const uint32_t mask = __ballot_sync(0xffffffffu, accept && s < d.n_samples);
-                if (lane == 0) masks[pair] = mask;
+                if (lane == 0) { masks[pair] = mask; accs[t] += (uint32_t)__popc(mask); }
             }
             __syncthreads();
+            if (sw == A.n_sweeps - 1) {
+                // the launch ends here: publish the energies the decisions used, permuted like the configurations
+                for (int item = tid; item < NT * 32; item += nthr) {
+                    const int t = item >> 5, lane = item & 31;
+                    const int p = t - e1;
+                    int src = t;
+                    if (p >= 0 && (p >> 1) < npairs && ((masks[p >> 1] >> lane) & 1u)) src = (p & 1) ? t - 1 : t + 1;
+                    const size_t o = ((size_t)(w * 32 + lane) * d.R + a) * NT + t;
+                    A.U[o] = (int64_t)Uint[src * 32 + lane];
+                    A.M[o] = Mint[src * 32 + lane];
+                }
+            }
             // ---- masked swap of the two configurations (layout independent: same slot in both systems)
             for (int item = tid; item < npairs * 128; item += nthr) {
                 const int pair = item >> 7, k = item & 127;
@@ -328,6 +345,7 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
         }
     }
     __syncthreads();
+    if (tid < NT && accs[tid]) atomicAdd(&A.pt_acc[tid], (unsigned long long)accs[tid]);
 
     // ---- write back (slot order -> global compact order)
     for (int i = tid; i < NT * 128; i += nthr) {
@@ -339,7 +357,7 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
 // ------------------------------------------------------------------------------- host side
 static size_t ladder8_smem(int NT, bool with_pt)
 {
-    size_t b = (size_t)NT * 512 * 4 + 3 * 512 * 4 + (size_t)NT * 3 * sizeof(uint4) + 32 * 4;
+    size_t b = (size_t)NT * 512 * 4 + 3 * 512 * 4 + (size_t)NT * 3 * sizeof(uint4) + 32 * 4 + MAX_NT * 4;
     if (with_pt) b += (size_t)NT * 4 * (PW1 * 64 + 13 * 16);
     return b;
 }
@@ -347,21 +365,20 @@ static size_t ladder8_smem(int NT, bool with_pt)
 bool ladder8_supported(const sg_ctx *c)
 {
     const Dims &d = c->d;
-    return c->kind == SG_PMJ && d.fast_accept && d.L == 8 && ladder8_smem(d.NT, true) <= (size_t)113 * 1024;
+    return c->path == SG_PATH_AUTO && c->kind == SG_PMJ && d.fast_accept && d.L == 8 &&
+           ladder8_smem(d.NT, true) <= (size_t)113 * 1024;
 }
 
 // n_sweeps sweeps (global indices sweep0...) with the exchanges that fall due (pt_every; 0 = none).
 // Returns kernels launched (1) or -1.  The caller advances its sweep / exchange counters.
 int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_sweeps, int pt_every)
 {
-    static bool configured = false;
-    if (!configured) {
+    if (attr_needed(c, ATTR_LADDER8)) {
         if (cudaFuncSetAttribute(k_ladder8_pmj<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess ||
             cudaFuncSetAttribute(k_ladder8_pmj<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess ||
             cudaFuncSetAttribute(k_ladder8_pmj<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess ||
             cudaFuncSetAttribute(k_ladder8_pmj<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess)
             return -1;
-        configured = true;
     }
     const Dims &d = c->d;
     Ladder8Args A;
@@ -387,6 +404,9 @@ int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_swe
     const int threads = 64 * G;
     A.one = 1u;
     A.mone = 0xffffffffu;
+    A.U = c->U;
+    A.M = c->M;
+    A.pt_acc = c->pt_acc;
     const size_t smem = ladder8_smem(d.NT, pt_every > 0);
     const int spt = d.NT % G == 0 ? d.NT / G : 0;
     if (spt == 4) k_ladder8_pmj<4><<<d.W * d.R, threads, smem, c->stream>>>(A);

@@ -393,11 +393,9 @@ static int launch_measure_L(sg_ctx *c, int s0, int ns, bool want_rec)
 {
     const Dims &d = c->d;
     const size_t smem = measure_smem<L>(d.P);
-    static bool configured = false;
-    if (!configured) {
+    if (attr_needed(c, ATTR_MEASURE + L / 2 - 2)) {      // L = 4..16 -> ids 11..17
         if (cudaFuncSetAttribute(k_measure_pmj<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)measure_smem<L>(6)) != cudaSuccess)
             return -1;
-        configured = true;
     }
     const int w0 = s0 >> 5, nw = (ns + 31) >> 5;
     k_measure_pmj<L><<<(unsigned)(nw * d.NT), 256, smem, c->stream>>>(d, c->spins, c->twiddle, w0, s0,
@@ -408,7 +406,7 @@ static int launch_measure_L(sg_ctx *c, int s0, int ns, bool want_rec)
 bool measure_fused_supported(const sg_ctx *c)
 {
     const int L = c->d.L;
-    return c->kind == SG_PMJ && (L == 4 || L == 6 || L == 8 || L == 10 || L == 12 || L == 16);
+    return c->path == SG_PATH_AUTO && c->kind == SG_PMJ && (L == 4 || L == 6 || L == 8 || L == 10 || L == 12 || L == 16);
 }
 
 // samples [s0, s0+ns), s0 a multiple of 32: records (optional) and accumulators in one launch

@@ -242,7 +242,8 @@ k_energy_pmj(Dims d, const uint32_t *__restrict__ spins, const uint32_t *__restr
 __global__ void __launch_bounds__(128)
 k_pt_decide_pmj(Dims d, const int64_t *__restrict__ U, const int32_t *__restrict__ M,
                 const SlotTab *__restrict__ tab, const double *__restrict__ exp_tab, double h,
-                uint32_t exchange, int npairs, uint32_t *__restrict__ swapmask)
+                uint32_t exchange, int npairs, uint32_t *__restrict__ swapmask,
+                unsigned long long *__restrict__ pt_acc)
 {
     const int lane = threadIdx.x & 31;
     const int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -257,33 +258,63 @@ k_pt_decide_pmj(Dims d, const int64_t *__restrict__ U, const int32_t *__restrict
     const uint4 r = philox4x32_10(0u, exchange, (uint32_t)(s + d.s_first), ctr3(4, a, t), d.k0, d.k1);
     const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(exp_tab, -x));
     const uint32_t mask = __ballot_sync(0xffffffffu, accept && s < d.n_samples);
-    if (lane == 0) swapmask[(size_t)(w * d.R + a) * (d.NT / 2) + pair] = mask;
+    if (lane == 0) {
+        swapmask[(size_t)(w * d.R + a) * (d.NT / 2) + pair] = mask;
+        if (mask) atomicAdd(&pt_acc[t], (unsigned long long)__popc(mask));
+    }
 }
 
+// One CTA per (pair, replica, word): reads the pair's mask once and leaves if no lane swaps (the common
+// case on a wide ladder); otherwise trades the selected lanes of the two configurations and of their U, M.
 __global__ void __launch_bounds__(256)
 k_pt_swap_pmj(Dims d, uint32_t *__restrict__ spins, const uint32_t *__restrict__ swapmask,
-              uint32_t exchange, int npairs)
+              uint32_t exchange, int npairs, int64_t *__restrict__ U, int32_t *__restrict__ M)
 {
-    const int NQ = d.N >> 2;
-    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (tid >= (long long)d.W * d.R * npairs * NQ) return;
-    const int j = (int)(tid % NQ);
-    const int g = (int)(tid / NQ);
-    const int pair = g % npairs, a = (g / npairs) % d.R, w = g / (npairs * d.R);
+    const int pair = blockIdx.x, a = blockIdx.y, w = blockIdx.z;
     const uint32_t mask = swapmask[(size_t)(w * d.R + a) * (d.NT / 2) + pair];
     if (mask == 0) return;
     const int t = (int)(exchange & 1u) + 2 * pair;
     const size_t sys = ((size_t)w * d.R + a) * d.NT + t;
-    uint4 *A = reinterpret_cast<uint4 *>(spins + sys * d.N) + j;
-    uint4 *B = reinterpret_cast<uint4 *>(spins + (sys + 1) * d.N) + j;
-    uint4 x = *A, y = *B;
-    uint32_t dd;
-    dd = (x.x ^ y.x) & mask; x.x ^= dd; y.x ^= dd;
-    dd = (x.y ^ y.y) & mask; x.y ^= dd; y.y ^= dd;
-    dd = (x.z ^ y.z) & mask; x.z ^= dd; y.z ^= dd;
-    dd = (x.w ^ y.w) & mask; x.w ^= dd; y.w ^= dd;
-    *A = x;
-    *B = y;
+    uint4 *A = reinterpret_cast<uint4 *>(spins + sys * d.N);
+    uint4 *B = reinterpret_cast<uint4 *>(spins + (sys + 1) * d.N);
+    for (int j = threadIdx.x; j < (d.N >> 2); j += blockDim.x) {
+        uint4 x = A[j], y = B[j];
+        uint32_t dd;
+        dd = (x.x ^ y.x) & mask; x.x ^= dd; y.x ^= dd;
+        dd = (x.y ^ y.y) & mask; x.y ^= dd; y.y ^= dd;
+        dd = (x.z ^ y.z) & mask; x.z ^= dd; y.z ^= dd;
+        dd = (x.w ^ y.w) & mask; x.w ^= dd; y.w ^= dd;
+        A[j] = x;
+        B[j] = y;
+    }
+    if (threadIdx.x < 32 && ((mask >> threadIdx.x) & 1u)) {
+        const size_t o = ((size_t)(w * 32 + threadIdx.x) * d.R + a) * d.NT + t;
+        const int64_t u = U[o]; U[o] = U[o + 1]; U[o + 1] = u;
+        const int32_t m = M[o]; M[o] = M[o + 1]; M[o + 1] = m;
+    }
+}
+
+// ------------------------------------------------------------------------------------ hash
+// One warp per system: sum over its words of mix64(index, word) (order-free; sg_get_state_hash).
+__device__ __forceinline__ uint64_t mix64(uint64_t x)
+{
+    x ^= x >> 30; x *= 0xbf58476d1ce4e5b9ULL;
+    x ^= x >> 27; x *= 0x94d049bb133111ebULL;
+    x ^= x >> 31;
+    return x;
+}
+
+__global__ void __launch_bounds__(128)
+k_hash_words(const uint32_t *__restrict__ words, long long n_sys, int words_per_sys, uint64_t *__restrict__ out)
+{
+    const int lane = threadIdx.x & 31;
+    const long long sys = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (sys >= n_sys) return;
+    const uint32_t *p = words + (size_t)sys * words_per_sys;
+    uint64_t h = 0;
+    for (int i = lane; i < words_per_sys; i += 32) h += mix64(((uint64_t)(uint32_t)i << 32) | p[i]);
+    for (int o = 16; o; o >>= 1) h += __shfl_xor_sync(0xffffffffu, h, o);
+    if (lane == 0) out[sys] = h;
 }
 
 // ------------------------------------------------------------------------------- measurement
@@ -434,10 +465,20 @@ int launch_pt_pmj(sg_ctx *c, uint64_t exchange)
     const int npairs = (d.NT - (int)(exchange & 1)) / 2;
     if (npairs <= 0) return 0;
     k_pt_decide_pmj<<<blocks_for((long long)d.W * d.R * npairs, 4), 128, 0, c->stream>>>(
-        d, c->U, c->M, c->tab, c->exp64_tab, c->h, (uint32_t)exchange, npairs, c->swapmask);
-    k_pt_swap_pmj<<<blocks_for((long long)d.W * d.R * npairs * (d.N >> 2), 256), 256, 0, c->stream>>>(
-        d, c->spins, c->swapmask, (uint32_t)exchange, npairs);
+        d, c->U, c->M, c->tab, c->exp64_tab, c->h, (uint32_t)exchange, npairs, c->swapmask, c->pt_acc);
+    k_pt_swap_pmj<<<dim3(npairs, d.R, d.W), 256, 0, c->stream>>>(d, c->spins, c->swapmask, (uint32_t)exchange, npairs,
+                                                                 c->U, c->M);
     return 2;
+}
+
+int launch_hash(sg_ctx *c, uint64_t *dev_out)
+{
+    const Dims &d = c->d;
+    const long long n_sys = (long long)d.W * d.R * d.NT;
+    const int wps = c->kind == SG_PMJ ? d.N : d.N / 4;
+    const uint32_t *words = c->kind == SG_PMJ ? c->spins : reinterpret_cast<const uint32_t *>(c->spins8);
+    k_hash_words<<<blocks_for(n_sys, 4), 128, 0, c->stream>>>(words, n_sys, wps, dev_out);
+    return 1;
 }
 
 int launch_hist_pmj(sg_ctx *c, int s0, int ns)

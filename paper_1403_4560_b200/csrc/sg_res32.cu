@@ -12,7 +12,13 @@
 // p = (colour + pi) & 1 that decides on which side the second x-neighbour sits is warp-uniform.
 // Lane = 8*pair + 4*which + quad; the x-neighbour across a quad boundary comes from the adjacent lane.
 //
-// Energy for the exchange step (R12): in the last colour-1 half sweep every thread accumulates the
+// Exchange step (R12), split over two launches so that it costs no pass over the state: the launch that ends at an
+// exchange point writes per-lane U, M (below); the NEXT launch decides the swap of its pair from those (one warp, 32
+// lanes = 32 samples, the same decision in both CTAs of the pair) and, only for the lanes that swap, merges the
+// partner's configuration into its own while loading ("swap on load").  State and energies are double-buffered
+// (read spins_in / U_in, write spins_out / U) because the partner CTA needs this CTA's old configuration.
+//
+// Energy for the exchange step: in the last colour-1 half sweep every thread accumulates the
 // post-flip unsatisfied-bond counts of its colour-1 sites (every bond has exactly one colour-1 end) and
 // the spin words of both colours in bit-sliced registers; one warp transpose per plane turns them into
 // per-lane integers U, M for the decision kernel.
@@ -26,10 +32,19 @@ namespace sg {
 
 struct Res32Args {
     Dims d;
-    uint32_t *spins;
+    const uint32_t *spins_in; // state before this launch (and before the pending exchange, if any)
+    uint32_t *spins_out;      // state after it (a different buffer: a CTA may need its partner's OLD configuration)
     const uint4 *Jp;          // packed couplings (k_pack_J_res32)
-    int64_t *U;
+    const int64_t *U_in;      // energies of the state in spins_in (read only if do_exchange)
+    const int32_t *M_in;
+    int64_t *U;               // energies of the state in spins_out (written only if want_energy)
     int32_t *M;
+    const SlotTab *tab;       // beta per slot (exchange decision)
+    const double *exp_tab;    // dexp64 table (R12)
+    unsigned long long *pt_acc;
+    double h;
+    int do_exchange;          // apply exchange `exchange` (R12) to the loaded state before sweeping
+    uint32_t exchange;
     uint32_t rk[20];
     uint64_t sweep0;          // global index of the first sweep of this launch
     int n_sweeps;
@@ -188,13 +203,14 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
     uint4 *ring = S4 + 2 * RQ;                                             // [16 warps][2 stages][6][32] 96 KB
     uint64_t *bars = reinterpret_cast<uint64_t *>(ring + R_WARPS * N_STAGES * CHUNK_U4);   // [16][2]
     uint64_t *sysbar_p = bars + R_WARPS * N_STAGES;                        // load barrier of the system
-    int *sUM = reinterpret_cast<int *>(sysbar_p + 1);                      // [2][32]
+    int *sUM = reinterpret_cast<int *>(sysbar_p + 1);                      // [2][32], then [64]: swap mask of this CTA
     const Dims &d = A.d;
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);        // warp-uniform for the compiler: uniform datapath
     const int t = blockIdx.x, a = blockIdx.y, w = blockIdx.z;      // x fastest: the 128 systems of a word are consecutive CTAs
     const int sys = (w * d.R + a) * d.NT + t;
-    uint4 *gS = reinterpret_cast<uint4 *>(A.spins + (size_t)sys * RN);
+    const uint4 *gS = reinterpret_cast<const uint4 *>(A.spins_in + (size_t)sys * RN);
+    uint4 *gO = reinterpret_cast<uint4 *>(A.spins_out + (size_t)sys * RN);
     const int zhalf = warp >> 3, wj = warp & 7;
     // chunk of (colour, Z) for this warp: Jp_w + ((colour * 16 + Z) * 8 + wj) * CHUNK_U4
     const uint4 *Jpw = A.Jp + ((size_t)w * CHUNKS_PER_WORD + wj) * CHUNK_U4;
@@ -229,6 +245,28 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
                          : "memory");
     }
     if (tid < 64) sUM[tid] = 0;
+    // ---- pending exchange: decide the swap of this slot's pair (warp 0; lane l = sample 32 w + l)
+    int partner = -1;
+    if (A.do_exchange) {
+        const int e1 = (int)(A.exchange & 1u), p = t - e1;
+        if (p >= 0 && (p >> 1) < (d.NT - e1) / 2) partner = (p & 1) ? t - 1 : t + 1;
+    }
+    if (warp == 0) {
+        uint32_t mask = 0u;
+        if (partner >= 0) {
+            const int tl = partner < t ? partner : t;               // lower slot of the pair
+            const int smp = w * 32 + lane;
+            const size_t o = ((size_t)smp * d.R + a) * d.NT + tl;
+            const double Et = __dsub_rn((double)(2 * A.U_in[o] - 3 * (int64_t)RN), __dmul_rn(A.h, (double)A.M_in[o]));
+            const double Eu = __dsub_rn((double)(2 * A.U_in[o + 1] - 3 * (int64_t)RN), __dmul_rn(A.h, (double)A.M_in[o + 1]));
+            const double x = __dmul_rn(__dsub_rn(A.tab[tl].beta, A.tab[tl + 1].beta), __dsub_rn(Et, Eu));
+            const uint4 r = philox_rk8(0u, A.exchange, (uint32_t)(smp + d.s_first), ctr3(4, a, tl), A.rk);
+            const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
+            mask = __ballot_sync(0xffffffffu, accept && smp < d.n_samples);
+            if (lane == 0 && tl == t && mask) atomicAdd(&A.pt_acc[tl], (unsigned long long)__popc(mask));
+        }
+        if (lane == 0) sUM[64] = (int)mask;
+    }
 
     SlotK K;                                                // block-uniform: stays in uniform registers / the constant bank
 #pragma unroll
@@ -241,8 +279,25 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
     const uint32_t c3 = ctr3(3, a, t);
     const Geo32 geo = geo_of(wj, lane);
     const int pi = (wj >> 2) & 1;
-    __syncthreads();                                        // sysbar initialised, sUM zeroed
+    __syncthreads();                                        // sysbar initialised, sUM zeroed, swap mask known
     mbar_wait(sysbar, 0u);                                  // the system has landed (async-proxy writes visible)
+    {
+        const uint32_t xmask = (uint32_t)sUM[64];           // block-uniform
+        if (xmask) {                                        // swap on load: take the partner's bits in the swapping lanes
+            const uint4 *gP = reinterpret_cast<const uint4 *>(A.spins_in + (size_t)(sys - t + partner) * RN);
+#pragma unroll 4
+            for (int i = tid; i < 2 * RQ; i += R_THREADS) {
+                uint4 v = S4[i];
+                const uint4 pv = gP[i];
+                v.x ^= (v.x ^ pv.x) & xmask;
+                v.y ^= (v.y ^ pv.y) & xmask;
+                v.z ^= (v.z ^ pv.z) & xmask;
+                v.w ^= (v.w ^ pv.w) & xmask;
+                S4[i] = v;
+            }
+            __syncthreads();
+        }
+    }
 
     auto half_sweep = [&](auto P_tag, auto E_tag, int hs) {
         constexpr int P = decltype(P_tag)::value;
@@ -311,7 +366,7 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
 
     // ---- write back (plain vector stores: a bulk-async store would hold the CTA until its completion — measured slower)
 #pragma unroll 8
-    for (int i = 0; i < 2 * RQ / R_THREADS; ++i) gS[i * R_THREADS + tid] = S4[i * R_THREADS + tid];
+    for (int i = 0; i < 2 * RQ / R_THREADS; ++i) gO[i * R_THREADS + tid] = S4[i * R_THREADS + tid];
 }
 
 // canonical couplings J[w][colour][dir][H] -> packed copy (see above); one thread per packed uint4
@@ -348,7 +403,7 @@ __global__ void __launch_bounds__(256) k_pack_J_res32(Dims d, const uint32_t *__
     Jp[idx] = make_uint4(v[0], v[1], v[2], v[3]);
 }
 
-constexpr size_t RES32_SMEM = (size_t)RN * 4 + (size_t)R_WARPS * N_STAGES * CHUNK_BYTES + R_WARPS * N_STAGES * 8 + 8 + 64 * 4;
+constexpr size_t RES32_SMEM = (size_t)RN * 4 + (size_t)R_WARPS * N_STAGES * CHUNK_BYTES + R_WARPS * N_STAGES * 8 + 8 + 68 * 4;
 
 }  // namespace
 
@@ -357,7 +412,7 @@ size_t res32_packed_bytes(int W) { return (size_t)W * CHUNKS_PER_WORD * CHUNK_BY
 bool res32_supported(const sg_ctx *c)
 {
     const Dims &d = c->d;
-    return c->kind == SG_PMJ && d.fast_accept && d.L == 32 && c->Jp != nullptr;
+    return c->path == SG_PATH_AUTO && c->kind == SG_PMJ && d.fast_accept && d.L == 32 && c->Jp != nullptr;
 }
 
 // packed copy of the couplings (after every k_init_J_pmj)
@@ -371,21 +426,28 @@ int launch_pack_J_res32(sg_ctx *c)
 
 // n_sweeps consecutive sweeps from global sweep index sweep0; want_energy: also write U, M of the final
 // state (fresh energies for the exchange step).  Returns kernels launched (1) or -1.
-int launch_res32_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, bool want_energy)
+int launch_res32_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, bool want_energy, bool do_exchange, uint64_t exchange)
 {
-    static bool configured = false;
-    if (!configured) {
+    if (attr_needed(c, ATTR_RES32)) {
         if (cudaFuncSetAttribute(k_res32_pmj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RES32_SMEM) != cudaSuccess)
             return -1;
-        configured = true;
     }
     const Dims &d = c->d;
     Res32Args A;
     A.d = d;
-    A.spins = c->spins;
+    A.spins_in = c->spins;
+    A.spins_out = c->spins_alt;
     A.Jp = c->Jp;
-    A.U = c->U;
-    A.M = c->M;
+    A.U_in = c->U;
+    A.M_in = c->M;
+    A.U = c->U_alt;
+    A.M = c->M_alt;
+    A.tab = c->tab;
+    A.exp_tab = c->exp64_tab;
+    A.pt_acc = c->pt_acc;
+    A.h = c->h;
+    A.do_exchange = do_exchange ? 1 : 0;
+    A.exchange = (uint32_t)exchange;
     for (int r = 0; r < 10; ++r) {
         A.rk[2 * r] = d.k0 + (uint32_t)r * 0x9E3779B9u;
         A.rk[2 * r + 1] = d.k1 + (uint32_t)r * 0xBB67AE85u;

@@ -12,6 +12,7 @@ import numpy as np
 PMJ, GAUSS = 0, 1
 NK, REC, NMOM = 12, 25, 66
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ESTATE = 0, -1, -2, -3, -4, -5
+PATH_AUTO, PATH_GENERIC = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "csrc", "libsg_b200.so")
@@ -41,7 +42,10 @@ EXPORTS = {
     "sg_get_counters": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "sg_get_launch_count": (C.c_int, [C.c_void_p, C.c_void_p]),
     "sg_last_error": (C.c_char_p, [C.c_void_p]),
-    "sg_probe_alu_peak": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "sg_set_kernel_path": (C.c_int, [C.c_void_p, C.c_int]),
+    "sg_get_state_hash": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "sg_get_energies_cached": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "sg_get_pt_stats": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
 }
 
 if not os.path.exists(LIB_PATH):
@@ -66,15 +70,6 @@ def _p(a):
 
 def sg_workspace_bytes(L, n_samples, n_replicas, n_temps, coupling_kind):
     return int(_lib.sg_workspace_bytes(L, n_samples, n_replicas, n_temps, coupling_kind))
-
-
-def sg_probe_alu_peak(stream=None):
-    """Measured ALU-pipe (LOP3) peak of the current device in lane-ops/s (include/sg.h)."""
-    v = C.c_double()
-    rc = _lib.sg_probe_alu_peak(C.c_void_p(stream.cuda_stream) if stream is not None else None, C.byref(v))
-    if rc != OK:
-        raise SgError(rc, "sg_probe_alu_peak failed")
-    return v.value
 
 
 class Simulation:
@@ -180,6 +175,29 @@ class Simulation:
         M = np.empty((self.n_samples, self.R, self.NT), dtype=np.int32)
         self._check(_lib.sg_get_energies(self._h, _p(U), _p(M)))
         return U, M
+
+    def sg_get_energies_cached(self):
+        """The kernels' own (U, M) (raises SgError(ESTATE) if they are not up to date with the state)."""
+        U = np.empty((self.n_samples, self.R, self.NT), dtype=np.int64)
+        M = np.empty((self.n_samples, self.R, self.NT), dtype=np.int32)
+        self._check(_lib.sg_get_energies_cached(self._h, _p(U), _p(M)))
+        return U, M
+
+    def sg_set_kernel_path(self, path):
+        self._check(_lib.sg_set_kernel_path(self._h, int(path)))
+
+    def sg_get_state_hash(self):
+        nw = (self.n_samples + 31) // 32 if self.kind == PMJ else self.n_samples
+        out = np.empty((nw, self.R, self.NT), dtype=np.uint64)
+        self._check(_lib.sg_get_state_hash(self._h, _p(out)))
+        return out
+
+    def sg_get_pt_stats(self):
+        """(proposed, accepted) per adjacent slot pair, summed over samples and replicas."""
+        prop = np.zeros(max(self.NT - 1, 0), dtype=np.uint64)
+        acc = np.zeros(max(self.NT - 1, 0), dtype=np.uint64)
+        self._check(_lib.sg_get_pt_stats(self._h, _p(prop), _p(acc)))
+        return prop, acc
 
     def sg_get_thresholds(self):
         out = np.empty((self.NT, 7, 2), dtype=np.uint64)

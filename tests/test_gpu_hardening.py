@@ -1,0 +1,369 @@
+"""GPU parity hardening ("Next round" #1; SURVEY.md §8d "Parity protocol at scale").
+
+(a) whole-pool cross-path check: the shared-memory-resident kernels (SG_PATH_AUTO) against the plain
+    global-memory kernels (SG_PATH_GENERIC, the path the oracle pins sample by sample in test_gpu_parity.py)
+    at the FULL pool size of configs 2-5: one 64-bit hash per system + the recounted AND the kernels' own
+    (U, M), bit for bit; the resident path repeated 10 times must reproduce its hashes (no intermittent race).
+(b) the §8d protocol: >= 8 samples per config (first / last word, lanes 0, 13, 31, random) followed by the
+    oracle for the FULL sweep count of configs 2-5 (16 host threads), all samples of config 2 for 32 sweeps.
+(c) the energies the fused kernels compute for themselves (sg_get_energies_cached) against the oracle's tracked
+    (U, M) on tight ladders where 20-80 % of the proposed swaps are accepted; accepted-swap counters
+    (sg_get_pt_stats) equal to the oracle's, summed over every sample of the pool.
+(d) sg_set_first_sample (the multi-GPU keying) on every kernel path against Oracle(sample = first + s).
+"""
+import os
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+import pytest
+
+from paper_1403_4560_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sg():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1403_4560_b200 import sg as _sg
+    return _sg
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import ea_oracle
+    ea_oracle.lib()
+    return ea_oracle
+
+
+def close(a, b, tol=1e-12):
+    a = np.asarray(a)
+    b = np.asarray(b)
+    return np.all(np.abs(a - b) <= tol * np.maximum(np.abs(b), 1.0))
+
+
+def oracle_job(O, L, h, R, temps, kind, seed, sample, plan, measure_at_end=False):
+    """Run one oracle sample through `plan` = [(n_sweeps, pt_every, meas_every), ...]; returns its final state."""
+    o = O.Oracle(L, h, R, temps, kind=kind, seed=seed, sample=sample)
+    for seg in plan:
+        o.run(*seg)
+    if measure_at_end:
+        o.measure(False)
+    U, M = o.energies()
+    mom, n = o.moments()
+    out = dict(spins=o.spins(), U=U, M=M, mom=mom, n=n, pt=o.pt_stats())
+    o.close()
+    return out
+
+
+NCPU = os.cpu_count() or 1
+POOL = ThreadPoolExecutor(max_workers=max(2, min(8, NCPU // 2)))          # short oracle jobs of the tests below
+POOL_LONG = ThreadPoolExecutor(max_workers=max(1, min(32, NCPU - 2)))     # the full-length runs of (b), started at module start
+
+
+# ------------------------------------------------------------------------------------------------ (a)
+# name, runs on both paths: list of ("run", n, pt_every, meas_every) / ("sweep", n) / ("pt",)
+CROSS = [
+    ("C2", [("run", 16, 1, 16), ("sweep", 3), ("pt",), ("run", 5, 1, 0)]),
+    ("C3", [("run", 6, 1, 0), ("sweep", 2), ("pt",)]),
+    ("C4", [("run", 3, 1, 0), ("sweep", 1), ("pt",)]),
+    ("C5", [("run", 16, 4, 0), ("sweep", 16), ("pt",), ("run", 8, 4, 0)]),
+]
+
+
+def _apply(sim, ops):
+    for op in ops:
+        if op[0] == "run":
+            sim.sg_run(*op[1:])
+        elif op[0] == "sweep":
+            sim.sg_sweep(op[1])
+        else:
+            sim.sg_pt_exchange()
+
+
+@pytest.mark.parametrize("case", CROSS, ids=[c[0] for c in CROSS])
+def test_whole_pool_resident_path_equals_generic_path(sg, case):
+    name, ops = case
+    w = W.BY_NAME[name]
+    temps = w.temps()
+    fast = sg.Simulation(w.L, w.h, w.n_samples, w.n_replicas, temps, w.kind, w.seed)
+    _apply(fast, ops)
+    h_fast = fast.sg_get_state_hash()
+    Uc, Mc = fast.sg_get_energies_cached()          # the last operation is an exchange: the kernels' own energies
+    Ur, Mr = fast.sg_get_energies()                 # recount of the same state
+    assert np.array_equal(Uc, Ur) and np.array_equal(Mc, Mr), "%s: the fused kernels' own U, M differ from the recount" % name
+    mom_fast, n_fast = fast.sg_get_moments()
+    acc_fast = fast.sg_get_pt_stats()
+    # determinism: the same run again (9 more times) must reproduce every hash
+    for rep in range(9):
+        fast.sg_reset()
+        _apply(fast, ops)
+        assert np.array_equal(fast.sg_get_state_hash(), h_fast), "%s: repeat %d of the resident path differs" % (name, rep)
+    fast.close()
+    gen = sg.Simulation(w.L, w.h, w.n_samples, w.n_replicas, temps, w.kind, w.seed)
+    gen.sg_set_kernel_path(sg.PATH_GENERIC)
+    _apply(gen, ops)
+    h_gen = gen.sg_get_state_hash()
+    bad = np.argwhere(h_gen != h_fast)
+    assert bad.size == 0, "%s: %d of %d systems differ between the paths, first (word, replica, slot) = %s" % (
+        name, len(bad), h_gen.size, bad[0])
+    Ug, Mg = gen.sg_get_energies()
+    assert np.array_equal(Ug, Ur) and np.array_equal(Mg, Mr)
+    Ugc, Mgc = gen.sg_get_energies_cached()
+    assert np.array_equal(Ugc, Ur) and np.array_equal(Mgc, Mr)
+    mom_gen, n_gen = gen.sg_get_moments()
+    assert n_gen == n_fast and close(mom_fast, mom_gen)
+    acc_gen = gen.sg_get_pt_stats()
+    assert np.array_equal(acc_fast[0], acc_gen[0]) and np.array_equal(acc_fast[1], acc_gen[1])
+    assert acc_gen[0].sum() > 0
+    gen.close()
+
+
+@pytest.mark.parametrize("seed", list(range(100, 112)))
+def test_l32_stress_many_seeds_whole_pool(sg, seed):
+    """ADVICE round 1 (sg_res32.cu ring-stage reuse): config-5-shaped runs with different seeds, EVERY word of
+    the pool compared with the generic path, on a ladder tight enough that swaps happen (swap-on-load path)."""
+    temps = W.ladder(1.30, 1.36, 8)
+    nw = 24
+    fast = sg.Simulation(32, 0.2, 32 * nw, 4, temps, sg.PMJ, seed)
+    gen = sg.Simulation(32, 0.2, 32 * nw, 4, temps, sg.PMJ, seed)
+    gen.sg_set_kernel_path(sg.PATH_GENERIC)
+    for sim in (fast, gen):
+        sim.sg_run(12, 4, 0)
+        sim.sg_run(7, 2, 0)
+    assert np.array_equal(fast.sg_get_state_hash(), gen.sg_get_state_hash())
+    pf, af = fast.sg_get_pt_stats()
+    pg, ag = gen.sg_get_pt_stats()
+    assert np.array_equal(pf, pg) and np.array_equal(af, ag)
+    assert 0.02 * pf.sum() < af.sum() < 0.98 * pf.sum()
+    fast.close(); gen.close()
+
+
+# ------------------------------------------------------------------------------------------------ (b)
+def _protocol_samples(n, seed):
+    rng = np.random.default_rng(seed)
+    base = [0, 13, 31, n - 32, n - 32 + 13, n - 1]
+    extra = [int(x) for x in rng.choice(np.arange(32, n - 32), size=2, replace=False)]
+    return sorted(set(base + extra))
+
+
+def _plan(w):
+    half = w.n_sweeps // 2
+    if w.meas_every:
+        return [(half, w.pt_every, 0), (w.n_sweeps - half, w.pt_every, w.meas_every)]
+    return [(w.n_sweeps, w.pt_every, 0)]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def oracle_full_runs(O, sg):
+    """Start the oracle on 8 samples of each of configs 2-5 for the FULL sweep count (bench.py's step plan) when the
+    module starts, on the host cores, while the other tests run; the protocol tests at the end collect the futures."""
+    jobs = {}
+    for name in ("C4", "C3", "C5", "C2"):            # longest first
+        w = W.BY_NAME[name]
+        for s in _protocol_samples(w.n_samples, w.seed):
+            jobs[(name, s)] = POOL_LONG.submit(oracle_job, O, w.L, w.h, w.n_replicas, w.temps(), w.kind, w.seed, s, _plan(w),
+                                          not w.meas_every)
+    return jobs
+
+
+def test_all_samples_of_config2_first_32_sweeps(sg, O):
+    """every one of the 2048 samples of config 2 for the first 32 sweeps (PT every sweep,
+    one measurement at sweep 16 and 32)."""
+    w = W.BY_NAME["C2"]
+    temps = w.temps()
+    sim = sg.Simulation(w.L, w.h, w.n_samples, w.n_replicas, temps, w.kind, w.seed)
+    sim.sg_run(32, 1, 16)
+    spins = sim.sg_get_spins()
+    Uc, Mc = sim.sg_get_energies_cached()
+    mom, n = sim.sg_get_moments()
+    prop, acc = sim.sg_get_pt_stats()
+    futs = [POOL.submit(oracle_job, O, w.L, w.h, w.n_replicas, temps, w.kind, w.seed, s, [(32, 1, 16)])
+            for s in range(w.n_samples)]
+    acc_oracle = 0
+    for s, f in enumerate(futs):
+        want = f.result()
+        assert np.array_equal(spins[s], want["spins"]), "sample %d" % s
+        assert np.array_equal(Uc[s], want["U"]) and np.array_equal(Mc[s], want["M"]), "sample %d: kernels' own energies" % s
+        assert close(mom[s], want["mom"])
+        acc_oracle += want["pt"][1]
+    assert int(acc.sum()) == acc_oracle            # accepted swaps, whole pool
+    sim.close()
+
+
+def test_config5_first_sweeps_many_samples(sg, O):
+    """SURVEY.md §8d (1) for config 5 (4 sweeps, one exchange): three whole words (96 samples) + lane 7 of 32 more words."""
+    w = W.BY_NAME["C5"]
+    temps = w.temps()
+    sim = sg.Simulation(w.L, w.h, w.n_samples, w.n_replicas, temps, w.kind, w.seed)
+    sim.sg_run(4, 4, 0)
+    Uc, Mc = sim.sg_get_energies_cached()
+    samples = list(range(0, 32)) + list(range(32 * 100, 32 * 101)) + list(range(w.n_samples - 32, w.n_samples)) + \
+        [32 * k + 7 for k in range(1, 256, 8)]
+    futs = {s: POOL.submit(oracle_job, O, w.L, w.h, w.n_replicas, temps, w.kind, w.seed, s, [(4, 4, 0)]) for s in samples}
+    for s, f in futs.items():
+        want = f.result()
+        assert np.array_equal(sim.sg_get_spins(s, 1)[0], want["spins"]), "sample %d" % s
+        assert np.array_equal(Uc[s], want["U"]) and np.array_equal(Mc[s], want["M"])
+    sim.close()
+
+
+# ------------------------------------------------------------------------------------------------ (c)
+TIGHT = [
+    # name, L, h, n_samples, R, NT, (T_lo, T_hi), kind, pt_every, n_sweeps
+    ("ladder8", 8, 0.2, 64, 4, 12, (0.8, 1.6), 0, 1, 24),
+    ("ladder8-pt2", 8, -0.3, 40, 2, 9, (0.7, 1.4), 0, 2, 24),
+    ("ladder-L10", 10, 0.1, 33, 4, 10, (0.9, 1.5), 0, 1, 20),
+    ("ladder-L12", 12, 0.1, 32, 4, 12, (0.9, 1.5), 0, 1, 16),
+    ("ladder-L16", 16, 0.2, 32, 2, 8, (1.0, 1.3), 0, 2, 12),
+    ("ladder-L6", 6, 0.3, 37, 4, 7, (0.6, 2.0), 0, 1, 30),
+    ("res32", 32, 0.2, 33, 2, 6, (1.30, 1.40), 0, 4, 16),
+    ("res32-pt1", 32, -0.1, 32, 4, 5, (1.50, 1.58), 0, 1, 6),
+    ("gladder-L8", 8, 0.3, 6, 4, 10, (0.7, 1.6), 1, 1, 20),
+    ("gladder-L16", 16, 0.3, 3, 2, 8, (0.9, 1.3), 1, 1, 8),
+    ("generic-pmj-L4-big-h", 4, 1.7, 32, 2, 8, (1.0, 4.0), 0, 1, 30),
+    ("generic-gauss-L6", 6, 0.2, 4, 2, 8, (0.6, 1.8), 1, 1, 20),
+]
+
+
+@pytest.mark.parametrize("case", TIGHT, ids=[c[0] for c in TIGHT])
+def test_fused_kernels_own_energies_and_acceptance_on_tight_ladders(sg, O, case):
+    _, L, h, ns, R, NT, (Tlo, Thi), kind, pt_every, n_sweeps = case
+    temps = W.ladder(Tlo, Thi, NT)
+    sim = sg.Simulation(L, h, ns, R, temps, kind, 77)
+    sim.sg_run(n_sweeps, pt_every, 0)
+    Uc, Mc = sim.sg_get_energies_cached()
+    spins = sim.sg_get_spins()
+    prop, acc = sim.sg_get_pt_stats()
+    futs = [POOL.submit(oracle_job, O, L, h, R, temps, kind, 77, s, [(n_sweeps, pt_every, 0)]) for s in range(ns)]
+    prop_o = acc_o = 0
+    for s, f in enumerate(futs):
+        want = f.result()
+        assert np.array_equal(spins[s], want["spins"]), "sample %d: spins" % s
+        assert np.array_equal(Uc[s], want["U"]), "sample %d: the kernel's own U differs from the oracle's tracked U" % s
+        assert np.array_equal(Mc[s], want["M"]), "sample %d: the kernel's own M" % s
+        prop_o += want["pt"][0]
+        acc_o += want["pt"][1]
+    assert int(prop.sum()) == prop_o and int(acc.sum()) == acc_o
+    assert 0.2 * prop_o <= acc_o <= 0.8 * prop_o, "acceptance %d / %d outside 20-80 %%: the ladder does not exercise the swap" % (acc_o, prop_o)
+    # a sweep without exchange invalidates the kernels' energies
+    sim.sg_sweep(1)
+    with pytest.raises(sg.SgError) as e:
+        sim.sg_get_energies_cached()
+    assert e.value.code == sg.ESTATE
+    # the separate exchange primitive refreshes them (and permutes them with the configurations)
+    sim.sg_pt_exchange()
+    Uc, Mc = sim.sg_get_energies_cached()
+    Ur, Mr = sim.sg_get_energies()
+    assert np.array_equal(Uc, Ur) and np.array_equal(Mc, Mr)
+    sim.close()
+
+
+# ------------------------------------------------------------------------------------------------ (d)
+SHARD = [
+    # name, L, h, R, NT, kind, force generic path
+    ("ladder8", 8, 0.2, 4, 6, 0, False),
+    ("ladder-L12", 12, 0.1, 2, 4, 0, False),
+    ("ladder-L6", 6, 0.1, 2, 5, 0, False),
+    ("res32", 32, 0.2, 2, 3, 0, False),
+    ("generic-pmj-L8", 8, 0.2, 2, 4, 0, True),
+    ("generic-pmj-L32", 32, 0.2, 2, 2, 0, True),
+    ("gladder-L8", 8, 0.3, 2, 4, 1, False),
+    ("generic-gauss-L8", 8, 0.3, 2, 4, 1, True),
+    ("generic-gauss-L6", 6, 0.3, 2, 4, 1, False),
+]
+
+
+@pytest.mark.parametrize("first", [96, 4096])
+@pytest.mark.parametrize("case", SHARD, ids=[c[0] for c in SHARD])
+def test_first_sample_keys_every_kernel_path(sg, O, case, first):
+    """sg_set_first_sample(F): local sample s must be GLOBAL sample F + s on every kernel path (couplings, initial
+    state, sweep draws keyed by the global word, PT draws by the global sample)."""
+    _, L, h, R, NT, kind, generic = case
+    ns = 64 if kind == 0 else 5
+    temps = W.ladder(1.0, 1.3, NT)
+    sim = sg.Simulation(L, h, ns, R, temps, kind, 9)
+    if generic:
+        sim.sg_set_kernel_path(sg.PATH_GENERIC)
+    sim.sg_set_first_sample(first)
+    sim.sg_reset()
+    sim.sg_run(6, 1, 3)
+    sim.sg_sweep(1)
+    sim.sg_pt_exchange()
+    mom, n = sim.sg_get_moments()
+    picks = [0, 13, 31, 32, ns - 1] if kind == 0 else [0, 2, ns - 1]
+    futs = {s: POOL.submit(oracle_job, O, L, h, R, temps, kind, 9, first + s, [(6, 1, 3), (1, 1, 0)]) for s in picks}
+    Uc, Mc = sim.sg_get_energies_cached()
+    for s, f in futs.items():
+        want = f.result()
+        Jg = sim.sg_get_couplings(s, 1)[0]
+        o = O.Oracle(L, h, R, temps, kind=kind, seed=9, sample=first + s)
+        assert np.array_equal(Jg.view(np.uint32), o.couplings().view(np.uint32))
+        o.close()
+        assert np.array_equal(sim.sg_get_spins(s, 1)[0], want["spins"]), "local sample %d (global %d)" % (s, first + s)
+        assert np.array_equal(Uc[s], want["U"]) and np.array_equal(Mc[s], want["M"])
+        assert close(mom[s], want["mom"])
+    sim.close()
+
+
+def test_shard_equals_slice_of_unsharded_pool(sg):
+    """A shard [F, F + 64) of a 160-sample pool is bit-identical to samples F.. of the unsharded run (both kinds)."""
+    for kind, L, F, ns_all, ns in ((0, 8, 96, 160, 64), (1, 8, 3, 8, 4)):
+        temps = W.ladder(1.0, 1.3, 5)
+        whole = sg.Simulation(L, 0.2, ns_all, 2, temps, kind, 21)
+        part = sg.Simulation(L, 0.2, ns, 2, temps, kind, 21)
+        part.sg_set_first_sample(F)
+        part.sg_reset()
+        for sim in (whole, part):
+            sim.sg_run(9, 1, 4)
+        assert np.array_equal(part.sg_get_spins(), whole.sg_get_spins(F, ns))
+        assert np.array_equal(part.sg_get_moments()[0], whole.sg_get_moments()[0][F:F + ns])
+        whole.close(); part.close()
+
+
+def test_sweep_counter_guard(sg):
+    sim = sg.Simulation(4, 0.1, 1, 2, [1.0, 2.0])
+    sim.sg_sweep(1)
+    with pytest.raises(sg.SgError) as e:
+        sim.sg_sweep(2**31 - 1)          # 1 + (2^31 - 1) = 2^31: the Philox time word 2 * sweep + colour would wrap
+    assert e.value.code == sg.EINVAL
+    with pytest.raises(sg.SgError):
+        sim.sg_run(2**31 - 1, 1, 0)
+    with pytest.raises(sg.SgError):
+        sim.sg_set_kernel_path(7)
+    sim.close()
+
+
+@pytest.mark.parametrize("name", ["C2", "C5", "C3", "C4"])
+def test_full_sweep_count_protocol(sg, oracle_full_runs, name):
+    """>= 8 chosen samples for the FULL run of the config, in bench.py's launch shapes
+    (first half without measurement, second half with the config's cadence): spins, (U, M) bit-exact, moments 1e-12."""
+    w = W.BY_NAME[name]
+    samples = _protocol_samples(w.n_samples, w.seed)
+    assert len(samples) >= 8
+    sim = sg.Simulation(w.L, w.h, w.n_samples, w.n_replicas, w.temps(), w.kind, w.seed)
+    for seg in _plan(w):
+        sim.sg_run(*seg)
+    if not w.meas_every:
+        sim.sg_measure(False)
+    Uc, Mc = sim.sg_get_energies_cached() if w.n_sweeps % w.pt_every == 0 else (None, None)
+    U, M = sim.sg_get_energies()
+    mom, n_meas = sim.sg_get_moments()
+    prop, acc = sim.sg_get_pt_stats()
+    assert sim.sg_get_counters() == (w.n_sweeps, w.n_sweeps // w.pt_every)
+    for s in samples:
+        want = oracle_full_runs[(name, s)].result()
+        got = sim.sg_get_spins(s, 1)[0]
+        assert np.array_equal(got, want["spins"]), "%s sample %d: %d spins differ after the full run" % (
+            name, s, int((got != want["spins"]).sum()))
+        assert np.array_equal(U[s], want["U"]) and np.array_equal(M[s], want["M"])
+        if Uc is not None:
+            assert np.array_equal(Uc[s], want["U"]) and np.array_equal(Mc[s], want["M"]), "%s sample %d: kernels' own energies" % (name, s)
+        assert n_meas == want["n"]
+        assert close(mom[s], want["mom"]), "%s sample %d: moments differ by %g" % (name, s, np.abs(mom[s] - want["mom"]).max())
+    assert prop.sum() == (w.n_sweeps // w.pt_every) // 2 * (w.n_temps // 2 + (w.n_temps - 1) // 2) * w.n_samples * w.n_replicas \
+        + ((w.n_sweeps // w.pt_every) % 2) * (w.n_temps // 2) * w.n_samples * w.n_replicas
+    assert np.all(acc <= prop)
+    sim.close()
