@@ -1,21 +1,23 @@
 #!/usr/bin/env python
 """bench.py — spin-flip attempts per ns of the B200 hot path (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl ours|reference]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
 A step = one pass of the whole hot path over one batch of synthetic input:
-sg_reset (disorder + initial state on device) -> first half of the sweeps with parallel tempering
-(thermalisation) -> second half with PT and overlap measurement + accumulation.
-Default workload: BASELINE.json configs[1] (C2: L=8, 2048 samples, 4 replicas, 20 temperatures,
-2^14 sweeps, PT every sweep).  `value` = flip attempts of all ranks / device time (max over ranks).
-N > 1: every rank simulates its own 2048-sample shard of a larger disorder pool (weak scaling,
-global Philox keys, no data-path collective; one final all-reduce of the per-slot moment sums).
-Prints ONE JSON line on rank 0.
+sg_reset (disorder + initial state on device) -> the config's sweeps with parallel tempering at its cadence
+(first half = thermalisation; second half with overlap measurement + accumulation where the
+config measures).  Default workload: BASELINE.json configs[4] (C5: L=32, 8192 samples, 4 replicas,
+32 temperatures, 1024 sweeps, PT every 4) — the largest single-GPU config, the one north_star calls the
+throughput run.  `value` = flip attempts of all ranks / device time (max over ranks).  The same JSON line
+carries short runs of the other +-J configs and of the Gaussian one (`other_configs`).
+N > 1: every rank simulates its own shard of a larger disorder pool (weak scaling, global Philox keys, no
+data-path collective; one final all-reduce of the per-slot moment / energy sums).  Prints ONE JSON line on rank 0.
 """
 import argparse
 import json
 import os
+import subprocess
 import sys
 import threading
 import time
@@ -30,9 +32,11 @@ from paper_1403_4560_b200 import workloads as W  # noqa: E402
 ALU_OPS_PER_WORDSITE = 30     # algorithmic ALU-pipe lane-ops per 32-sample word-site update:
 #                               6 bond XOR3 + 8 count + 7 threshold carries + 4 compare/flip + 5 Philox share
 HBM_BYTES_PER_WORDSITE_LAUNCH = 8   # spin word read once + written once per LAUNCH of a resident kernel
-# dram__bytes_read.sum + dram__bytes_write.sum of the roofline launch below, from the ncu --set full captures
-# summarised in profiles/r01_v3_resident_kernels.md (C2) and profiles/r01_v4_final_kernels.md (C3, C5)
-NCU_TRAFFIC_BYTES = {"C2": 10.92e6, "C3": 114.6e6, "C5": 8.746e9}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE roofline launch (the sweep kernel alone, n_k sweeps), from the
+# `ncu --set full` capture named beside it; a pointer to profiles/, not re-measured by this run
+NCU_TRAFFIC = {"C2": (10.92e6, "profiles/r01_v3_resident_kernels.md"),
+               "C3": (114.6e6, "profiles/r01_v4_final_kernels.md"),
+               "C5": (8.746e9, "profiles/r01_v4_final_kernels.md")}
 ALU_LANES_PER_SM = 64         # INT/LOP3 lanes per SM per clock (16 per SMSP x 4; B300_MICROARCH pipe table)
 N_SM = 148
 
@@ -53,11 +57,11 @@ def probe_alu_peak(stream):
 
 
 def peaks():
-    p = {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback"}
+    p = {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback (B200_PROFILING.md)"}
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
             j = json.load(f)
-        p.update(hbm_gbs=float(j["hbm_gbs"]), sm_max_mhz=float(j.get("sm_max_mhz", 1965.0)), src="measured")
+        p.update(hbm_gbs=float(j["hbm_gbs"]), sm_max_mhz=float(j.get("sm_max_mhz", 1965.0)), src="MEASURED_PEAKS.json")
     except Exception:
         pass
     return p
@@ -141,16 +145,15 @@ def run_reference(args, w):
         return
     cores = os.cpu_count() or 1
     threads = min(cores, 32)
-    per_sweep = w.N * w.n_replicas * w.n_temps * 40e-9            # ~40 ns per attempt per core
-    n_sweeps = int(max(16, min(w.n_sweeps, 4.0 / per_sweep)))       # ~4 s of CPU work per sample
-    n_sweeps -= n_sweeps % max(1, 2 * max(w.meas_every, 1))
-    n_sweeps = max(n_sweeps, 2 * max(w.meas_every, 1))
+    per_sweep = w.N * w.n_replicas * w.n_temps * 15e-9            # ~15 ns per attempt per core
+    n_sweeps = int(max(8, min(w.n_sweeps, 4.0 / per_sweep)))        # ~4 s of CPU work per sample
+    q = max(1, 2 * max(w.meas_every, 1), 2 * w.pt_every)
+    n_sweeps = max(q, n_sweeps - n_sweeps % q)
     for _ in range(args.warmup):
         oracle_rate(w, threads, max(2, n_sweeps // 16), threads)
-    rates, secs = [], []
+    secs = []
     for _ in range(args.steps):
-        r, dt = oracle_rate(w, threads, n_sweeps, threads)
-        rates.append(r)
+        _, dt = oracle_rate(w, threads, n_sweeps, threads)
         secs.append(dt)
     total_attempts = w.N * threads * w.n_replicas * w.n_temps * n_sweeps * args.steps
     value = total_attempts / sum(secs) / 1e9
@@ -168,9 +171,11 @@ def run_reference(args, w):
 
 def workload_config(w, n_gpus):
     return {"workload": "%s: L=%d, %d samples/GPU x %d replicas x %d temperatures, %s couplings, h=%g, %d sweeps, "
-                        "PT every %d, measure every %d in the 2nd half" % (
+                        "PT every %d, %s" % (
                             w.name, w.L, w.n_samples, w.n_replicas, w.n_temps, "+-J" if w.kind == W.PMJ else "Gaussian fp32",
-                            w.h, w.n_sweeps, w.pt_every, w.meas_every),
+                            w.h, w.n_sweeps, w.pt_every,
+                            ("measure every %d in the 2nd half" % w.meas_every) if w.meas_every else
+                            "no measurement inside the step (R16)"),
             "L": w.L, "n_samples_per_gpu": w.n_samples, "n_replicas": w.n_replicas, "n_temps": w.n_temps,
             "n_sweeps": w.n_sweeps, "pt_every": w.pt_every, "meas_every": w.meas_every, "seed": w.seed,
             "parallelism": "samples sharded over %d GPU(s), no data-path collective" % n_gpus,
@@ -178,6 +183,108 @@ def workload_config(w, n_gpus):
 
 
 # -------------------------------------------------------------------------------- our arm
+def wordsites_per_sweep(w):
+    if w.kind == W.PMJ:
+        return w.N * w.n_words * w.n_replicas * w.n_temps
+    return w.N * w.n_samples * w.n_replicas * w.n_temps
+
+
+def time_steps(sim, w, plan, steps, warmup, stream, flush, barrier):
+    """W untimed + K timed steps; returns (per-step ms list, launches in the timed steps)."""
+    import torch
+
+    def step():
+        sim.sg_reset()
+        for seg in plan:
+            sim.sg_run(*seg)
+
+    for _ in range(warmup):
+        step()
+    barrier()
+    launches0 = sim.sg_get_launch_count()
+    evs = []
+    with torch.cuda.stream(stream):
+        for _ in range(steps):
+            flush.zero_()                                  # L2 flush, outside the events
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            step()
+            e1.record(stream)
+            evs.append((e0, e1))
+    barrier()
+    return [a.elapsed_time(b) for a, b in evs], sim.sg_get_launch_count() - launches0
+
+
+def time_sweep_kernel(sim, w, stream, dev, reps=3):
+    """The dominant kernel alone (the sweep), same process and clocks: CUDA events on the library's stream around each
+    of `reps` launches of n_k back-to-back sweeps.  Returns (ms per n_k sweeps, n_k, launches per n_k sweeps)."""
+    import torch
+    n_k = 256 if w.N * w.n_samples < (1 << 28) else 16
+    sim.sg_sweep(8)
+    l0 = sim.sg_get_launch_count()
+    kev = []
+    for _ in range(reps):
+        k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k0.record(stream)
+        sim.sg_sweep(n_k)
+        k1.record(stream)
+        kev.append((k0, k1))
+    torch.cuda.synchronize(dev)
+    launches = (sim.sg_get_launch_count() - l0) // reps
+    return float(sum(a.elapsed_time(b) for a, b in kev)) / reps, n_k, launches
+
+
+def roofline_block(w, sweep_ms, n_k, sweep_launches, step_ms, alu_peak, pk):
+    ws = wordsites_per_sweep(w)
+    nominal = ALU_LANES_PER_SM * N_SM * pk["sm_max_mhz"] * 1e6 / 1e12       # T lane-ops / s
+    sweep_rate = w.flip_attempts(n_k) / (sweep_ms * 1e6)
+    launch_s = sweep_ms * 1e-3 / max(1, sweep_launches)
+    share = (sweep_ms / n_k) * w.n_sweeps / step_ms
+    if w.kind != W.PMJ:
+        return {"bound": "alu", "kernel": "sweep (Gaussian fp32 byte path)", "achieved": None, "peak": None, "unit": "Tlaneop/s",
+                "frac": None, "traffic": None, "sweep_only_flips_per_ns": sweep_rate, "share_of_step": share,
+                "launch_us": 1e6 * launch_s, "sweeps_per_launch": n_k // max(1, sweep_launches),
+                "note": "BASELINE.json sets no roofline target for the Gaussian path (parity only); no op-count model is claimed"}
+    ach = ALU_OPS_PER_WORDSITE * ws * n_k / (sweep_ms * 1e-3) / 1e12
+    hbm_ach = HBM_BYTES_PER_WORDSITE_LAUNCH * ws / launch_s / 1e9
+    traffic, traffic_src = NCU_TRAFFIC.get(w.name, (None, None))
+    return {"bound": "alu", "kernel": "sweep (+-J multispin)", "achieved": ach, "peak": alu_peak, "unit": "Tlaneop/s",
+            "frac": ach / alu_peak, "traffic": traffic,
+            "traffic_source": ("ncu --set full capture of one such launch, summarised in %s (an earlier commit's capture; "
+                               "a pointer, not re-measured by this run)" % traffic_src) if traffic_src else None,
+            "peak_source": "measured in this run: dependency-free LOP3 micro-benchmark (csrc/probe/alu_probe.cu); "
+                           "nominal 64 INT lanes/SM/clk x 148 SMs x %.0f MHz = %.2f" % (pk["sm_max_mhz"], nominal),
+            "peak_nominal": nominal, "frac_of_nominal": ach / nominal,
+            "alu_ops_per_wordsite": ALU_OPS_PER_WORDSITE, "launch_us": 1e6 * launch_s,
+            "sweeps_per_launch": n_k // max(1, sweep_launches),
+            "sweep_only_flips_per_ns": sweep_rate, "share_of_step": share,
+            "hbm": {"achieved": hbm_ach, "peak": pk["hbm_gbs"], "peak_source": pk["src"], "unit": "GB/s", "frac": hbm_ach / pk["hbm_gbs"],
+                    "note": "algorithmic 8 B per word-site per LAUNCH (state resident in shared memory for all "
+                            "sweeps of a launch): HBM is not the binding roof, the ALU pipe is (DESIGN.md 6)"}}
+
+
+def short_run(sg, torch, name, sweeps, dev, stream, flush, alu_peak, pk):
+    """A short run of another config for the `other_configs` block: whole-step value (same cadence, fewer sweeps),
+    sweep kernel alone, roofline fraction."""
+    w = W.BY_NAME[name].scaled(n_sweeps=sweeps)
+    temps = np.asarray(w.temps(), dtype=np.float64)
+    sim = sg.Simulation(w.L, w.h, w.n_samples, w.n_replicas, temps, w.kind, w.seed, stream=stream)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+
+    ms, launches = time_steps(sim, w, step_plan(w), 2, 1, stream, flush, barrier)
+    step_ms = float(np.mean(ms))
+    sweep_ms, n_k, sl = time_sweep_kernel(sim, w, stream, dev)
+    prop, acc = sim.sg_get_pt_stats()
+    sim.close()
+    rb = roofline_block(w, sweep_ms, n_k, sl, step_ms, alu_peak, pk)
+    return {"workload": "%s at %d of %d sweeps (same PT / measurement cadence)" % (name, sweeps, W.BY_NAME[name].n_sweeps),
+            "value": w.flip_attempts() / (step_ms * 1e6), "unit": "flips/ns", "ms_per_step": step_ms,
+            "sweep_only_flips_per_ns": rb["sweep_only_flips_per_ns"], "frac": rb["frac"], "gpu_launches_per_step": launches // 2,
+            "pt_acceptance": float(acc.sum()) / max(1.0, float(prop.sum()))}
+
+
 def run_ours(args, w):
     import torch
     import torch.distributed as dist
@@ -203,57 +310,22 @@ def run_ours(args, w):
     plan = step_plan(w)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
-    def step():
-        sim.sg_reset()
-        for seg in plan:
-            sim.sg_run(*seg)
-
     def barrier():
         torch.cuda.synchronize(dev)
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    for _ in range(args.warmup):
-        step()
-    barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    launches0 = sim.sg_get_launch_count()
-    evs = []
-    with torch.cuda.stream(stream):
-        for _ in range(args.steps):
-            flush.zero_()                                  # L2 flush, outside the events
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            step()
-            e1.record(stream)
-            evs.append((e0, e1))
-    barrier()
-    launches = sim.sg_get_launch_count() - launches0
-    step_ms = [a.elapsed_time(b) for a, b in evs]
+    step_ms, launches = time_steps(sim, w, plan, args.steps, args.warmup, stream, flush, barrier)
     total_ms = float(sum(step_ms))
-
-    # dominant kernel alone (the sweep), same process and clocks: CUDA events on the library's stream around
-    # each of `reps` launches of n_k back-to-back sweeps (one launch each on the resident-kernel paths)
-    n_k = 256 if w.N * w.n_samples < (1 << 28) else 16
-    reps = 3
-    sim.sg_sweep(8)
-    l0 = sim.sg_get_launch_count()
-    kev = []
-    for _ in range(reps):
-        k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        k0.record(stream)
-        sim.sg_sweep(n_k)
-        k1.record(stream)
-        kev.append((k0, k1))
-    torch.cuda.synchronize(dev)
-    sweep_launches = sim.sg_get_launch_count() - l0
-    sweep_ms = float(sum(a.elapsed_time(b) for a, b in kev)) / reps          # per n_k sweeps
-    sweep_launches //= reps
-    alu_peak_measured = probe_alu_peak(stream) / 1e12                  # T lane-ops/s, LOP3 micro-benchmark
+    sweep_ms, n_k, sweep_launches = time_sweep_kernel(sim, w, stream, dev)
+    prop, acc = sim.sg_get_pt_stats()
     sampler.stop_flag = True
     sampler.join()
+    alu_peak_measured = probe_alu_peak(stream) / 1e12                        # T lane-ops/s, LOP3 micro-benchmark
+    sim.close()
 
     t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
     if world > 1:
@@ -262,13 +334,20 @@ def run_ours(args, w):
     attempts_per_step = w.flip_attempts() * world
     value = attempts_per_step * args.steps / (total_ms_max * 1e6)          # per ns
 
-    # end to end through the C-ABI with host buffers: create (host temperatures -> device tables),
-    # run, read the moment accumulators back into pinned host memory, destroy.
-    pinned = torch.empty((w.n_samples, w.n_temps, sg.NMOM), dtype=torch.float64).pin_memory()
-    pin_np = pinned.numpy()
+    # end to end through the C-ABI with host buffers: create (host temperatures -> device tables), run, read the
+    # step's result back into pinned host memory (moment accumulators where the config measures, else the per-system
+    # energies (U, M) the run ended with), destroy.
+    measures = w.meas_every > 0
+    if measures:
+        pinned = torch.empty((w.n_samples, w.n_temps, sg.NMOM), dtype=torch.float64).pin_memory()
+        pin_np = pinned.numpy()
+        d2h = pin_np.nbytes
+    else:
+        pinU = torch.empty((w.n_samples, w.n_replicas, w.n_temps), dtype=torch.int64).pin_memory()
+        pinM = torch.empty((w.n_samples, w.n_replicas, w.n_temps), dtype=torch.int32).pin_memory()
+        d2h = pinU.numpy().nbytes + pinM.numpy().nbytes
     e2e_steps = max(1, min(args.steps, 3))
     h2d = w.n_temps * 8 + w.n_temps * 192 + 5761 * 8 + 1441 * 4 + 2 * w.L * 8
-    d2h = pin_np.nbytes
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
@@ -277,7 +356,10 @@ def run_ours(args, w):
         s2.sg_reset()
         for seg in plan:
             s2.sg_run(*seg)
-        s2.sg_get_moments_into(pin_np)
+        if measures:
+            s2.sg_get_moments_into(pin_np)
+        else:
+            s2.sg_get_energies_cached_into(pinU.numpy(), pinM.numpy())
         s2.close()
     torch.cuda.synchronize(dev)
     e2e_s = time.perf_counter() - t0
@@ -286,54 +368,59 @@ def run_ours(args, w):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     e2e_value = attempts_per_step * e2e_steps / (float(t.item()) * 1e9)
 
-    # the one exchange step of the sharded job: disorder sums of the moment accumulators
-    sums = torch.from_numpy(pin_np.sum(axis=0)).to(dev)
-    if world > 1:
-        dist.all_reduce(sums, op=dist.ReduceOp.SUM)
+    # the one exchange step of the sharded job: disorder sums over ALL ranks' samples of what the
+    # step returned; reported so that the reduction is exercised and checkable (N = 1: the local sums)
+    if measures:
+        local = torch.from_numpy(pin_np.sum(axis=0)).to(dev)                 # [n_temps][NMOM]
+    else:
+        local = torch.stack([torch.from_numpy(pinU.numpy().sum(axis=(0, 1)).astype(np.float64)),
+                             torch.from_numpy(pinM.numpy().sum(axis=(0, 1)).astype(np.float64))]).to(dev)
+    sums = shard.reduce_moment_sums(local)
+    n_sys = float(w.n_samples * world * w.n_replicas)
+    if measures:
+        n_meas = (w.n_sweeps - w.n_sweeps // 2) // w.meas_every
+        n_terms = float(w.n_samples * world * n_meas * (w.n_replicas * (w.n_replicas - 1) // 2))
+        reduced = {"what": "[<q^2>] per slot over all ranks' samples, pairs and measurements (accumulator 1 / terms)",
+                   "per_slot": [float(x) / n_terms for x in sums[:, 1].tolist()]}
+    else:
+        reduced = {"what": "mean energy per spin (2U - 3N - hM)/N per slot over all ranks' samples and replicas",
+                   "per_slot": [float((2.0 * u / n_sys - 3.0 * w.N - w.h * m / n_sys) / w.N) for u, m in zip(sums[0].tolist(), sums[1].tolist())]}
 
     if rank == 0:
-        wordsites_per_sweep = w.N * w.n_words * w.n_replicas * w.n_temps if w.kind == W.PMJ else w.N * w.n_samples * w.n_replicas * w.n_temps
-        nominal = ALU_LANES_PER_SM * N_SM * pk["sm_max_mhz"] * 1e6 / 1e12       # T lane-ops / s
-        peak = alu_peak_measured
-        ach = ALU_OPS_PER_WORDSITE * wordsites_per_sweep * n_k / (sweep_ms * 1e-3) / 1e12
-        sweep_rate = w.flip_attempts(n_k) / (sweep_ms * 1e6)
-        launch_s = sweep_ms * 1e-3 / max(1, sweep_launches)
-        hbm_ach = HBM_BYTES_PER_WORDSITE_LAUNCH * wordsites_per_sweep / launch_s / 1e9 if w.kind == W.PMJ else None
-        roofline = {"bound": "alu", "kernel": "sweep (+-J multispin)", "achieved": ach, "peak": peak, "unit": "Tlaneop/s",
-                    "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(w.name),
-                    "peak_source": "measured in this run: dependency-free LOP3 micro-benchmark (csrc/probe/alu_probe.cu); "
-                                   "nominal 64 INT lanes/SM/clk x 148 SMs x %.0f MHz = %.2f" % (pk["sm_max_mhz"], nominal),
-                    "peak_nominal": nominal, "frac_of_nominal": ach / nominal,
-                    "alu_ops_per_wordsite": ALU_OPS_PER_WORDSITE, "launch_us": 1e6 * launch_s,
-                    "launches_timed": sweep_launches * reps, "sweeps_per_launch": n_k // max(1, sweep_launches),
-                    "sweep_only_flips_per_ns": sweep_rate,
-                    "share_of_step": (sweep_ms / n_k) * w.n_sweeps / (total_ms / args.steps),
-                    "hbm": {"achieved": hbm_ach, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                            "frac": (hbm_ach / pk["hbm_gbs"]) if hbm_ach else None,
-                            "note": "algorithmic 8 B per word-site per LAUNCH (state resident in shared memory for all "
-                                    "sweeps of a launch): HBM is not the binding roof, the ALU pipe is (DESIGN.md 6)"}}
-        if w.kind != W.PMJ:
-            roofline.update({"kernel": "sweep (Gaussian fp32)", "note": "no roofline target for the Gaussian path"})
+        ms_per_step = total_ms_max / args.steps
+        roofline = roofline_block(w, sweep_ms, n_k, sweep_launches, total_ms / args.steps, alu_peak_measured, pk)
         out = {"metric": "spin_flip_attempts_per_ns", "value": value, "unit": "flips/ns", "n_gpus": world,
-               "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps,
+               "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                "dtype": "u32" if w.kind == W.PMJ else "f32", "data": "synthetic",
                "config": workload_config(w, world), "clocks": sampler.result(),
-               "e2e": {"value": e2e_value, "unit": "flips/ns", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+               "e2e": {"value": e2e_value, "unit": "flips/ns", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                       "result": "moment accumulators" if measures else "per-system energies (U, M) of the final state"},
                "gpu_launches": int(launches), "roofline": roofline,
+               "pt": {"proposed": int(prop.sum()), "accepted": int(acc.sum()),
+                      "acceptance_per_pair": [round(float(a) / max(1.0, float(p)), 4) for p, a in zip(prop.tolist(), acc.tolist())]},
+               "reduced_over_ranks": reduced,
                "paper_context": "33 ps/attempt = 30.3 flips/ns on a GTX 580 (PAPER.md:68); other hardware, not a target"}
+        if world == 1 and not args.no_other_configs:
+            others = {}
+            del workspace
+            torch.cuda.empty_cache()
+            for name, sweeps in (("C2", 2048), ("C3", 1024), ("C4", 256)):
+                if name != w.name:
+                    others[name] = short_run(sg, torch, name, sweeps, dev, stream, flush, alu_peak_measured, pk)
+            out["other_configs"] = others
         if world == 1 and not args.no_cpu_baseline:
             cores = os.cpu_count() or 1
             threads = min(cores, 32)
-            per_sweep = w.N * w.n_replicas * w.n_temps * 40e-9
-            n_sw = int(max(32, min(w.n_sweeps, 45.0 / per_sweep)))        # ~10-20 s of CPU work (the oracle runs ~12 ns per attempt)
-            n_sw -= n_sw % 32
+            per_sweep = w.N * w.n_replicas * w.n_temps * 15e-9
+            n_sw = int(max(8, min(w.n_sweeps, 15.0 / per_sweep)))          # ~10-20 s of CPU work (the oracle runs ~12-15 ns per attempt)
+            q = max(1, 2 * max(w.meas_every, 1), 2 * w.pt_every)
+            n_sw = max(q, n_sw - n_sw % q)
             r, dt = oracle_rate(w, threads, n_sw, threads)
             out["cpu_baseline"] = {"value": r, "unit": "flips/ns", "cores": threads, "kind": "oracle",
                                    "sample": "%d samples x %d sweeps of %s (same PT / measurement cadence), %.1f s" % (
                                        threads, n_sw, w.name, dt)}
         print(json.dumps(out))
-    sim.close()
     if world > 1:
         dist.destroy_process_group()
 
@@ -344,10 +431,20 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2", choices=sorted(W.BY_NAME))
+    ap.add_argument("--workload", default="C5", choices=sorted(W.BY_NAME))
     ap.add_argument("--sweeps", type=int, default=0, help="override the workload's sweep count (debugging)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true")
     args = ap.parse_args()
+    world_env = os.environ.get("WORLD_SIZE")
+    if args.gpus > 1 and world_env is None:
+        # launched directly with --gpus N: re-run under torch.distributed.run, one rank per GPU
+        port = 29500 + os.getpid() % 2000
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
+    if world_env is not None and int(world_env) != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%s" % (args.gpus, world_env))
     w = W.BY_NAME[args.workload]
     if args.sweeps:
         w = w.scaled(n_sweeps=args.sweeps)

@@ -143,6 +143,11 @@ int upload_tables(sg_ctx *c)
         }
     }
     c->d.fast_accept = monotone ? 1 : 0;
+    bool below = monotone;                                  // binary-search compare (sg_accept.cuh): thr[c <= 6] < 2^32
+    for (int t = 0; t < NT && below; ++t)
+        for (int code = 0; code < 7; ++code)
+            if (c->thr[((size_t)t * 7 + (code >> 1)) * 2 + (1 - (code & 1))] >= 4294967296ULL) below = false;
+    c->d.bs_accept = below ? 1 : 0;
     std::vector<double> t64(DEXP64_N);
     std::vector<float> t32(DEXP32_N);
     for (int i = 0; i < DEXP64_N; ++i) t64[i] = exp(-(double)i / 256.0);
@@ -341,6 +346,7 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     d.k0 = (uint32_t)seed; d.k1 = (uint32_t)(seed >> 32);
     d.neg_h = h < 0.0 ? 1u : 0u;
     d.fast_accept = 0;
+    d.bs_accept = 0;
     d.s_first = 0;
     c->own_ws = workspace == nullptr;
     c->ws_bytes = lo.total;

@@ -22,6 +22,7 @@ struct Dims {
     uint32_t k0, k1;          // Philox key = (seed lo, seed hi)
     uint32_t neg_h;           // 1 if h < 0 (field alignment a = ~s)
     int fast_accept;          // |h| <= 1 and threshold table monotone: comparator path
+    int bs_accept;            // fast_accept and every threshold of the codes c <= 6 is < 2^32 (h != 0): binary-search compare
 };
 
 // Per-slot device tables (one struct array in the workspace).

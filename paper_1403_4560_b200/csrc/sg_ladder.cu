@@ -146,7 +146,7 @@ __device__ __forceinline__ void ladder_energy(const uint32_t *__restrict__ Ssys,
     M = 2 * (int)bs_warp_total(bigM, pm, lane) - N;
 }
 
-template <int L>
+template <int L, bool BS>
 __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const __grid_constant__ LadderArgs A)
 {
     using G_ = Geo<L>;
@@ -176,16 +176,17 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
         uint4 *jd = reinterpret_cast<uint4 *>(Jsm);
         for (int i = tid; i < 3 * N / 4; i += nthr) jd[i] = js[i];
         for (int t = tid; t < NT; t += nthr) {                 // acceptance constants (SlotK of sg_accept.cuh)
-            uint32_t lo[7], zc[7];
+            uint32_t lo[7], hi[7], kw[10];
             for (int c = 0; c < 7; ++c) {
-                const uint2 v = A.tab[t].c64[c];               // (0 - thr) as 64 bits: hi = 0 only for thr = 0
+                const uint2 v = A.tab[t].c64[c];               // (0 - thr) as 64 bits
                 lo[c] = v.x;
-                zc[c] = v.y == 0u ? 1u : 0u;
+                hi[c] = v.y;
             }
+            slotk_words<BS>(lo, hi, kw);
             uint4 *k4 = reinterpret_cast<uint4 *>(thr + t * 8);
-            k4[0] = make_uint4(lo[0], lo[1], lo[2], lo[3]);
-            k4[1] = make_uint4(lo[4], lo[5], lo[6], zc[3] - 1u);
-            k4[2] = make_uint4(zc[1] + zc[5] - 1u, zc[0] + zc[2] + zc[4] + zc[6] - 2u, 0u, 0u);
+            k4[0] = make_uint4(kw[0], kw[1], kw[2], kw[3]);
+            k4[1] = make_uint4(kw[4], kw[5], kw[6], kw[7]);
+            k4[2] = make_uint4(kw[8], kw[9], 0u, 0u);
         }
         for (int t = tid; t < NT; t += nthr) accs[t] = 0u;
     }
@@ -269,7 +270,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         uint32_t out[4];
 #pragma unroll
                         for (int e = 0; e < 4; ++e)
-                            out[e] = flip_word_k(s[e], amask, xor3(s[e], v0[e], JA[e]), xor3(s[e], os[e], JB[e]),
+                            out[e] = flip_word_k<BS>(s[e], amask, xor3(s[e], v0[e], JA[e]), xor3(s[e], os[e], JB[e]),
                                                  xor3(s[e], vyp[e], Jyp[e]), xor3(s[e], vym[e], Jym[e]),
                                                  xor3(s[e], vzp[e], Jzp[e]), xor3(s[e], vzm[e], Jzm[e]), rr[e], K, A.one,
                                                  A.mone);
@@ -343,7 +344,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         uint32_t out[4];
 #pragma unroll
                         for (int e = 0; e < 4; ++e)
-                            out[e] = flip_word_k(s[e], amask, xor3(s[e], v[e][0], Jq[e][0]), xor3(s[e], v[e][1], Jq[e][1]),
+                            out[e] = flip_word_k<BS>(s[e], amask, xor3(s[e], v[e][0], Jq[e][0]), xor3(s[e], v[e][1], Jq[e][1]),
                                                  xor3(s[e], v[e][2], Jq[e][2]), xor3(s[e], v[e][3], Jq[e][3]),
                                                  xor3(s[e], v[e][4], Jq[e][4]), xor3(s[e], v[e][5], Jq[e][5]), rr[e], K, A.one,
                                                  A.mone);
@@ -441,10 +442,13 @@ template <int L>
 static cudaError_t launch_l(sg_ctx *c, const LadderArgs &A, int threads, size_t smem, cudaStream_t st, int grid)
 {
     if (attr_needed(c, ATTR_LADDER + L / 2 - 2)) {       // L = 4..16 -> ids 1..7
-        cudaError_t e = cudaFuncSetAttribute(k_ladder_pmj<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(k_ladder_pmj<L, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(k_ladder_pmj<L, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
     }
-    k_ladder_pmj<L><<<grid, threads, smem, st>>>(A);
+    if (A.d.bs_accept) k_ladder_pmj<L, true><<<grid, threads, smem, st>>>(A);
+    else k_ladder_pmj<L, false><<<grid, threads, smem, st>>>(A);
     return cudaGetLastError();
 }
 

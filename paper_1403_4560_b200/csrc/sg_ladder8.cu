@@ -78,7 +78,7 @@ __device__ __forceinline__ void reduce4(const uint32_t *__restrict__ in, uint32_
     }
 }
 
-template <int P, bool ENERGY>
+template <int P, bool ENERGY, bool BS>
 __device__ __forceinline__ void half_sweep_quad(uint32_t *__restrict__ Sa, const uint32_t *__restrict__ So, int slot,
                                                 int s_yp, int s_ym, int s_zp, int s_zm, const uint32_t (&JA)[4],
                                                 const uint32_t (&JB)[4], const uint32_t (&Jyp)[4],
@@ -112,10 +112,10 @@ __device__ __forceinline__ void half_sweep_quad(uint32_t *__restrict__ Sa, const
         const uint32_t u0 = xor3(s[e], v0[e], JA[e]), u1 = xor3(s[e], vB[e], JB[e]), u2 = xor3(s[e], vyp[e], Jyp[e]);
         const uint32_t u3 = xor3(s[e], vym[e], Jym[e]), u4 = xor3(s[e], vzp[e], Jzp[e]), u5 = xor3(s[e], vzm[e], Jzm[e]);
         if (!ENERGY) {
-            out[e] = flip_word_k(s[e], amask, u0, u1, u2, u3, u4, u5, rr[e], K, one, mone);
+            out[e] = flip_word_k<BS>(s[e], amask, u0, u1, u2, u3, u4, u5, rr[e], K, one, mone);
         } else {
             uint32_t n0, n1, n2;
-            const uint32_t acc = accept_word(u0, u1, u2, u3, u4, u5, ~(s[e] ^ amask), rr[e], K, one, mone, n0, n1, n2);
+            const uint32_t acc = accept_word<BS>(u0, u1, u2, u3, u4, u5, ~(s[e] ^ amask), rr[e], K, one, mone, n0, n1, n2);
             out[e] = s[e] ^ acc;
             // post-flip unsatisfied count of this site: n if not flipped, 6 - n if flipped
             // 6 - n: bit0 = n0; bit1 = 1 for n in {0,3,4}; bit2 = 1 for n in {0,1,2}
@@ -151,7 +151,7 @@ __device__ __forceinline__ void half_sweep_quad(uint32_t *__restrict__ Sa, const
 }
 
 // SPT = systems per thread (NT / G) when it is a compile-time constant (unrolled), 0 = run-time loop
-template <int SPT>
+template <int SPT, bool BS>
 __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ Ladder8Args A)
 {
     constexpr int N = 512, H = 256;
@@ -186,15 +186,16 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
         reinterpret_cast<uint4 *>(Jsm)[cd * 64 + slot_of_row(qq & 7, qq >> 3)] = reinterpret_cast<const uint4 *>(gJ)[i];
     }
     for (int t = tid; t < NT; t += nthr) {                 // acceptance constants (see SlotK)
-        uint32_t lo[7], zc[7];
+        uint32_t lo[7], hi[7], kw[10];
         for (int c = 0; c < 7; ++c) {
-            const uint2 v = A.tab[t].c64[c];               // (0 - thr) as 64 bits: hi = 0 only for thr = 0
+            const uint2 v = A.tab[t].c64[c];               // (0 - thr) as 64 bits
             lo[c] = v.x;
-            zc[c] = v.y == 0u ? 1u : 0u;
+            hi[c] = v.y;
         }
-        thr[t * 3 + 0] = make_uint4(lo[0], lo[1], lo[2], lo[3]);
-        thr[t * 3 + 1] = make_uint4(lo[4], lo[5], lo[6], zc[3] - 1u);
-        thr[t * 3 + 2] = make_uint4(zc[1] + zc[5] - 1u, zc[0] + zc[2] + zc[4] + zc[6] - 2u, 0u, 0u);
+        slotk_words<BS>(lo, hi, kw);
+        thr[t * 3 + 0] = make_uint4(kw[0], kw[1], kw[2], kw[3]);
+        thr[t * 3 + 1] = make_uint4(kw[4], kw[5], kw[6], kw[7]);
+        thr[t * 3 + 2] = make_uint4(kw[8], kw[9], 0u, 0u);
     }
     if (tid < MAX_NT) accs[tid] = 0u;
     __syncthreads();
@@ -248,14 +249,14 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
                     uint32_t *red = red0 + (size_t)t * PW1 * 64 + (pi * 32 + j);
                     const uint4 *kt = thr + t * 3;
                     if (want_energy) {
-                        if (p) half_sweep_quad<1, true>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
+                        if (p) half_sweep_quad<1, true, BS>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
                                                         r_cur, kt, amask, A.one, A.mone, red);
-                        else   half_sweep_quad<0, true>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
+                        else   half_sweep_quad<0, true, BS>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
                                                         r_cur, kt, amask, A.one, A.mone, red);
                     } else {
-                        if (p) half_sweep_quad<1, false>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
+                        if (p) half_sweep_quad<1, false, BS>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
                                                          r_cur, kt, amask, A.one, A.mone, red);
-                        else   half_sweep_quad<0, false>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
+                        else   half_sweep_quad<0, false, BS>(Sa, So, slot, s_yp, s_ym, s_zp, s_zm, JA, JB, Jyp, Jym, Jzp, Jzm,
                                                          r_cur, kt, amask, A.one, A.mone, red);
                     }
                 };
@@ -374,11 +375,11 @@ bool ladder8_supported(const sg_ctx *c)
 int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_sweeps, int pt_every)
 {
     if (attr_needed(c, ATTR_LADDER8)) {
-        if (cudaFuncSetAttribute(k_ladder8_pmj<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess ||
-            cudaFuncSetAttribute(k_ladder8_pmj<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess ||
-            cudaFuncSetAttribute(k_ladder8_pmj<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess ||
-            cudaFuncSetAttribute(k_ladder8_pmj<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) != cudaSuccess)
-            return -1;
+        bool ok = true;
+        auto set = [&](auto kern) { ok = ok && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) == cudaSuccess; };
+        set(k_ladder8_pmj<0, false>); set(k_ladder8_pmj<1, false>); set(k_ladder8_pmj<2, false>); set(k_ladder8_pmj<4, false>);
+        set(k_ladder8_pmj<0, true>); set(k_ladder8_pmj<1, true>); set(k_ladder8_pmj<2, true>); set(k_ladder8_pmj<4, true>);
+        if (!ok) return -1;
     }
     const Dims &d = c->d;
     Ladder8Args A;
@@ -409,10 +410,18 @@ int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_swe
     A.pt_acc = c->pt_acc;
     const size_t smem = ladder8_smem(d.NT, pt_every > 0);
     const int spt = d.NT % G == 0 ? d.NT / G : 0;
-    if (spt == 4) k_ladder8_pmj<4><<<d.W * d.R, threads, smem, c->stream>>>(A);
-    else if (spt == 2) k_ladder8_pmj<2><<<d.W * d.R, threads, smem, c->stream>>>(A);
-    else if (spt == 1) k_ladder8_pmj<1><<<d.W * d.R, threads, smem, c->stream>>>(A);
-    else k_ladder8_pmj<0><<<d.W * d.R, threads, smem, c->stream>>>(A);
+    const int grid = d.W * d.R;
+    if (d.bs_accept) {
+        if (spt == 4) k_ladder8_pmj<4, true><<<grid, threads, smem, c->stream>>>(A);
+        else if (spt == 2) k_ladder8_pmj<2, true><<<grid, threads, smem, c->stream>>>(A);
+        else if (spt == 1) k_ladder8_pmj<1, true><<<grid, threads, smem, c->stream>>>(A);
+        else k_ladder8_pmj<0, true><<<grid, threads, smem, c->stream>>>(A);
+    } else {
+        if (spt == 4) k_ladder8_pmj<4, false><<<grid, threads, smem, c->stream>>>(A);
+        else if (spt == 2) k_ladder8_pmj<2, false><<<grid, threads, smem, c->stream>>>(A);
+        else if (spt == 1) k_ladder8_pmj<1, false><<<grid, threads, smem, c->stream>>>(A);
+        else k_ladder8_pmj<0, false><<<grid, threads, smem, c->stream>>>(A);
+    }
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

@@ -133,7 +133,7 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void *src, uint32_
 }
 
 // sa / so: byte addresses of the own-colour / other-colour array; qb: byte offset of the quad in them
-template <int P, bool ENERGY>
+template <int P, bool ENERGY, bool BS>
 __device__ __forceinline__ void quad_update(uint32_t sa, uint32_t so, uint32_t qb, const Geo32 &g, const Quad6 &Jq,
                                             const uint4 r4, const SlotK &K, uint32_t amask, uint32_t one, uint32_t mone,
                                             int lane, uint32_t (&accU)[8], uint32_t (&accM)[7])
@@ -163,10 +163,10 @@ __device__ __forceinline__ void quad_update(uint32_t sa, uint32_t so, uint32_t q
         const uint32_t u0 = xor3(s[e], v0[e], JA[e]), u1 = xor3(s[e], vB[e], JB[e]), u2 = xor3(s[e], vyp[e], Jyp[e]);
         const uint32_t u3 = xor3(s[e], vym[e], Jym[e]), u4 = xor3(s[e], vzp[e], Jzp[e]), u5 = xor3(s[e], vzm[e], Jzm[e]);
         if (!ENERGY) {
-            out[e] = flip_word_k(s[e], amask, u0, u1, u2, u3, u4, u5, rr[e], K, one, mone);
+            out[e] = flip_word_k<BS>(s[e], amask, u0, u1, u2, u3, u4, u5, rr[e], K, one, mone);
         } else {
             uint32_t n0, n1, n2;
-            const uint32_t acc = accept_word(u0, u1, u2, u3, u4, u5, ~(s[e] ^ amask), rr[e], K, one, mone, n0, n1, n2);
+            const uint32_t acc = accept_word<BS>(u0, u1, u2, u3, u4, u5, ~(s[e] ^ amask), rr[e], K, one, mone, n0, n1, n2);
             out[e] = s[e] ^ acc;
             // post-flip unsatisfied count: n if not flipped, 6 - n if flipped
             // 6 - n: bit0 = n0; bit1 = 1 for n in {0,3,4}; bit2 = 1 for n in {0,1,2}
@@ -196,6 +196,7 @@ __device__ __forceinline__ void quad_update(uint32_t sa, uint32_t so, uint32_t q
     }
 }
 
+template <bool BS>
 __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constant__ Res32Args A)
 {
     extern __shared__ __align__(128) uint32_t smem[];
@@ -323,7 +324,7 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
             Jq.zp = lds128(jc + 2048);
             Jq.zm = lds128(jc + 2560);
             const uint32_t qb = geo.tb + 4096u * (uint32_t)(2 * it + zhalf);
-            quad_update<P, ENERGY>(sa, so, qb, geo, Jq, philox_rk8(qb >> 4, time, wglob, c3, A.rk), K, amask, A.one,
+            quad_update<P, ENERGY, BS>(sa, so, qb, geo, Jq, philox_rk8(qb >> 4, time, wglob, c3, A.rk), K, amask, A.one,
                                    A.mone, lane, accU, accM);
             // Refill the stage two steps ahead only now: every lane has CONSUMED its coupling registers, so the
             // shared-memory loads of the stage have completed (a load that is merely issued could still be in the
@@ -429,7 +430,8 @@ int launch_pack_J_res32(sg_ctx *c)
 int launch_res32_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, bool want_energy, bool do_exchange, uint64_t exchange)
 {
     if (attr_needed(c, ATTR_RES32)) {
-        if (cudaFuncSetAttribute(k_res32_pmj, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RES32_SMEM) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_res32_pmj<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RES32_SMEM) != cudaSuccess ||
+            cudaFuncSetAttribute(k_res32_pmj<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RES32_SMEM) != cudaSuccess)
             return -1;
     }
     const Dims &d = c->d;
@@ -458,17 +460,17 @@ int launch_res32_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, bool want_energy,
     A.one = 1u;
     A.mone = 0xffffffffu;
     for (int t = 0; t < d.NT; ++t) {                        // SlotK of sg_accept.cuh from the host threshold table
-        uint32_t zc[7];
+        uint32_t lo[7], hi[7];
         for (int code = 0; code < 7; ++code) {
-            const uint64_t th = c->thr[((size_t)t * 7 + (code >> 1)) * 2 + (1 - (code & 1))];
-            A.kc[t][code] = (uint32_t)((uint64_t)0 - th);
-            zc[code] = th == 0 ? 1u : 0u;
+            const uint64_t neg = (uint64_t)0 - c->thr[((size_t)t * 7 + (code >> 1)) * 2 + (1 - (code & 1))];
+            lo[code] = (uint32_t)neg;
+            hi[code] = (uint32_t)(neg >> 32);
         }
-        A.kc[t][7] = zc[3] - 1u;
-        A.kc[t][8] = zc[1] + zc[5] - 1u;
-        A.kc[t][9] = zc[0] + zc[2] + zc[4] + zc[6] - 2u;
+        if (d.bs_accept) slotk_words<true>(lo, hi, A.kc[t]);
+        else slotk_words<false>(lo, hi, A.kc[t]);
     }
-    k_res32_pmj<<<dim3(d.NT, d.R, d.W), R_THREADS, RES32_SMEM, c->stream>>>(A);
+    if (d.bs_accept) k_res32_pmj<true><<<dim3(d.NT, d.R, d.W), R_THREADS, RES32_SMEM, c->stream>>>(A);
+    else k_res32_pmj<false><<<dim3(d.NT, d.R, d.W), R_THREADS, RES32_SMEM, c->stream>>>(A);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

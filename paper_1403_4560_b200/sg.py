@@ -183,6 +183,10 @@ class Simulation:
         self._check(_lib.sg_get_energies_cached(self._h, _p(U), _p(M)))
         return U, M
 
+    def sg_get_energies_cached_into(self, U, M):
+        """Fill caller-owned (e.g. pinned) int64 / int32 host arrays of shape [n_samples][R][NT]."""
+        self._check(_lib.sg_get_energies_cached(self._h, C.c_void_p(U.ctypes.data), C.c_void_p(M.ctypes.data)))
+
     def sg_set_kernel_path(self, path):
         self._check(_lib.sg_set_kernel_path(self._h, int(path)))
 
