@@ -231,6 +231,12 @@ typedef struct ea_oracle {
     double t64[DEXP64_N];
     float t32[DEXP32_N];
     uint64_t n_pt_prop, n_pt_acc;
+    /* diagnostics ("logarithm binning test", "distribution of the overlap parameter") */
+    int pq_bins;            /* 0 = off */
+    uint64_t *pq;           /* [NT][pq_bins] counts of the overlap q_ab(0), all pairs, all measurements */
+    int n_windows;          /* 0 = off */
+    double *accw;           /* [n_windows][NT][EA_NMOM]: the accumulators of R9 per window [2^k, 2^(k+1)) of the sweep counter */
+    int64_t *n_meas_w;      /* [n_windows] */
 } ea_oracle;
 
 static const int KVEC[EA_NK][3] = {      /* in units of (2pi/Lx, 2pi/Ly, 2pi/Lz); R8 */
@@ -271,6 +277,7 @@ void ea_destroy(ea_oracle *o)
     free(o->T); free(o->beta); free(o->beta_f); free(o->thr); free(o->nbr); free(o->colour);
     free(o->Jpm); free(o->Jg); free(o->Jfix); free(o->S); free(o->U); free(o->M);
     free(o->acc); free(o->ck); free(o->sk);
+    free(o->pq); free(o->accw); free(o->n_meas_w);
     free(o);
 }
 
@@ -481,6 +488,35 @@ void ea_pt_exchange(ea_oracle *o)
 
 int ea_n_pairs(const ea_oracle *o) { return o->R * (o->R - 1) / 2; }
 
+/* accumulators, R9 (one measurement of one slot added to A[EA_NMOM]):
+ * [0..3]  sum over pairs of q, q^2, q^3, q^4  (q = q_ab(0))           -> Eq. 3
+ * [4+5k+0..2] sum over pairs of Re q(Kk), Im q(Kk), |q(Kk)|^2          -> Eq. 4
+ * [4+5k+3] sum over the unordered couples of pairs sharing exactly one replica of Re(q_p conj q_p')
+ * [4+5k+4] sum over the disjoint pair-couples of Re(q_p conj q_p')
+ * [64],[65] the same two cross sums for k = 0 */
+static void add_moments(double *A, double rec[6][EA_REC], const int *pa, const int *pb, int P)
+{
+    for (int q = 0; q < P; ++q) {
+        double v = rec[q][0];
+        A[0] += v; A[1] += v * v; A[2] += v * v * v; A[3] += (v * v) * (v * v);
+        for (int k = 0; k < EA_NK; ++k) {
+            double re = rec[q][1 + 2 * k], im = rec[q][2 + 2 * k];
+            A[4 + 5 * k + 0] += re;
+            A[4 + 5 * k + 1] += im;
+            A[4 + 5 * k + 2] += re * re + im * im;
+        }
+    }
+    for (int q = 0; q < P; ++q)
+        for (int q2 = q + 1; q2 < P; ++q2) {
+            int shared = (pa[q] == pa[q2]) + (pa[q] == pb[q2]) + (pb[q] == pa[q2]) + (pb[q] == pb[q2]);
+            int slot = shared == 1 ? 3 : 4;
+            A[slot == 3 ? 64 : 65] += rec[q][0] * rec[q2][0];
+            for (int k = 0; k < EA_NK; ++k)
+                A[4 + 5 * k + slot] += rec[q][1 + 2 * k] * rec[q2][1 + 2 * k] +
+                                       rec[q][2 + 2 * k] * rec[q2][2 + 2 * k];
+        }
+}
+
 /* overlaps of all replica pairs at every slot: literal Eq. 2
  * out (may be NULL): [NT][n_pairs][25] = q(0), Re q(K0), Im q(K0), ..., Re q(K11), Im q(K11);
  * pair order (0,1),(0,2),(0,3),(1,2),(1,3),(2,3).  Always adds to the accumulators (R9). */
@@ -515,32 +551,32 @@ void ea_measure(ea_oracle *o, double *out)
             for (int q = 0; q < P; ++q)
                 memcpy(out + ((size_t)t * P + q) * EA_REC, rec[q], sizeof(double) * EA_REC);
 
-        /* accumulators, R9:
-         * [0..3]  sum over pairs of q, q^2, q^3, q^4  (q = q_ab(0))           -> Eq. 3
-         * [4+5k+0..2] sum over pairs of Re q(Kk), Im q(Kk), |q(Kk)|^2          -> Eq. 4
-         * [4+5k+3] sum over the unordered couples of pairs sharing exactly one replica of Re(q_p conj q_p')
-         * [4+5k+4] sum over the disjoint pair-couples of Re(q_p conj q_p')
-         * [64],[65] the same two cross sums for k = 0 */
-        double *A = o->acc + (size_t)t * EA_NMOM;
-        for (int q = 0; q < P; ++q) {
-            double v = rec[q][0];
-            A[0] += v; A[1] += v * v; A[2] += v * v * v; A[3] += (v * v) * (v * v);
-            for (int k = 0; k < EA_NK; ++k) {
-                double re = rec[q][1 + 2 * k], im = rec[q][2 + 2 * k];
-                A[4 + 5 * k + 0] += re;
-                A[4 + 5 * k + 1] += im;
-                A[4 + 5 * k + 2] += re * re + im * im;
-            }
+        /* P(q): the integer overlap Q = sum_j S^a_j S^b_j = N q_ab(0) takes the N + 1 values -N, -N+2, ..., N;
+         * idx = (Q + N)/2 = number of agreeing sites in 0..N; bin = floor(idx * pq_bins / (N + 1)) */
+        if (o->pq_bins > 0) {
+            int pp = 0;
+            for (int a = 0; a < R; ++a)
+                for (int b = a + 1; b < R; ++b) {
+                    if (pp >= 6) break;
+                    const int *Sa = Sys(o, a, t), *Sb = Sys(o, b, t);
+                    int64_t agree = 0;
+                    for (int j = 0; j < N; ++j) if (Sa[j] == Sb[j]) ++agree;
+                    o->pq[(size_t)t * o->pq_bins + (size_t)((agree * (int64_t)o->pq_bins) / ((int64_t)N + 1))] += 1;
+                    ++pp;
+                }
         }
-        for (int q = 0; q < P; ++q)
-            for (int q2 = q + 1; q2 < P; ++q2) {
-                int shared = (pa[q] == pa[q2]) + (pa[q] == pb[q2]) + (pb[q] == pa[q2]) + (pb[q] == pb[q2]);
-                int slot = shared == 1 ? 3 : 4;
-                A[slot == 3 ? 64 : 65] += rec[q][0] * rec[q2][0];
-                for (int k = 0; k < EA_NK; ++k)
-                    A[4 + 5 * k + slot] += rec[q][1 + 2 * k] * rec[q2][1 + 2 * k] +
-                                           rec[q][2 + 2 * k] * rec[q2][2 + 2 * k];
-            }
+        /* logarithmic binning: a measurement taken when the sweep counter is s >= 1 also goes to the
+         * window k = min(floor(log2 s), n_windows - 1), i.e. s in [2^k, 2^(k+1)) */
+        double *AW = NULL;
+        if (o->n_windows > 0 && o->sweeps >= 1) {
+            int k = 0;
+            while ((o->sweeps >> (k + 1)) != 0) ++k;
+            if (k > o->n_windows - 1) k = o->n_windows - 1;
+            AW = o->accw + ((size_t)k * o->NT + t) * EA_NMOM;
+            if (t == 0) o->n_meas_w[k] += 1;
+        }
+        add_moments(o->acc + (size_t)t * EA_NMOM, rec, pa, pb, P);
+        if (AW) add_moments(AW, rec, pa, pb, P);
     }
     o->n_meas += 1;
 }
@@ -618,6 +654,34 @@ void ea_get_counters(const ea_oracle *o, uint64_t *sweeps, uint64_t *exchanges)
 {
     if (sweeps) *sweeps = o->sweeps;
     if (exchanges) *exchanges = o->exchanges;
+}
+/* diagnostics: switch on the P(q) histogram with n_bins bins (1 <= n_bins <= N + 1; N + 1 = one bin per value of q) */
+int ea_enable_pq(ea_oracle *o, int n_bins)
+{
+    if (n_bins < 1 || n_bins > o->N + 1) return -1;
+    free(o->pq);
+    o->pq = (uint64_t *)calloc((size_t)o->NT * n_bins, sizeof(uint64_t));
+    o->pq_bins = o->pq ? n_bins : 0;
+    return o->pq ? 0 : -1;
+}
+void ea_get_pq(const ea_oracle *o, uint64_t *out)          /* [NT][pq_bins] */
+{
+    memcpy(out, o->pq, sizeof(uint64_t) * (size_t)o->NT * o->pq_bins);
+}
+/* diagnostics: switch on the per-window accumulators of the logarithmic-binning test */
+int ea_enable_log_binning(ea_oracle *o, int n_windows)
+{
+    if (n_windows < 1 || n_windows > 40) return -1;
+    free(o->accw); free(o->n_meas_w);
+    o->accw = (double *)calloc((size_t)n_windows * o->NT * EA_NMOM, sizeof(double));
+    o->n_meas_w = (int64_t *)calloc((size_t)n_windows, sizeof(int64_t));
+    o->n_windows = (o->accw && o->n_meas_w) ? n_windows : 0;
+    return o->n_windows ? 0 : -1;
+}
+void ea_get_window_moments(const ea_oracle *o, int k, double *out, int64_t *n_meas)   /* [NT][66] of window k */
+{
+    memcpy(out, o->accw + (size_t)k * o->NT * EA_NMOM, sizeof(double) * o->NT * EA_NMOM);
+    if (n_meas) *n_meas = o->n_meas_w[k];
 }
 void ea_get_pt_stats(const ea_oracle *o, uint64_t *proposed, uint64_t *accepted)
 {

@@ -45,6 +45,10 @@ def lib():
             ("ea_get_moments", [vp, vp, vp], None),
             ("ea_get_counters", [vp, vp, vp], None),
             ("ea_get_pt_stats", [vp, vp, vp], None),
+            ("ea_enable_pq", [vp, i32], i32),
+            ("ea_get_pq", [vp, vp], None),
+            ("ea_enable_log_binning", [vp, i32], i32),
+            ("ea_get_window_moments", [vp, i32, vp, vp], None),
             ("ea_philox4x32_10", [vp, vp, vp], None),
             ("ea_dlog", [dbl], dbl),
             ("ea_dsincos2pi", [dbl, vp, vp], None),
@@ -195,6 +199,27 @@ class Oracle:
         a, b = C.c_uint64(), C.c_uint64()
         lib().ea_get_counters(self._h, C.byref(a), C.byref(b))
         return a.value, b.value
+
+    def enable_pq(self, n_bins=None):
+        self.pq_bins = self.N + 1 if n_bins is None else int(n_bins)
+        if lib().ea_enable_pq(self._h, self.pq_bins) != 0:
+            raise ValueError("ea_enable_pq rejected n_bins")
+
+    def pq(self):
+        out = np.zeros((self.NT, self.pq_bins), dtype=np.uint64)
+        lib().ea_get_pq(self._h, _p(out))
+        return out
+
+    def enable_log_binning(self, n_windows):
+        self.n_windows = int(n_windows)
+        if lib().ea_enable_log_binning(self._h, self.n_windows) != 0:
+            raise ValueError("ea_enable_log_binning rejected n_windows")
+
+    def window_moments(self, k):
+        out = np.zeros((self.NT, NMOM), dtype=np.float64)
+        n = C.c_int64()
+        lib().ea_get_window_moments(self._h, int(k), _p(out), C.byref(n))
+        return out, n.value
 
     def pt_stats(self):
         a, b = C.c_uint64(), C.c_uint64()
