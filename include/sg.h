@@ -166,6 +166,27 @@ int sg_get_energies_cached(sg_ctx *ctx, int64_t *U, int32_t *M);
  * HOST ptrs to n_temps-1 values each; either may be NULL.  Synchronous. */
 int sg_get_pt_stats(sg_ctx *ctx, uint64_t *proposed, uint64_t *accepted);
 
+/* ---- diagnostics: device-side accumulators, switched on per context ---- */
+
+/* Overlap distribution P(q): from now on every measurement also counts, per (sample, slot), the
+ * overlap of every replica pair in a histogram of n_bins bins, 1 <= n_bins <= N + 1.  The integer overlap
+ * Q = sum_j S^a_j S^b_j = N q_ab(0) takes N + 1 values; with `agree` = (Q + N) / 2 agreeing sites the bin is
+ * floor(agree * n_bins / (N + 1)) (n_bins = N + 1: one bin per value).  The library allocates
+ * n_samples * n_temps * n_bins uint32 counters (freed by sg_destroy; zeroed by sg_reset).
+ * Errors: SG_EINVAL (n_bins out of range), SG_ENOMEM. */
+int sg_enable_pq(sg_ctx *ctx, int n_bins);
+/* out: HOST ptr, [n_samples][n_temps][n_bins] uint32.  SG_ESTATE if sg_enable_pq was not called.  Synchronous. */
+int sg_get_pq(sg_ctx *ctx, uint32_t *out);
+
+/* Logarithmic-binning equilibration test (Fig. 5 caption): from now on a measurement taken when the
+ * global sweep counter is s >= 1 also adds its moments (R9) to the accumulators of window
+ * k = min(floor(log2 s), n_windows - 1), i.e. s in [2^k, 2^(k+1)).  1 <= n_windows <= 40.  The library allocates
+ * n_windows * n_samples * n_temps * SG_NMOM doubles (freed by sg_destroy; zeroed by sg_reset). */
+int sg_enable_log_binning(sg_ctx *ctx, int n_windows);
+/* Window k: out HOST ptr [n_samples][n_temps][SG_NMOM] (may be NULL), n_meas = measurements that fell into the window
+ * (may be NULL).  SG_ESTATE if not enabled, SG_EINVAL if k is out of range.  Synchronous. */
+int sg_get_window_moments(sg_ctx *ctx, int k, double *out, int64_t *n_meas);
+
 /* Description of the last error of this context (or of the last failed sg_create if ctx is NULL).
  * The string is owned by the library and valid until the next call on the same context. */
 const char *sg_last_error(sg_ctx *ctx);

@@ -175,6 +175,9 @@ int do_reset(sg_ctx *c)
     int rc;
     if ((rc = check_cuda(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * (size_t)d.n_samples * d.NT * SG_NMOM, c->stream), "zero acc"))) return rc;
     if ((rc = check_cuda(c, cudaMemsetAsync(c->pt_acc, 0, sizeof(unsigned long long) * MAX_NT, c->stream), "zero pt counters"))) return rc;
+    if (c->pq && (rc = check_cuda(c, cudaMemsetAsync(c->pq, 0, sizeof(uint32_t) * (size_t)d.n_samples * d.NT * c->pq_bins, c->stream), "zero P(q)"))) return rc;
+    if (c->acc_win && (rc = check_cuda(c, cudaMemsetAsync(c->acc_win, 0, sizeof(double) * (size_t)c->n_windows * d.n_samples * d.NT * SG_NMOM, c->stream), "zero windows"))) return rc;
+    std::fill(c->n_meas_win.begin(), c->n_meas_win.end(), 0);
     c->launches += c->kind == SG_PMJ ? launch_init_pmj(c) : launch_init_gauss(c);
     if (c->Jp) c->launches += launch_pack_J_res32(c);
     c->sweeps = c->exchanges = 0;
@@ -237,6 +240,11 @@ int do_measure(sg_ctx *c, double *out)
         }
     }
     c->n_meas += 1;
+    if (c->acc_win && c->sweeps >= 1) {                  // the window meas_out() selected
+        int k = 0;
+        while ((c->sweeps >> (k + 1)) != 0) ++k;
+        c->n_meas_win[std::min(k, c->n_windows - 1)] += 1;
+    }
     return SG_OK;
 }
 
@@ -335,6 +343,10 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     c->sweeps = c->exchanges = c->launches = 0;
     c->n_meas = 0;
     c->path = SG_PATH_AUTO;
+    c->pq = nullptr;
+    c->pq_bins = 0;
+    c->acc_win = nullptr;
+    c->n_windows = 0;
     c->um_fresh = false;
     c->pending_exchange = false;
     c->attr_done = 0;
@@ -490,6 +502,8 @@ int sg_destroy(sg_ctx *c)
     if (!c) return SG_EINVAL;
     cudaStreamSynchronize(c->stream);
     if (c->own_ws) cudaFree(c->ws);
+    if (c->pq) cudaFree(c->pq);
+    if (c->acc_win) cudaFree(c->acc_win);
     delete c;
     return SG_OK;
 }
@@ -637,6 +651,62 @@ int sg_get_moments(sg_ctx *c, double *out, int64_t *n_meas)
         if ((rc = check_cuda(c, cudaStreamSynchronize(c->stream), "sync moments"))) return rc;
     }
     if (n_meas) *n_meas = c->n_meas;
+    return SG_OK;
+}
+
+int sg_enable_pq(sg_ctx *c, int n_bins)
+{
+    if (!c) return SG_EINVAL;
+    if (n_bins < 1 || n_bins > c->d.N + 1) return fail(c, SG_EINVAL, "sg_enable_pq: need 1 <= n_bins <= N + 1");
+    int rc;
+    if ((rc = check_cuda(c, cudaStreamSynchronize(c->stream), "sg_enable_pq sync"))) return rc;
+    if (c->pq) cudaFree(c->pq);
+    c->pq = nullptr;
+    c->pq_bins = 0;
+    const size_t bytes = sizeof(uint32_t) * (size_t)c->d.n_samples * c->d.NT * n_bins;
+    if (cudaMalloc(&c->pq, bytes) != cudaSuccess) { cudaGetLastError(); c->pq = nullptr; return fail(c, SG_ENOMEM, "sg_enable_pq: cudaMalloc failed"); }
+    c->pq_bins = n_bins;
+    return check_cuda(c, cudaMemsetAsync(c->pq, 0, bytes, c->stream), "zero P(q)");
+}
+
+int sg_get_pq(sg_ctx *c, uint32_t *out)
+{
+    if (!c || !out) return SG_EINVAL;
+    if (!c->pq) return fail(c, SG_ESTATE, "sg_get_pq: sg_enable_pq was not called");
+    int rc;
+    const size_t bytes = sizeof(uint32_t) * (size_t)c->d.n_samples * c->d.NT * c->pq_bins;
+    if ((rc = check_cuda(c, cudaMemcpyAsync(out, c->pq, bytes, cudaMemcpyDeviceToHost, c->stream), "copy P(q)"))) return rc;
+    return check_cuda(c, cudaStreamSynchronize(c->stream), "sync P(q)");
+}
+
+int sg_enable_log_binning(sg_ctx *c, int n_windows)
+{
+    if (!c) return SG_EINVAL;
+    if (n_windows < 1 || n_windows > 40) return fail(c, SG_EINVAL, "sg_enable_log_binning: need 1 <= n_windows <= 40");
+    int rc;
+    if ((rc = check_cuda(c, cudaStreamSynchronize(c->stream), "sg_enable_log_binning sync"))) return rc;
+    if (c->acc_win) cudaFree(c->acc_win);
+    c->acc_win = nullptr;
+    c->n_windows = 0;
+    const size_t bytes = sizeof(double) * (size_t)n_windows * c->d.n_samples * c->d.NT * SG_NMOM;
+    if (cudaMalloc(&c->acc_win, bytes) != cudaSuccess) { cudaGetLastError(); c->acc_win = nullptr; return fail(c, SG_ENOMEM, "sg_enable_log_binning: cudaMalloc failed"); }
+    c->n_windows = n_windows;
+    c->n_meas_win.assign(n_windows, 0);
+    return check_cuda(c, cudaMemsetAsync(c->acc_win, 0, bytes, c->stream), "zero windows");
+}
+
+int sg_get_window_moments(sg_ctx *c, int k, double *out, int64_t *n_meas)
+{
+    if (!c) return SG_EINVAL;
+    if (!c->acc_win) return fail(c, SG_ESTATE, "sg_get_window_moments: sg_enable_log_binning was not called");
+    if (k < 0 || k >= c->n_windows) return fail(c, SG_EINVAL, "sg_get_window_moments: window out of range");
+    if (out) {
+        const size_t n = (size_t)c->d.n_samples * c->d.NT * SG_NMOM;
+        int rc;
+        if ((rc = check_cuda(c, cudaMemcpyAsync(out, c->acc_win + (size_t)k * n, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream), "copy window"))) return rc;
+        if ((rc = check_cuda(c, cudaStreamSynchronize(c->stream), "sync window"))) return rc;
+    }
+    if (n_meas) *n_meas = c->n_meas_win[k];
     return SG_OK;
 }
 

@@ -25,6 +25,17 @@ struct Dims {
     int bs_accept;            // fast_accept and every threshold of the codes c <= 6 is < 2^32 (h != 0): binary-search compare
 };
 
+// Where a measurement kernel adds its results (R9 + the diagnostics of SURVEY.md 8f rank 4).
+struct MeasOut {
+    double *acc;              // [n_samples][NT][SG_NMOM] total accumulators
+    double *acc_win;          // the same for the current window of the logarithmic-binning test, or NULL
+    uint32_t *pq;             // [n_samples][NT][pq_bins] counts of the integer overlap, or NULL
+    int pq_bins;
+};
+
+// bin of the overlap histogram for `agree` agreeing sites of N (sg_enable_pq): floor(agree * bins / (N + 1))
+__host__ __device__ inline int pq_bin(int agree, int N, int bins) { return (int)(((long long)agree * bins) / ((long long)N + 1)); }
+
 // Per-slot device tables (one struct array in the workspace).
 struct SlotTab {
     // PMJ fast path: c64[c] = (uint64)(0 - thr(code c)), code c = 2 n_u + (1 - a), c = 0..6
@@ -77,6 +88,12 @@ struct sg_ctx {
     uint64_t *hashes;                   // [W][R][NT] scratch of sg_get_state_hash
     unsigned long long *pt_acc;         // [MAX_NT] accepted swaps per lower slot t of the pair (t, t+1), all samples and replicas
     double *acc;                        // [n_samples][NT][SG_NMOM]
+    // diagnostics (library-owned allocations, not part of the workspace)
+    uint32_t *pq;                       // [n_samples][NT][pq_bins] or NULL (sg_enable_pq)
+    int pq_bins;
+    double *acc_win;                    // [n_windows][n_samples][NT][SG_NMOM] or NULL (sg_enable_log_binning)
+    int n_windows;
+    std::vector<int64_t> n_meas_win;    // measurements per window
     uint16_t *hist;                     // scratch [chunk samples][NT][P][N_HIST][L]
     double *rec;                        // scratch [chunk samples][NT][P][SG_REC]
     int chunk_samples;                  // samples per measurement chunk (multiple of 32)
@@ -118,6 +135,7 @@ int launch_pack_gauss(sg_ctx *c, int s0, int ns);
 int launch_couplings_pmj(sg_ctx *c, int s0, int ns, float *dev_out);   // -> [ns][3][N] float
 int launch_couplings_gauss(sg_ctx *c, int s0, int ns, float *dev_out);
 int launch_hash(sg_ctx *c, uint64_t *dev_out);             // one 64-bit hash per system -> dev_out
+sg::MeasOut meas_out(const sg_ctx *c);                     // where the measurement kernels add (window from the sweep counter)
 
 // kernel families for sg_ctx::attr_done
 enum { ATTR_LADDER8 = 0, ATTR_LADDER = 1, ATTR_GLADDER = 8, ATTR_RES32 = 10, ATTR_MEASURE = 11, ATTR_MEASURE32 = 18, ATTR_GMEASURE = 19, ATTR_TPACK = 24 };

@@ -11,7 +11,7 @@ namespace sg {
 // acc : [n_samples][NT][SG_NMOM]
 __global__ void __launch_bounds__(64)
 k_finalize(Dims d, const uint16_t *__restrict__ hist, const double *__restrict__ tw, int s0, int ns,
-           double *__restrict__ rec, double *__restrict__ acc)
+           double *__restrict__ rec, MeasOut mo)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= ns * d.NT) return;
@@ -50,9 +50,15 @@ k_finalize(Dims d, const uint16_t *__restrict__ hist, const double *__restrict__
     }
     const int s = s0 + sl;
     if (s >= d.n_samples) return;
-    double *A = acc + ((size_t)s * d.NT + t) * SG_NMOM;
+    if (mo.pq)
+        for (int p = 0; p < d.P; ++p) {
+            const uint16_t *hp = hist + (((size_t)sl * d.NT + t) * d.P + p) * (size_t)(N_HIST * L);
+            int D0 = 0;
+            for (int m = 0; m < L; ++m) D0 += hp[m];
+            atomicAdd(&mo.pq[((size_t)s * d.NT + t) * mo.pq_bins + pq_bin(d.N - D0, d.N, mo.pq_bins)], 1u);
+        }
     double a[SG_NMOM];
-    for (int j = 0; j < SG_NMOM; ++j) a[j] = A[j];
+    for (int j = 0; j < SG_NMOM; ++j) a[j] = 0.0;
     for (int p = 0; p < d.P; ++p) {
         const double v = r[p][0];
         a[0] += v; a[1] += v * v; a[2] += v * v * v; a[3] += (v * v) * (v * v);
@@ -78,7 +84,28 @@ k_finalize(Dims d, const uint16_t *__restrict__ hist, const double *__restrict__
             for (int k = 0; k < SG_NK; ++k)
                 a[4 + 5 * k + slot] += r[p][1 + 2 * k] * r[p2][1 + 2 * k] + r[p][2 + 2 * k] * r[p2][2 + 2 * k];
         }
-    for (int j = 0; j < SG_NMOM; ++j) A[j] = a[j];
+    double *A = mo.acc + ((size_t)s * d.NT + t) * SG_NMOM;
+    for (int j = 0; j < SG_NMOM; ++j) A[j] += a[j];
+    if (mo.acc_win) {
+        double *B = mo.acc_win + ((size_t)s * d.NT + t) * SG_NMOM;
+        for (int j = 0; j < SG_NMOM; ++j) B[j] += a[j];
+    }
+}
+
+MeasOut meas_out(const sg_ctx *c)
+{
+    MeasOut mo;
+    mo.acc = c->acc;
+    mo.pq = c->pq;
+    mo.pq_bins = c->pq_bins;
+    mo.acc_win = nullptr;
+    if (c->acc_win && c->sweeps >= 1) {            // window floor(log2(sweep counter)), clamped to the last one
+        int k = 0;
+        while ((c->sweeps >> (k + 1)) != 0) ++k;
+        if (k > c->n_windows - 1) k = c->n_windows - 1;
+        mo.acc_win = c->acc_win + (size_t)k * c->d.n_samples * c->d.NT * SG_NMOM;
+    }
+    return mo;
 }
 
 int launch_finalize(sg_ctx *c, int s0, int ns, bool want_rec)
@@ -86,7 +113,7 @@ int launch_finalize(sg_ctx *c, int s0, int ns, bool want_rec)
     const Dims &d = c->d;
     const int n = ns * d.NT;
     k_finalize<<<(unsigned)((n + 63) / 64), 64, 0, c->stream>>>(d, c->hist, c->twiddle, s0, ns,
-                                                                    want_rec ? c->rec : nullptr, c->acc);
+                                                                    want_rec ? c->rec : nullptr, meas_out(c));
     return 1;
 }
 
@@ -155,7 +182,7 @@ __device__ __forceinline__ BinGeom bin_geometry(int hh, int b)
 template <int L>
 __global__ void __launch_bounds__(256)
 k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restrict__ tw, int w0, int s0,
-              double *__restrict__ rec, double *__restrict__ acc)
+              double *__restrict__ rec, MeasOut mo)
 {
     using C = MeasureCfg<L>;
     constexpr int N = C::N, NB = C::NB, Lh = L / 2, H = N / 2;
@@ -279,7 +306,11 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
                 tot += cm;
                 v[m] = (double)(L * L - 2 * cm);
             }
-            if (hh == 0) r[0] = (double)(N - 2 * tot) * invN;
+            if (hh == 0) {
+                r[0] = (double)(N - 2 * tot) * invN;
+                if (mo.pq && w * 32 + l < d.n_samples)       // overlap histogram: N - tot sites agree
+                    atomicAdd(&mo.pq[((size_t)(w * 32 + l) * d.NT + t) * mo.pq_bins + pq_bin(N - tot, N, mo.pq_bins)], 1u);
+            }
             double re = 0.0, im = 0.0;
 #pragma unroll
             for (int m = 0; m < L; ++m) {
@@ -374,8 +405,10 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
         const int l = item / SG_NMOM, j = item - l * SG_NMOM;
         const int s = w * 32 + l;
         if (s >= d.n_samples) continue;
-        double *A = acc + ((size_t)s * d.NT + t) * SG_NMOM + j;
-        *A += OUT[l * OUT_LD + j];
+        const size_t o = ((size_t)s * d.NT + t) * SG_NMOM + j;
+        const double v = OUT[l * OUT_LD + j];
+        mo.acc[o] += v;
+        if (mo.acc_win) mo.acc_win[o] += v;
     }
 }
 
@@ -399,7 +432,7 @@ static int launch_measure_L(sg_ctx *c, int s0, int ns, bool want_rec)
     }
     const int w0 = s0 >> 5, nw = (ns + 31) >> 5;
     k_measure_pmj<L><<<(unsigned)(nw * d.NT), 256, smem, c->stream>>>(d, c->spins, c->twiddle, w0, s0,
-                                                                      want_rec ? c->rec : nullptr, c->acc);
+                                                                      want_rec ? c->rec : nullptr, meas_out(c));
     return 1;
 }
 

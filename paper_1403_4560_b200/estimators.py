@@ -113,3 +113,48 @@ def indicators(mom, n_meas: int, L: int, n_pairs: int = 6, block: int = 32) -> D
                 d = jk[k] - jk[k].mean(axis=0)
                 out[k + "_err"] = np.sqrt((nb - 1.0) / nb * np.sum(d * d, axis=0))
     return out
+
+
+def log_binning(windows, n_meas_windows, L: int, n_pairs: int = 6, block: int = 32):
+    """Logarithmic-binning equilibration test (Fig. 5 caption): the indicators evaluated separately on
+    the measurements of every window [2^k, 2^(k+1)) of the sweep counter (`sg_get_window_moments`).
+
+    windows          list of [n_samples][n_temps][66] window accumulators, index = k
+    n_meas_windows   measurements that fell into each window
+    Returns a list (index k) of `indicators(...)` dicts (None for an empty window).  A run passes the test when the
+    last few windows agree within their errors (see `log_binning_passes`).
+    """
+    return [indicators(w, int(n), L, n_pairs, block) if n > 0 else None for w, n in zip(windows, n_meas_windows)]
+
+
+def log_binning_passes(series, name: str, last: int = 3, n_sigma: float = 3.0) -> np.ndarray:
+    """Per temperature slot: do the `last` non-empty windows of `series` (from `log_binning`) agree on indicator
+    `name` within n_sigma combined jackknife errors?  Returns a bool array [n_temps]."""
+    pts = [s for s in series if s is not None][-last:]
+    if len(pts) < 2 or (name + "_err") not in pts[-1]:
+        raise ValueError("need at least two non-empty windows with jackknife errors")
+    ok = np.ones_like(pts[-1][name], dtype=bool)
+    for s in pts[:-1]:
+        err = np.sqrt(s[name + "_err"] ** 2 + pts[-1][name + "_err"] ** 2)
+        ok &= np.abs(s[name] - pts[-1][name]) <= n_sigma * err
+    return ok
+
+
+def overlap_distribution(pq, L: int):
+    """P(q) per slot from the device histogram of `sg_get_pq` ([n_samples][n_temps][n_bins] counts).
+
+    Returns (q_centres [n_bins], P [n_temps][n_bins] disorder-averaged and normalised to sum 1 per slot,
+    P_sample [n_samples][n_temps][n_bins] normalised per sample).  Bin b holds the overlaps with
+    floor(agree * n_bins / (N + 1)) = b, agree = (N q + N) / 2; the centre is the mean q of the values it covers.
+    """
+    pq = np.asarray(pq, dtype=np.float64)
+    n_bins = pq.shape[2]
+    N = L ** 3
+    agree = np.arange(N + 1)
+    which = (agree * n_bins) // (N + 1)
+    qv = (2.0 * agree - N) / N
+    centres = np.array([qv[which == b].mean() if np.any(which == b) else np.nan for b in range(n_bins)])
+    tot = pq.sum(axis=2, keepdims=True)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        per_sample = np.where(tot > 0, pq / tot, 0.0)
+    return centres, per_sample.mean(axis=0), per_sample

@@ -46,6 +46,10 @@ EXPORTS = {
     "sg_get_state_hash": (C.c_int, [C.c_void_p, C.c_void_p]),
     "sg_get_energies_cached": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "sg_get_pt_stats": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "sg_enable_pq": (C.c_int, [C.c_void_p, C.c_int]),
+    "sg_get_pq": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "sg_enable_log_binning": (C.c_int, [C.c_void_p, C.c_int]),
+    "sg_get_window_moments": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]),
 }
 
 if not os.path.exists(LIB_PATH):
@@ -88,6 +92,7 @@ class Simulation:
         self.NT = int(self.temps.size)
         self.kind = int(coupling_kind)
         self.n_pairs = self.R * (self.R - 1) // 2
+        self.pq_bins, self.n_windows = 1, 0
         self._h = C.c_void_p()
         self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
         need = sg_workspace_bytes(self.L, self.n_samples, self.R, self.NT, self.kind)
@@ -202,6 +207,25 @@ class Simulation:
         acc = np.zeros(max(self.NT - 1, 0), dtype=np.uint64)
         self._check(_lib.sg_get_pt_stats(self._h, _p(prop), _p(acc)))
         return prop, acc
+
+    def sg_enable_pq(self, n_bins=None):
+        self.pq_bins = self.N + 1 if n_bins is None else int(n_bins)
+        self._check(_lib.sg_enable_pq(self._h, self.pq_bins))
+
+    def sg_get_pq(self):
+        out = np.empty((self.n_samples, self.NT, self.pq_bins), dtype=np.uint32)
+        self._check(_lib.sg_get_pq(self._h, _p(out)))
+        return out
+
+    def sg_enable_log_binning(self, n_windows):
+        self.n_windows = int(n_windows)
+        self._check(_lib.sg_enable_log_binning(self._h, self.n_windows))
+
+    def sg_get_window_moments(self, k):
+        out = np.empty((self.n_samples, self.NT, NMOM), dtype=np.float64)
+        n = C.c_int64()
+        self._check(_lib.sg_get_window_moments(self._h, int(k), _p(out), C.byref(n)))
+        return out, n.value
 
     def sg_get_thresholds(self):
         out = np.empty((self.NT, 7, 2), dtype=np.uint64)
