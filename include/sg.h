@@ -44,7 +44,11 @@ typedef enum sg_status {
     SG_ESTATE = -5        /* call not valid in the current state */
 } sg_status;
 
-enum { SG_PMJ = 0, SG_GAUSS = 1 }; /* coupling_kind */
+/* coupling_kind.  SG_PMJ_TPACK: the same +-J model and the same trajectories as SG_PMJ, simulated in the paper's own
+ * packing (R17): the temperature copies of one (sample, replica) are the bits of a word, the
+ * lattice lives in shared memory, parallel tempering is a bit permutation.  For few samples and many temperatures;
+ * L in {4, 6, 8, 10, 12, 16}, n_temps <= 64 (SG_EUNSUPPORTED otherwise). */
+enum { SG_PMJ = 0, SG_GAUSS = 1, SG_PMJ_TPACK = 2 };
 
 #define SG_NK 12   /* non-zero wave vectors per record (R8) */
 #define SG_REC 25  /* doubles per (sample, slot, pair) record: q(0), Re q(K0), Im q(K0), ... (R9) */
@@ -65,7 +69,7 @@ size_t sg_workspace_bytes(int L, int n_samples, int n_replicas, int n_temps, int
  *   temps         host ptr, n_temps temperatures T > 0, non-decreasing (slot 0 coldest; equal neighbours
  *                 are allowed: every proposed swap between them is accepted); copied
  *   n_temps       1 <= n_temps <= 64
- *   coupling_kind SG_PMJ or SG_GAUSS
+ *   coupling_kind SG_PMJ, SG_GAUSS or SG_PMJ_TPACK
  *   workspace     device ptr, 256-byte aligned, >= sg_workspace_bytes(...) bytes, must outlive the
  *                 context; or NULL: the library cudaMallocs (and frees in sg_destroy)
  *   cuda_stream   a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL = default

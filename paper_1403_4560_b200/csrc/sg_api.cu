@@ -22,7 +22,7 @@ constexpr int DEXP64_N = 5761, DEXP32_N = 1441;
 inline size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-    size_t spins, spins_alt, J, Jp, tab, exp64, exp32, tw, U, M, U_alt, M_alt, swap, pt_acc, hashes, acc, hist, rec, stage, total;
+    size_t spins, spins_alt, J, Jp, tps, J6, tab, exp64, exp32, tw, U, M, U_alt, M_alt, swap, pt_acc, hashes, acc, hist, rec, stage, total;
     int chunk_meas, chunk_stage, S_pad;
 };
 
@@ -32,7 +32,7 @@ bool valid_args(int L, int n_samples, int R, int NT, int kind)
     if (n_samples < 1 || n_samples > (1 << 24)) return false;
     if (R != 2 && R != 4) return false;
     if (NT < 1 || NT > MAX_NT) return false;
-    if (kind != SG_PMJ && kind != SG_GAUSS) return false;
+    if (kind != SG_PMJ && kind != SG_GAUSS && kind != SG_PMJ_TPACK) return false;
     return true;
 }
 
@@ -42,14 +42,19 @@ Layout make_layout(int L, int n_samples, int R, int NT, int kind)
     const size_t N = (size_t)L * L * L;
     const int P = R * (R - 1) / 2;
     const int W = (n_samples + 31) / 32;
-    lo.S_pad = kind == SG_PMJ ? W * 32 : n_samples;
+    lo.S_pad = kind != SG_GAUSS ? W * 32 : n_samples;
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += up(bytes); return o; };
-    if (kind == SG_PMJ) {
+    lo.tps = lo.J6 = 0;
+    if (kind != SG_GAUSS) {
         lo.spins = take((size_t)W * R * NT * N * 4);
-        lo.spins_alt = L == 32 ? take((size_t)W * R * NT * N * 4) : 0;     // k_res32_pmj reads one buffer, writes the other
+        lo.spins_alt = (kind == SG_PMJ && L == 32) ? take((size_t)W * R * NT * N * 4) : 0;   // k_res32_pmj reads one buffer, writes the other
         lo.J = take((size_t)W * 3 * N * 4);
-        lo.Jp = L == 32 ? take(res32_packed_bytes(W)) : 0;
+        lo.Jp = (kind == SG_PMJ && L == 32) ? take(res32_packed_bytes(W)) : 0;
+        if (kind == SG_PMJ_TPACK) {
+            lo.tps = take(tp_state_bytes(L, n_samples, R, NT));
+            lo.J6 = take((size_t)n_samples * N);
+        }
     } else {
         lo.Jp = 0;
         lo.spins_alt = 0;
@@ -65,7 +70,7 @@ Layout make_layout(int L, int n_samples, int R, int NT, int kind)
     lo.U_alt = take(sizeof(int64_t) * (size_t)lo.S_pad * R * NT);
     lo.M_alt = take(sizeof(int32_t) * (size_t)lo.S_pad * R * NT);
     lo.pt_acc = take(sizeof(unsigned long long) * MAX_NT);
-    lo.hashes = take(sizeof(uint64_t) * (size_t)(kind == SG_PMJ ? W : n_samples) * R * NT);
+    lo.hashes = take(sizeof(uint64_t) * (size_t)(kind != SG_GAUSS ? W : n_samples) * R * NT);
     lo.swap = take(sizeof(uint32_t) * (size_t)lo.S_pad * R * (NT / 2 + 1));
     lo.acc = take(sizeof(double) * (size_t)n_samples * NT * SG_NMOM);
     // measurement scratch, chunked over samples (multiples of 32)
@@ -178,8 +183,12 @@ int do_reset(sg_ctx *c)
     if (c->pq && (rc = check_cuda(c, cudaMemsetAsync(c->pq, 0, sizeof(uint32_t) * (size_t)d.n_samples * d.NT * c->pq_bins, c->stream), "zero P(q)"))) return rc;
     if (c->acc_win && (rc = check_cuda(c, cudaMemsetAsync(c->acc_win, 0, sizeof(double) * (size_t)c->n_windows * d.n_samples * d.NT * SG_NMOM, c->stream), "zero windows"))) return rc;
     std::fill(c->n_meas_win.begin(), c->n_meas_win.end(), 0);
-    c->launches += c->kind == SG_PMJ ? launch_init_pmj(c) : launch_init_gauss(c);
+    c->launches += is_packed(c) ? launch_init_pmj(c) : launch_init_gauss(c);
     if (c->Jp) c->launches += launch_pack_J_res32(c);
+    if (c->kind == SG_PMJ_TPACK) {
+        c->launches += launch_tp_pack_J(c);
+        c->tp_state = 2;                                    // the initial state was generated in the sample-packed layout
+    }
     c->sweeps = c->exchanges = 0;
     c->n_meas = 0;
     c->um_fresh = false;
@@ -192,6 +201,11 @@ int do_reset(sg_ctx *c)
 // materialises it here: decision kernel from the kernels' own U, M, then the masked swap of spins and U, M.
 int flush_pending(sg_ctx *c)
 {
+    if (c->kind == SG_PMJ_TPACK && c->tp_state == 1) {      // the temperature-packed copy is newer: convert it back
+        c->launches += launch_tp_to_std(c);
+        c->tp_state = 0;
+        return check_launch(c, "layout conversion");
+    }
     if (!c->pending_exchange) return SG_OK;
     c->pending_exchange = false;
     c->launches += launch_pt_pmj(c, c->exchanges - 1);
@@ -204,9 +218,10 @@ int do_exchange(sg_ctx *c)
 {
     int rc;
     if ((rc = flush_pending(c))) return rc;
-    if (!c->um_fresh) c->launches += c->kind == SG_PMJ ? launch_energy_pmj(c) : launch_energy_gauss(c);
+    if (!c->um_fresh) c->launches += is_packed(c) ? launch_energy_pmj(c) : launch_energy_gauss(c);
     c->um_fresh = true;
-    c->launches += c->kind == SG_PMJ ? launch_pt_pmj(c, c->exchanges) : launch_pt_gauss(c, c->exchanges);
+    c->launches += is_packed(c) ? launch_pt_pmj(c, c->exchanges) : launch_pt_gauss(c, c->exchanges);
+    if (c->kind == SG_PMJ_TPACK) c->tp_state = 2;           // the swap ran on the sample-packed copy
     c->exchanges += 1;
     return check_launch(c, "pt kernels");
 }
@@ -225,7 +240,7 @@ int do_measure(sg_ctx *c, double *out)
             if (k < 0) return check_launch(c, "measure kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "measure kernel launch failed");
             c->launches += k;
         } else {
-            c->launches += c->kind == SG_PMJ ? launch_hist_pmj(c, s0, ns) : launch_hist_gauss(c, s0, ns);
+            c->launches += is_packed(c) ? launch_hist_pmj(c, s0, ns) : launch_hist_gauss(c, s0, ns);
             c->launches += launch_finalize(c, s0, ns, out != nullptr);
         }
         int rc = check_launch(c, "measure kernels");
@@ -268,11 +283,29 @@ int res32_step(sg_ctx *c, int n, bool energy_after)
     return SG_OK;
 }
 
+// SG_PMJ_TPACK: n sweeps on the temperature-packed state with the exchanges that fall due fused in
+int tp_step(sg_ctx *c, int n, int pt_every)
+{
+    if (c->tp_state == 2) {
+        c->launches += launch_tp_from_std(c);
+        c->tp_state = 0;
+    }
+    const int k = launch_tp_run(c, c->sweeps, n, c->exchanges, pt_every);
+    if (k < 0) return check_launch(c, "tpack kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "tpack kernel launch failed");
+    c->launches += k;
+    if (pt_every > 0) c->exchanges += (c->sweeps + (uint64_t)n) / (uint64_t)pt_every - c->sweeps / (uint64_t)pt_every;
+    c->sweeps += n;
+    c->um_fresh = pt_every > 0 && c->sweeps % (uint64_t)pt_every == 0;
+    c->tp_state = 1;
+    return SG_OK;
+}
+
 // n consecutive sweeps with nothing in between
 int do_sweeps(sg_ctx *c, int n)
 {
     if (n <= 0) return SG_OK;
     int rc;
+    if (tp_supported(c)) return tp_step(c, n, 0);
     if (res32_supported(c)) return res32_step(c, n, false);
     if ((rc = flush_pending(c))) return rc;
     c->um_fresh = false;
@@ -298,9 +331,10 @@ int do_sweeps(sg_ctx *c, int n)
         return SG_OK;
     }
     for (int i = 0; i < n; ++i) {
-        c->launches += c->kind == SG_PMJ ? launch_sweep_pmj(c, c->sweeps) : launch_sweep_gauss(c, c->sweeps);
+        c->launches += is_packed(c) ? launch_sweep_pmj(c, c->sweeps) : launch_sweep_gauss(c, c->sweeps);
         c->sweeps += 1;
     }
+    if (c->kind == SG_PMJ_TPACK) c->tp_state = 2;
     return SG_OK;
 }
 
@@ -354,7 +388,7 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     d.L = L; d.Lh = L / 2; d.N = L * L * L; d.H = d.N / 2;
     d.R = n_replicas; d.NT = n_temps; d.P = n_replicas * (n_replicas - 1) / 2;
     d.n_samples = n_samples;
-    d.W = coupling_kind == SG_PMJ ? (n_samples + 31) / 32 : n_samples;
+    d.W = coupling_kind != SG_GAUSS ? (n_samples + 31) / 32 : n_samples;
     d.k0 = (uint32_t)seed; d.k1 = (uint32_t)(seed >> 32);
     d.neg_h = h < 0.0 ? 1u : 0u;
     d.fast_accept = 0;
@@ -378,6 +412,9 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     c->J = (uint32_t *)(b + lo.J);
     c->Jg = (float *)(b + lo.J);
     c->Jp = (coupling_kind == SG_PMJ && L == 32) ? (uint4 *)(b + lo.Jp) : nullptr;
+    c->tps = coupling_kind == SG_PMJ_TPACK ? (uint32_t *)(b + lo.tps) : nullptr;
+    c->J6 = coupling_kind == SG_PMJ_TPACK ? (uint8_t *)(b + lo.J6) : nullptr;
+    c->tp_state = 0;
     c->tab = (SlotTab *)(b + lo.tab);
     c->exp64_tab = (double *)(b + lo.exp64);
     c->exp32_tab = (float *)(b + lo.exp32);
@@ -395,6 +432,8 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     c->stage8 = (int8_t *)(b + lo.stage);
     c->chunk_samples = lo.chunk_meas;
     int rc = upload_tables(c);
+    if (!rc && coupling_kind == SG_PMJ_TPACK && !tp_supported(c))
+        rc = fail(c, SG_EUNSUPPORTED, "sg_create: SG_PMJ_TPACK needs L in {4, 6, 8, 10, 12, 16} and a (sample, replica) lattice that fits in shared memory");
     if (!rc) rc = do_reset(c);
     if (rc) {
         g_create_err = c->err;
@@ -409,7 +448,7 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
 int sg_set_first_sample(sg_ctx *c, int64_t first_sample)
 {
     if (!c) return SG_EINVAL;
-    if (first_sample < 0 || first_sample > 0x7fffffff - c->d.n_samples - 32 || (c->kind == SG_PMJ && (first_sample & 31)))
+    if (first_sample < 0 || first_sample > 0x7fffffff - c->d.n_samples - 32 || (c->kind != SG_GAUSS && (first_sample & 31)))
         return fail(c, SG_EINVAL, "sg_set_first_sample: need 0 <= first_sample < 2^31, a multiple of 32 for SG_PMJ");
     c->d.s_first = (int)first_sample;
     return SG_OK;
@@ -450,6 +489,18 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
     if (n_sweeps < 0 || pt_every < 0 || meas_every < 0) return fail(c, SG_EINVAL, "sg_run: negative argument");
     if (sweeps_overflow(c, n_sweeps)) return fail(c, SG_EINVAL, "sg_run: the global sweep counter must stay below 2^31");
     int left = n_sweeps, rc;
+    if (tp_supported(c)) {
+        // sweeps and exchanges fused in one launch on the temperature-packed state; launches end at measurements
+        while (left > 0) {
+            uint64_t run = (uint64_t)left;
+            if (meas_every > 0) run = std::min<uint64_t>(run, (uint64_t)meas_every - c->sweeps % (uint64_t)meas_every);
+            if ((rc = tp_step(c, (int)run, pt_every))) return rc;
+            left -= (int)run;
+            if (meas_every > 0 && c->sweeps % (uint64_t)meas_every == 0)
+                if ((rc = do_measure(c, nullptr))) return rc;
+        }
+        return check_launch(c, "run kernels");
+    }
     if (ladder8_supported(c) || ladder_supported(c) || gladder_supported(c)) {
         // sweeps and the exchanges between them are fused in one launch; launches end at measurements
         while (left > 0) {
@@ -519,17 +570,20 @@ static int spins_range(sg_ctx *c, int s0, int ns, int8_t *out, const int8_t *in)
         const int rc = flush_pending(c);
         if (rc) return rc;
     }
-    if (in) c->um_fresh = false;
+    if (in) {
+        c->um_fresh = false;
+        if (c->kind == SG_PMJ_TPACK) c->tp_state = 2;
+    }
     for (int a = s0; a < s0 + ns; a += lo.chunk_stage) {
         const int n = std::min(lo.chunk_stage, s0 + ns - a);
         int rc;
         if (out) {
-            c->launches += c->kind == SG_PMJ ? launch_unpack_pmj(c, a, n) : launch_unpack_gauss(c, a, n);
+            c->launches += is_packed(c) ? launch_unpack_pmj(c, a, n) : launch_unpack_gauss(c, a, n);
             if ((rc = check_launch(c, "unpack kernel"))) return rc;
             if ((rc = check_cuda(c, cudaMemcpyAsync(out + (size_t)(a - s0) * per, c->stage8, per * n, cudaMemcpyDeviceToHost, c->stream), "copy spins"))) return rc;
         } else {
             if ((rc = check_cuda(c, cudaMemcpyAsync(c->stage8, in + (size_t)(a - s0) * per, per * n, cudaMemcpyHostToDevice, c->stream), "copy spins"))) return rc;
-            c->launches += c->kind == SG_PMJ ? launch_pack_pmj(c, a, n) : launch_pack_gauss(c, a, n);
+            c->launches += is_packed(c) ? launch_pack_pmj(c, a, n) : launch_pack_gauss(c, a, n);
             if ((rc = check_launch(c, "pack kernel"))) return rc;
         }
         if ((rc = check_cuda(c, cudaStreamSynchronize(c->stream), "sync spins"))) return rc;
@@ -552,7 +606,7 @@ int sg_get_couplings_range(sg_ctx *c, int s0, int ns, float *out)
     for (int a = s0; a < s0 + ns; a += lo.chunk_stage) {
         const int n = std::min(lo.chunk_stage, s0 + ns - a);
         float *dev = (float *)c->stage8;
-        c->launches += c->kind == SG_PMJ ? launch_couplings_pmj(c, a, n, dev) : launch_couplings_gauss(c, a, n, dev);
+        c->launches += is_packed(c) ? launch_couplings_pmj(c, a, n, dev) : launch_couplings_gauss(c, a, n, dev);
         int rc;
         if ((rc = check_launch(c, "couplings kernel"))) return rc;
         if ((rc = check_cuda(c, cudaMemcpyAsync(out + (size_t)(a - s0) * per, dev, sizeof(float) * per * n, cudaMemcpyDeviceToHost, c->stream), "copy couplings"))) return rc;
@@ -577,7 +631,7 @@ int sg_get_energies(sg_ctx *c, int64_t *U, int32_t *M)
     if (!c) return SG_EINVAL;
     int rc;
     if ((rc = flush_pending(c))) return rc;
-    c->launches += c->kind == SG_PMJ ? launch_energy_pmj(c) : launch_energy_gauss(c);     // always a recount
+    c->launches += is_packed(c) ? launch_energy_pmj(c) : launch_energy_gauss(c);     // always a recount
     if ((rc = check_launch(c, "energy kernel"))) return rc;
     c->um_fresh = true;
     return copy_energies(c, U, M);

@@ -73,6 +73,9 @@ struct sg_ctx {
     uint32_t *spins;                    // PMJ: [W][R][NT][2][H] colour-compacted words (the CURRENT state)
     uint32_t *spins_alt;                // PMJ, L = 32: second state buffer; k_res32_pmj reads `spins`, writes `spins_alt`, then they swap
     uint32_t *J;                        // PMJ: [W][2][3][H]
+    uint32_t *tps;                      // SG_PMJ_TPACK: [S][R][NW][2][H] temperature-packed state (sg_tpack.cu)
+    uint8_t *J6;                        // SG_PMJ_TPACK: [S][2][H] six bond bits per site
+    int tp_state;                       // SG_PMJ_TPACK: 0 = both layouts current, 1 = tps newer, 2 = spins (sample-packed) newer
     uint4 *Jp;                          // PMJ, L = 32: couplings repacked per warp step for k_res32_pmj (else NULL)
     int8_t *spins8;                     // GAUSS: [S][R][NT][2][H] colour-compacted bytes
     float *Jg;                          // GAUSS: [S][2][3][H]
@@ -134,6 +137,13 @@ int launch_unpack_gauss(sg_ctx *c, int s0, int ns);
 int launch_pack_gauss(sg_ctx *c, int s0, int ns);
 int launch_couplings_pmj(sg_ctx *c, int s0, int ns, float *dev_out);   // -> [ns][3][N] float
 int launch_couplings_gauss(sg_ctx *c, int s0, int ns, float *dev_out);
+size_t tp_state_bytes(int L, int n_samples, int R, int NT);
+bool tp_supported(const sg_ctx *c);                        // SG_PMJ_TPACK resident kernel usable?
+int launch_tp_pack_J(sg_ctx *c);                           // J -> J6
+int launch_tp_from_std(sg_ctx *c);                         // spins -> tps
+int launch_tp_to_std(sg_ctx *c);                           // tps -> spins
+int launch_tp_run(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0, int pt_every);   // 1 launch (-1 on error)
+inline bool is_packed(const sg_ctx *c) { return c->kind != SG_GAUSS; }   // sample-packed +-J state in c->spins
 int launch_hash(sg_ctx *c, uint64_t *dev_out);             // one 64-bit hash per system -> dev_out
 sg::MeasOut meas_out(const sg_ctx *c);                     // where the measurement kernels add (window from the sweep counter)
 

@@ -439,7 +439,7 @@ static int launch_measure_L(sg_ctx *c, int s0, int ns, bool want_rec)
 bool measure_fused_supported(const sg_ctx *c)
 {
     const int L = c->d.L;
-    return c->path == SG_PATH_AUTO && c->kind == SG_PMJ && (L == 4 || L == 6 || L == 8 || L == 10 || L == 12 || L == 16);
+    return c->path == SG_PATH_AUTO && is_packed(c) && (L == 4 || L == 6 || L == 8 || L == 10 || L == 12 || L == 16);
 }
 
 // samples [s0, s0+ns), s0 a multiple of 32: records (optional) and accumulators in one launch

@@ -475,8 +475,8 @@ int launch_hash(sg_ctx *c, uint64_t *dev_out)
 {
     const Dims &d = c->d;
     const long long n_sys = (long long)d.W * d.R * d.NT;
-    const int wps = c->kind == SG_PMJ ? d.N : d.N / 4;
-    const uint32_t *words = c->kind == SG_PMJ ? c->spins : reinterpret_cast<const uint32_t *>(c->spins8);
+    const int wps = is_packed(c) ? d.N : d.N / 4;
+    const uint32_t *words = is_packed(c) ? c->spins : reinterpret_cast<const uint32_t *>(c->spins8);
     k_hash_words<<<blocks_for(n_sys, 4), 128, 0, c->stream>>>(words, n_sys, wps, dev_out);
     return 1;
 }

@@ -9,7 +9,7 @@ import os
 
 import numpy as np
 
-PMJ, GAUSS = 0, 1
+PMJ, GAUSS, PMJ_TPACK = 0, 1, 2
 NK, REC, NMOM = 12, 25, 66
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ESTATE = 0, -1, -2, -3, -4, -5
 PATH_AUTO, PATH_GENERIC = 0, 1
@@ -196,7 +196,7 @@ class Simulation:
         self._check(_lib.sg_set_kernel_path(self._h, int(path)))
 
     def sg_get_state_hash(self):
-        nw = (self.n_samples + 31) // 32 if self.kind == PMJ else self.n_samples
+        nw = (self.n_samples + 31) // 32 if self.kind != GAUSS else self.n_samples
         out = np.empty((nw, self.R, self.NT), dtype=np.uint64)
         self._check(_lib.sg_get_state_hash(self._h, _p(out)))
         return out
