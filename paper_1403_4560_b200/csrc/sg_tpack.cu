@@ -4,7 +4,7 @@
 // One 32-bit word per lattice site holds the spins of the temperature copies of ONE (sample, replica): bit tl of
 // word j is slot t = 32 j + tl (N_T <= 64: one or two words per site).  The couplings are common to all bits
 // (6 bits per site, expanded to 0 / ~0 words on the fly), the lattice of a (sample, replica) lives in the shared
-// memory of one warp for all sweeps of a launch, and parallel tempering is a bit permutation inside the word
+// memory of one CTA for all sweeps of a launch, and parallel tempering is a bit permutation inside the word
 // (masked delta swap of neighbouring bits; one extra swap across the word boundary for N_T > 32).
 //
 // R17: every temperature copy keeps its OWN 32-bit Philox draw per site (the draws of slot t are exactly those of
@@ -35,7 +35,7 @@ struct TpArgs {
     uint64_t sweep0, exchange0;
     int n_sweeps, pt_every;
     int NW;                   // words per site: ceil(NT / 32)
-    int wpb;                  // warps (= (sample, replica) lattices) per CTA
+    int wpb;                  // unused (one CTA per lattice)
     int64_t *U;               // [S][R][NT] the kernel's own energies after the last exchange of the launch
     int32_t *M;
     unsigned long long *pt_acc;
@@ -60,8 +60,16 @@ __device__ __forceinline__ void nbr6(int c, int n, int (&ix)[6])
     ix[5] = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;                 // -z
 }
 
-template <int L>
-__global__ void __launch_bounds__(128) k_tp_run(const __grid_constant__ TpArgs A)
+constexpr int TP_THREADS = 256;
+
+// One CTA per (sample, replica) lattice.  Work item of a half sweep = (quad q, word j, group of 8 slots): the thread
+// counts the unsatisfied bonds of the quad's 4 sites for all slots of the word (bitwise, so the other groups' bits cost
+// nothing), then draws and decides its 8 slots and flips them with one atomicXor per site word (the groups of a word
+// touch disjoint bits, and no thread reads bits of another group).
+// SPI = slots per item: 8 when there are few lattices (more threads per lattice, lower latency), 32 when the GPU is
+// full anyway (the bond counting and the neighbour indices of a quad are then shared by all slots of the word).
+template <int L, int SPI>
+__global__ void __launch_bounds__(TP_THREADS) k_tp_run(const __grid_constant__ TpArgs A)
 {
     constexpr int N = L * L * L, H = N / 2, Q = H / 4;
     extern __shared__ __align__(16) unsigned char sm_raw[];
@@ -69,40 +77,39 @@ __global__ void __launch_bounds__(128) k_tp_run(const __grid_constant__ TpArgs A
     const int NT = d.NT, NW = A.NW;
     uint2 *thr = reinterpret_cast<uint2 *>(sm_raw);                      // [NT][7][2] thresholds as (lo, hi) of thr in [0, 2^32]
     uint32_t *spread = reinterpret_cast<uint32_t *>(thr + NT * 14);      // [256] bit i of the index -> bit 4 i
-    unsigned char *per_warp = reinterpret_cast<unsigned char *>(spread + 256);
-    const size_t warp_bytes = (size_t)NW * N * 4 + ((N + 15) & ~15);
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    uint32_t *S = reinterpret_cast<uint32_t *>(per_warp + (size_t)warp * warp_bytes);   // [NW][2][H]
-    uint8_t *Jb = reinterpret_cast<uint8_t *>(S + (size_t)NW * N);                       // [2][H]
+    uint32_t *S = spread + 256;                                          // [NW][2][H]
+    int *UM = reinterpret_cast<int *>(S + (size_t)NW * N);               // [2 (U, M)][NW][32] per-slot energies
+    uint32_t *masks = reinterpret_cast<uint32_t *>(UM + 4 * 32);         // [NW] accepted lower slots of the exchange
+    uint8_t *Jb = reinterpret_cast<uint8_t *>(masks + 4);                // [2][H]
+    const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5;
 
-    for (int i = tid; i < NT * 14; i += blockDim.x) {
+    for (int i = tid; i < NT * 14; i += nthr) {
         const uint2 v = A.tab[i / 14].c64g[(i % 14) >> 1][i & 1];        // (uint64)(0 - thr)
         const uint64_t th = (uint64_t)0 - (((uint64_t)v.y << 32) | v.x);
         thr[i] = make_uint2((uint32_t)th, (uint32_t)(th >> 32));
     }
-    for (int i = tid; i < 256; i += blockDim.x) {
+    for (int i = tid; i < 256; i += nthr) {
         uint32_t x = 0;
         for (int b = 0; b < 8; ++b) x |= ((uint32_t)(i >> b) & 1u) << (4 * b);
         spread[i] = x;
     }
-    const long long lat = (long long)blockIdx.x * A.wpb + warp;          // (sample, replica) lattice of this warp
-    const bool active = warp < A.wpb && lat < (long long)d.n_samples * d.R;
-    const int s = active ? (int)(lat / d.R) : 0, a = active ? (int)(lat % d.R) : 0;
+    const int lat = blockIdx.x;                                          // (sample, replica) lattice of this CTA
+    const int s = lat / d.R, a = lat % d.R;
     uint32_t *gS = A.tps + (size_t)lat * NW * N;
-    if (active) {
-        for (int i = lane; i < NW * N / 4; i += 32) reinterpret_cast<uint4 *>(S)[i] = reinterpret_cast<const uint4 *>(gS)[i];
+    for (int i = tid; i < NW * N / 4; i += nthr) reinterpret_cast<uint4 *>(S)[i] = reinterpret_cast<const uint4 *>(gS)[i];
+    {
         const uint32_t *gJ = reinterpret_cast<const uint32_t *>(A.J6 + (size_t)s * N);
-        for (int i = lane; i < N / 4; i += 32) reinterpret_cast<uint32_t *>(Jb)[i] = gJ[i];
+        for (int i = tid; i < N / 4; i += nthr) reinterpret_cast<uint32_t *>(Jb)[i] = gJ[i];
     }
-    __syncthreads();                                                     // the only CTA-wide barrier: tables ready
-    if (!active) return;
+    __syncthreads();
 
     const uint32_t amask = d.neg_h ? 0xffffffffu : 0u;
     const uint32_t wglob = (uint32_t)((s + d.s_first) >> 5);             // sweep draws are keyed by the packed word of the sample (R5)
     const uint32_t sglob = (uint32_t)(s + d.s_first);
     uint64_t exchange = A.exchange0;
-    uint32_t cnt[2] = {0u, 0u};                                          // accepted swaps with this lane's slot as the lower one
-    int Ureg[2] = {0, 0}, Mreg[2] = {0, 0};
+    uint32_t cnt[2] = {0u, 0u};                                          // warp 0: accepted swaps with this lane's slot as the lower one
+    constexpr int NG = 32 / SPI;                                         // slot groups (items) per word
+    const int n_items = Q * NW * NG;
 
     for (int sw = 0; sw < A.n_sweeps; ++sw) {
         const uint64_t sweep = A.sweep0 + (uint64_t)sw;
@@ -110,85 +117,80 @@ __global__ void __launch_bounds__(128) k_tp_run(const __grid_constant__ TpArgs A
         for (int colour = 0; colour < 2; ++colour) {
             const uint32_t time = 2u * (uint32_t)sweep + (uint32_t)colour;
 #pragma unroll 1
-            for (int q = lane; q < Q; q += 32) {
-                int ix[4][6];
-                uint32_t j6[4];
-                {
-                    const uint32_t jq = reinterpret_cast<const uint32_t *>(Jb + colour * H)[q];
+            for (int item = tid; item < n_items; item += nthr) {
+                const int q = item % Q, rest = item / Q;                 // consecutive threads: consecutive quads (conflict-free)
+                const int j = rest % NW, tb0 = SPI * (rest / NW);
+                const int nb = NT - 32 * j < 32 ? NT - 32 * j : 32;      // slots in this word
+                if (tb0 >= nb) continue;
+                uint32_t *Sa = S + (size_t)j * N + colour * H;
+                const uint32_t *So = S + (size_t)j * N + (1 - colour) * H;
+                const uint32_t jq = reinterpret_cast<const uint32_t *>(Jb + colour * H)[q];
+                uint32_t al[4], n0[4], n1[4], n2[4];                     // field alignment and unsatisfied-bond count planes
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        nbr6<L>(colour, 4 * q + e, ix[e]);
-                        j6[e] = (jq >> (8 * e)) & 0xffu;
-                    }
+                for (int e = 0; e < 4; ++e) {
+                    int ix[6];
+                    nbr6<L>(colour, 4 * q + e, ix);
+                    const uint32_t j6 = (jq >> (8 * e)) & 0xffu;
+                    const uint32_t sp = Sa[4 * q + e];
+                    uint32_t u[6];
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) u[k] = xor3(sp, So[ix[k]], 0u - ((j6 >> k) & 1u));
+                    const uint32_t s0 = xor3(u[0], u[1], u[2]), c0 = maj3(u[0], u[1], u[2]);
+                    const uint32_t s1 = xor3(u[3], u[4], u[5]), c1 = maj3(u[3], u[4], u[5]);
+                    const uint32_t kk = s0 & s1;
+                    n0[e] = s0 ^ s1;
+                    n1[e] = xor3(c0, c1, kk);
+                    n2[e] = maj3(c0, c1, kk);
+                    al[e] = sp ^ amask;
                 }
 #pragma unroll 1
-                for (int j = 0; j < NW; ++j) {
-                    uint32_t *Sa = S + (size_t)j * N + colour * H;
-                    const uint32_t *So = S + (size_t)j * N + (1 - colour) * H;
-                    const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[q];
-                    const uint32_t sp[4] = {sv.x, sv.y, sv.z, sv.w};
-                    uint32_t al[4], n0[4], n1[4], n2[4];                 // field alignment and unsatisfied-bond count planes
+              for (int tb = tb0; tb < tb0 + SPI && tb < nb; tb += 8) {
+                uint32_t cw[4];                                          // class nibbles of 8 slots: a | n0 << 1 | n1 << 2 | n2 << 3 = a + 2 n_u
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        uint32_t u[6];
+                for (int e = 0; e < 4; ++e)
+                    cw[e] = spread[(al[e] >> tb) & 0xffu] | (spread[(n0[e] >> tb) & 0xffu] << 1) |
+                            (spread[(n1[e] >> tb) & 0xffu] << 2) | (spread[(n2[e] >> tb) & 0xffu] << 3);
+                uint32_t acc[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
-                        for (int k = 0; k < 6; ++k) u[k] = xor3(sp[e], So[ix[e][k]], 0u - ((j6[e] >> k) & 1u));
-                        const uint32_t s0 = xor3(u[0], u[1], u[2]), c0 = maj3(u[0], u[1], u[2]);
-                        const uint32_t s1 = xor3(u[3], u[4], u[5]), c1 = maj3(u[3], u[4], u[5]);
-                        const uint32_t kk = s0 & s1;
-                        n0[e] = s0 ^ s1;
-                        n1[e] = xor3(c0, c1, kk);
-                        n2[e] = maj3(c0, c1, kk);
-                        al[e] = sp[e] ^ amask;
-                    }
-                    uint32_t acc[4] = {0u, 0u, 0u, 0u};
-                    const int nb = NT - 32 * j < 32 ? NT - 32 * j : 32;  // slots in this word
-#pragma unroll 1
-                    for (int tb = 0; tb < nb; tb += 8) {
-                        // class nibbles of the 8 slots tb .. tb + 7: a | n0 << 1 | n1 << 2 | n2 << 3 = a + 2 n_u
-                        uint32_t cw[4];
+                for (int t8 = 0; t8 < 8; ++t8) {
+                    const int tl = tb + t8;
+                    if (tl < nb) {
+                        const int t = 32 * j + tl;
+                        const uint4 r4 = philox_rk8((uint32_t)q, time, wglob, ctr3(3, a, t), A.rk);
+                        const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
+                        const uint2 *tt = thr + t * 14;
 #pragma unroll
-                        for (int e = 0; e < 4; ++e)
-                            cw[e] = spread[(al[e] >> tb) & 0xffu] | (spread[(n0[e] >> tb) & 0xffu] << 1) |
-                                    (spread[(n1[e] >> tb) & 0xffu] << 2) | (spread[(n2[e] >> tb) & 0xffu] << 3);
-#pragma unroll
-                        for (int t8 = 0; t8 < 8; ++t8) {
-                            const int tl = tb + t8;
-                            if (tl < nb) {                               // warp-uniform
-                                const int t = 32 * j + tl;
-                                const uint4 r4 = philox_rk8((uint32_t)q, time, wglob, ctr3(3, a, t), A.rk);
-                                const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
-                                const uint2 *tt = thr + t * 14;
-#pragma unroll
-                                for (int e = 0; e < 4; ++e) {
-                                    const uint32_t idx = (cw[e] >> (4 * t8)) & 15u;
-                                    const uint2 th = tt[idx];            // nibble = a + 2 n_u = index into thr[t][n_u][a]
-                                    const bool flip = th.y != 0u || rr[e] < th.x;                  // (uint64) r < thr
-                                    acc[e] |= flip ? (1u << tl) : 0u;
-                                }
-                            }
+                        for (int e = 0; e < 4; ++e) {
+                            const uint2 th = tt[(cw[e] >> (4 * t8)) & 15u];      // nibble = a + 2 n_u = index into thr[t][n_u][a]
+                            const bool flip = th.y != 0u || rr[e] < th.x;         // (uint64) r < thr
+                            acc[e] |= flip ? (1u << t8) : 0u;
                         }
                     }
-                    reinterpret_cast<uint4 *>(Sa)[q] = make_uint4(sp[0] ^ acc[0], sp[1] ^ acc[1], sp[2] ^ acc[2], sp[3] ^ acc[3]);
                 }
+#pragma unroll
+                for (int e = 0; e < 4; ++e)
+                    if (acc[e]) atomicXor(&Sa[4 * q + e], acc[e] << tb);
+              }
             }
-            __syncwarp();
+            __syncthreads();
         }
-        // ---- exchange step (R12): per-bit energies, decisions by the lane of the lower slot, bit permutation
+        // ---- exchange step (R12): per-bit energies, decisions by the lane of the lower slot (warp 0), bit permutation
         if (A.pt_every > 0 && (sweep + 1) % (uint64_t)A.pt_every == 0) {
+            if (tid < 4 * 32) UM[tid] = 0;
+            __syncthreads();
             for (int j = 0; j < NW; ++j) {
                 const uint32_t *s0 = S + (size_t)j * N, *s1 = s0 + H;
-                uint32_t bigU[14], bigM[13], inU[7], inM[6];
+                uint32_t bigU[10], bigM[8], inU[7], inM[6];              // per thread: <= ceil(H / 256) = 8 sites -> U <= 48, M <= 16
 #pragma unroll
-                for (int k = 0; k < 14; ++k) bigU[k] = 0;
+                for (int k = 0; k < 10; ++k) bigU[k] = 0;
 #pragma unroll
-                for (int k = 0; k < 13; ++k) bigM[k] = 0;
+                for (int k = 0; k < 8; ++k) bigM[k] = 0;
 #pragma unroll
                 for (int k = 0; k < 7; ++k) inU[k] = 0;
 #pragma unroll
                 for (int k = 0; k < 6; ++k) inM[k] = 0;
                 int pending = 0;
-                for (int n = lane; n < H; n += 32) {                     // the six bonds of every colour-0 site cover each bond once
+                for (int n = tid; n < H; n += nthr) {                    // the six bonds of every colour-0 site cover each bond once
                     int ix[6];
                     nbr6<L>(0, n, ix);
                     const uint32_t sa = s0[n], sb = s1[n], jb = Jb[n];
@@ -214,85 +216,93 @@ __global__ void __launch_bounds__(128) k_tp_run(const __grid_constant__ TpArgs A
                 }
                 bs_add(bigU, inU);
                 bs_add(bigM, inM);
-                Ureg[j] = (int)bs_warp_total(bigU, 14, lane);
-                Mreg[j] = 2 * (int)bs_warp_total(bigM, 13, lane) - N;
+                atomicAdd(&UM[j * 32 + lane], (int)bs_warp_total(bigU, 10, lane));
+                atomicAdd(&UM[64 + j * 32 + lane], (int)bs_warp_total(bigM, 8, lane));
             }
+            __syncthreads();
             const int e1 = (int)(exchange & 1u);
-            uint32_t mask[2] = {0u, 0u};
-            for (int j = 0; j < NW; ++j) {
-                const int t = 32 * j + lane;
-                // partner = slot t + 1: the next lane, or lane 0 of the next word
-                int Up = __shfl_down_sync(0xffffffffu, Ureg[j], 1), Mp = __shfl_down_sync(0xffffffffu, Mreg[j], 1);
-                if (j + 1 < NW) {
-                    const int U0 = __shfl_sync(0xffffffffu, Ureg[j + 1], 0), M0 = __shfl_sync(0xffffffffu, Mreg[j + 1], 0);
-                    if (lane == 31) { Up = U0; Mp = M0; }
+            if (warp == 0) {
+                int Ureg[2], Mreg[2];
+                uint32_t mask[2] = {0u, 0u};
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    Ureg[j] = j < NW ? UM[j * 32 + lane] : 0;
+                    Mreg[j] = j < NW ? 2 * UM[64 + j * 32 + lane] - N : 0;
                 }
-                bool accept = false;
-                if ((t & 1) == e1 && t + 1 < NT) {
-                    const double Et = __dsub_rn((double)(2 * Ureg[j] - 3 * N), __dmul_rn(A.h, (double)Mreg[j]));
-                    const double Eu = __dsub_rn((double)(2 * Up - 3 * N), __dmul_rn(A.h, (double)Mp));
-                    const double x = __dmul_rn(__dsub_rn(A.tab[t].beta, A.tab[t + 1].beta), __dsub_rn(Et, Eu));
-                    const uint4 r = philox_rk8(0u, (uint32_t)exchange, sglob, ctr3(4, a, t), A.rk);
-                    accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    if (j >= NW) continue;
+                    const int t = 32 * j + lane;
+                    // partner = slot t + 1: the next lane, or lane 0 of the next word
+                    int Up = __shfl_down_sync(0xffffffffu, Ureg[j], 1), Mp = __shfl_down_sync(0xffffffffu, Mreg[j], 1);
+                    if (j == 0) {
+                        const int U0 = __shfl_sync(0xffffffffu, Ureg[1], 0), M0 = __shfl_sync(0xffffffffu, Mreg[1], 0);
+                        if (lane == 31) { Up = U0; Mp = M0; }
+                    }
+                    bool accept = false;
+                    if ((t & 1) == e1 && t + 1 < NT) {
+                        const double Et = __dsub_rn((double)(2 * Ureg[j] - 3 * N), __dmul_rn(A.h, (double)Mreg[j]));
+                        const double Eu = __dsub_rn((double)(2 * Up - 3 * N), __dmul_rn(A.h, (double)Mp));
+                        const double x = __dmul_rn(__dsub_rn(A.tab[t].beta, A.tab[t + 1].beta), __dsub_rn(Et, Eu));
+                        const uint4 r = philox_rk8(0u, (uint32_t)exchange, sglob, ctr3(4, a, t), A.rk);
+                        accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
+                    }
+                    mask[j] = __ballot_sync(0xffffffffu, accept);
+                    cnt[j] += accept ? 1u : 0u;
                 }
-                mask[j] = __ballot_sync(0xffffffffu, accept);
-                cnt[j] += accept ? 1u : 0u;
+                if (lane < 2) masks[lane] = mask[lane];
+                if (sw == A.n_sweeps - 1) {                              // publish the kernel's own energies, permuted like the configurations
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        if (j >= NW) continue;
+                        const int Ud = __shfl_down_sync(0xffffffffu, Ureg[j], 1), Md = __shfl_down_sync(0xffffffffu, Mreg[j], 1);
+                        const int Uu = __shfl_up_sync(0xffffffffu, Ureg[j], 1), Mu = __shfl_up_sync(0xffffffffu, Mreg[j], 1);
+                        const int Ux = __shfl_sync(0xffffffffu, Ureg[j ^ 1], j == 0 ? 0 : 31), Mx = __shfl_sync(0xffffffffu, Mreg[j ^ 1], j == 0 ? 0 : 31);
+                        int Un = Ureg[j], Mn = Mreg[j];
+                        if (lane < 31 && ((mask[j] >> lane) & 1u)) { Un = Ud; Mn = Md; }
+                        if (lane > 0 && ((mask[j] >> (lane - 1)) & 1u)) { Un = Uu; Mn = Mu; }
+                        if (NW == 2 && (mask[0] >> 31) && ((j == 0 && lane == 31) || (j == 1 && lane == 0))) { Un = Ux; Mn = Mx; }
+                        const int t = 32 * j + lane;
+                        if (t < NT) {
+                            const size_t o = ((size_t)s * d.R + a) * NT + t;
+                            A.U[o] = (int64_t)Un;
+                            A.M[o] = Mn;
+                        }
+                    }
+                }
             }
-            // energies follow their configurations
-            for (int j = 0; j < NW; ++j) {
-                const int Ud = __shfl_down_sync(0xffffffffu, Ureg[j], 1), Md = __shfl_down_sync(0xffffffffu, Mreg[j], 1);
-                const int Uu = __shfl_up_sync(0xffffffffu, Ureg[j], 1), Mu = __shfl_up_sync(0xffffffffu, Mreg[j], 1);
-                int Un = Ureg[j], Mn = Mreg[j];
-                if (lane < 31 && ((mask[j] >> lane) & 1u)) { Un = Ud; Mn = Md; }
-                if (lane > 0 && ((mask[j] >> (lane - 1)) & 1u)) { Un = Uu; Mn = Mu; }
-                Ureg[j] = Un;
-                Mreg[j] = Mn;
-            }
-            if (NW == 2 && (mask[0] >> 31)) {                            // pair (31, 32) swapped: lane 31 of word 0 <-> lane 0 of word 1
-                const int U31 = __shfl_sync(0xffffffffu, Ureg[0], 31), M31 = __shfl_sync(0xffffffffu, Mreg[0], 31);
-                const int U32 = __shfl_sync(0xffffffffu, Ureg[1], 0), M32 = __shfl_sync(0xffffffffu, Mreg[1], 0);
-                if (lane == 31) { Ureg[0] = U32; Mreg[0] = M32; }
-                if (lane == 0) { Ureg[1] = U31; Mreg[1] = M31; }
-            }
+            __syncthreads();
             // bit permutation of every site word: swap bits (tl, tl + 1) for the accepted lower slots tl
             for (int j = 0; j < NW; ++j) {
-                const uint32_t m = mask[j] & 0x7fffffffu;
-                if (m == 0u) continue;                                   // warp-uniform
+                const uint32_t m = masks[j] & 0x7fffffffu;
+                if (m == 0u) continue;                                   // block-uniform
                 uint32_t *Sj = S + (size_t)j * N;
-                for (int n = lane; n < N; n += 32) {
+                for (int n = tid; n < N; n += nthr) {
                     const uint32_t x = Sj[n];
                     const uint32_t tt = ((x >> 1) ^ x) & m;
                     Sj[n] = x ^ tt ^ (tt << 1);
                 }
             }
-            if (NW == 2 && (mask[0] >> 31)) {
-                for (int n = lane; n < N; n += 32) {
+            if (NW == 2 && (masks[0] >> 31)) {                           // pair (31, 32): bit 31 of word 0 <-> bit 0 of word 1
+                for (int n = tid; n < N; n += nthr) {
                     const uint32_t x = S[n], y = S[N + n];
                     const uint32_t dd = ((x >> 31) ^ y) & 1u;
                     S[n] = x ^ (dd << 31);
                     S[N + n] = y ^ dd;
                 }
             }
-            __syncwarp();
-            if (sw == A.n_sweeps - 1) {                                  // publish the kernel's own energies (post-swap)
-                for (int j = 0; j < NW; ++j) {
-                    const int t = 32 * j + lane;
-                    if (t < NT) {
-                        const size_t o = ((size_t)s * d.R + a) * NT + t;
-                        A.U[o] = (int64_t)Ureg[j];
-                        A.M[o] = Mreg[j];
-                    }
-                }
-            }
             exchange += 1;
+            __syncthreads();
         }
     }
-    for (int j = 0; j < NW; ++j) {
-        const int t = 32 * j + lane;
-        if (t < NT && cnt[j]) atomicAdd(&A.pt_acc[t], (unsigned long long)cnt[j]);
+    if (warp == 0) {
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int t = 32 * j + lane;
+            if (j < NW && t < NT && cnt[j]) atomicAdd(&A.pt_acc[t], (unsigned long long)cnt[j]);
+        }
     }
-    __syncwarp();
-    for (int i = lane; i < NW * N / 4; i += 32) reinterpret_cast<uint4 *>(gS)[i] = reinterpret_cast<const uint4 *>(S)[i];
+    for (int i = tid; i < NW * N / 4; i += nthr) reinterpret_cast<uint4 *>(gS)[i] = reinterpret_cast<const uint4 *>(S)[i];
 }
 
 // ------------------------------------------------------------------------ layout conversion
@@ -362,28 +372,24 @@ k_tp_pack_J(Dims d, const uint32_t *__restrict__ J, uint8_t *__restrict__ J6)
     J6[tid] = (uint8_t)b;
 }
 
-size_t tp_smem(int L, int NT, int wpb)
+size_t tp_smem(int L, int NT)
 {
     const size_t N = (size_t)L * L * L;
     const int NW = (NT + 31) / 32;
-    return (size_t)NT * 14 * 8 + 1024 + (size_t)wpb * ((size_t)NW * N * 4 + ((N + 15) & ~(size_t)15));
-}
-
-int tp_wpb(int L, int NT, int R)
-{
-    for (int wpb = 4; wpb >= 1; wpb >>= 1)
-        if (tp_smem(L, NT, wpb) <= (size_t)227 * 1024) return wpb;
-    return 0;
+    return (size_t)NT * 14 * 8 + 1024 + (size_t)NW * N * 4 + 4 * 32 * 4 + 16 + N;
 }
 
 template <int L>
 cudaError_t launch_tp(sg_ctx *c, const TpArgs &A, size_t smem, int grid)
 {
     if (attr_needed(c, ATTR_TPACK + L / 2 - 2)) {        // L = 4..16 -> ids 24..30
-        cudaError_t e = cudaFuncSetAttribute(k_tp_run<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(k_tp_run<L, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(k_tp_run<L, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
     }
-    k_tp_run<L><<<grid, 128, smem, c->stream>>>(A);
+    if (grid >= 148 * 6) k_tp_run<L, 32><<<grid, TP_THREADS, smem, c->stream>>>(A);      // enough lattices to fill every SM
+    else k_tp_run<L, 8><<<grid, TP_THREADS, smem, c->stream>>>(A);
     return cudaGetLastError();
 }
 
@@ -396,7 +402,7 @@ bool tp_supported(const sg_ctx *c)
     const Dims &d = c->d;
     if (c->kind != SG_PMJ_TPACK || c->path != SG_PATH_AUTO) return false;
     if (d.L != 4 && d.L != 6 && d.L != 8 && d.L != 10 && d.L != 12 && d.L != 16) return false;
-    return tp_wpb(d.L, d.NT, d.R) > 0;
+    return tp_smem(d.L, d.NT) <= (size_t)227 * 1024;
 }
 
 int launch_tp_pack_J(sg_ctx *c)
@@ -445,14 +451,12 @@ int launch_tp_run(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0, 
     A.n_sweeps = n_sweeps;
     A.pt_every = pt_every;
     A.NW = (d.NT + 31) / 32;
-    A.wpb = tp_wpb(d.L, d.NT, d.R);
+    A.wpb = 1;
     A.U = c->U;
     A.M = c->M;
     A.pt_acc = c->pt_acc;
-    if (A.wpb <= 0) return -1;
-    const size_t smem = tp_smem(d.L, d.NT, A.wpb);
-    const long long lattices = (long long)d.n_samples * d.R;
-    const int grid = (int)((lattices + A.wpb - 1) / A.wpb);
+    const size_t smem = tp_smem(d.L, d.NT);
+    const int grid = d.n_samples * d.R;
     cudaError_t e;
     switch (d.L) {
     case 4: e = launch_tp<4>(c, A, smem, grid); break;
