@@ -33,6 +33,7 @@ struct LadderArgs {
     int64_t *U;               // the kernel's own energies after the last exchange of the launch (see sg_ladder8.cu)
     int32_t *M;
     unsigned long long *pt_acc;
+    int use_tab;              // shared memory has room for the energy tables (neighbour indices + gathered couplings)
 };
 
 __device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -146,6 +147,80 @@ __device__ __forceinline__ void ladder_energy(const uint32_t *__restrict__ Ssys,
     M = 2 * (int)bs_warp_total(bigM, pm, lane) - N;
 }
 
+// The same recount with everything that does not depend on the system taken from two tables built once per launch:
+// idxT[n] = the six neighbour indices of colour-0 site n (16 bits each), JgT[n] = its six coupling words in the same
+// order (+x, -x, +y, -y, +z, -z); four sites per step, their counts summed by a small adder tree before they are
+// added to the running bit-sliced totals.  ~2.3x fewer instructions per site than ladder_energy.
+template <int L>
+__device__ __forceinline__ void ladder_energy_tab(const uint32_t *__restrict__ Ssys, const uint4 *__restrict__ idxT,
+                                                  const uint32_t *__restrict__ JgT, int lane, int &U, int &M)
+{
+    constexpr int N = L * L * L, H = N / 2;
+    // per thread: at most ceil(H / 32) sites -> U <= 6 sites, spin count <= 2 sites: just enough planes
+    constexpr int SPT = (H + 31) / 32;
+    constexpr int PU = SPT * 6 < 8 ? 3 : SPT * 6 < 16 ? 4 : SPT * 6 < 32 ? 5 : SPT * 6 < 64 ? 6 : SPT * 6 < 128 ? 7 : SPT * 6 < 256 ? 8 : 9;
+    constexpr int PM = SPT * 2 < 8 ? 3 : SPT * 2 < 16 ? 4 : SPT * 2 < 32 ? 5 : SPT * 2 < 64 ? 6 : SPT * 2 < 128 ? 7 : 8;
+    static_assert(SPT * 6 < 512 && SPT * 2 < 256, "plane counts");
+    const uint32_t *s0 = Ssys, *s1 = Ssys + H;
+    uint32_t bigU[PU], bigM[PM];
+#pragma unroll
+    for (int k = 0; k < PU; ++k) bigU[k] = 0;
+#pragma unroll
+    for (int k = 0; k < PM; ++k) bigM[k] = 0;
+    for (int n0 = lane; n0 < H; n0 += 128) {
+        uint32_t w[4][3], sw[8];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int n = n0 + 32 * e;
+            if (n < H) {
+                const uint4 ii = idxT[n];
+                const uint2 j01 = *reinterpret_cast<const uint2 *>(JgT + 6 * n);
+                const uint2 j23 = *reinterpret_cast<const uint2 *>(JgT + 6 * n + 2);
+                const uint2 j45 = *reinterpret_cast<const uint2 *>(JgT + 6 * n + 4);
+                const uint32_t sa = s0[n];
+                const uint32_t u0 = xor3(sa, s1[ii.x & 0xffffu], j01.x), u1 = xor3(sa, s1[ii.x >> 16], j01.y);
+                const uint32_t u2 = xor3(sa, s1[ii.y & 0xffffu], j23.x), u3 = xor3(sa, s1[ii.y >> 16], j23.y);
+                const uint32_t u4 = xor3(sa, s1[ii.z & 0xffffu], j45.x), u5 = xor3(sa, s1[ii.z >> 16], j45.y);
+                const uint32_t a0 = xor3(u0, u1, u2), c0 = maj3(u0, u1, u2);
+                const uint32_t a1 = xor3(u3, u4, u5), c1 = maj3(u3, u4, u5);
+                const uint32_t kk = a0 & a1;
+                w[e][0] = a0 ^ a1;
+                w[e][1] = xor3(c0, c1, kk);
+                w[e][2] = maj3(c0, c1, kk);
+                sw[2 * e] = sa;
+                sw[2 * e + 1] = s1[n];
+            } else {
+                w[e][0] = w[e][1] = w[e][2] = 0u;
+                sw[2 * e] = sw[2 * e + 1] = 0u;
+            }
+        }
+        uint32_t ab[4], cd[4], U5[5];
+        bs_sum<3>(w[0], w[1], ab);
+        bs_sum<3>(w[2], w[3], cd);
+        bs_sum<4>(ab, cd, U5);
+        if constexpr (PU >= 5) bs_add(bigU, U5);
+        else {
+#pragma unroll
+            for (int k = 0; k < PU; ++k) bigU[k] = U5[k];               // L = 4: one group only
+        }
+        // 8 spin words -> 4 planes
+        const uint32_t x1 = xor3(sw[0], sw[1], sw[2]), y1 = maj3(sw[0], sw[1], sw[2]);
+        const uint32_t x2 = xor3(sw[3], sw[4], sw[5]), y2 = maj3(sw[3], sw[4], sw[5]);
+        const uint32_t x3 = xor3(x1, x2, sw[6]), y3 = maj3(x1, x2, sw[6]);
+        const uint32_t ones = x3 ^ sw[7], y4 = x3 & sw[7];
+        const uint32_t t1 = xor3(y1, y2, y3), f1 = maj3(y1, y2, y3);
+        const uint32_t twos = t1 ^ y4, f2 = t1 & y4;
+        const uint32_t M4[4] = {ones, twos, f1 ^ f2, f1 & f2};
+        if constexpr (PM >= 4) bs_add(bigM, M4);
+        else {
+#pragma unroll
+            for (int k = 0; k < PM; ++k) bigM[k] = M4[k];
+        }
+    }
+    U = (int)bs_warp_total(bigU, PU, lane);
+    M = 2 * (int)bs_warp_total(bigM, PM, lane) - N;
+}
+
 template <int L, bool BS>
 __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const __grid_constant__ LadderArgs A)
 {
@@ -161,6 +236,9 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     int *Mint = Uint + NT * 32;                           // [NT][32]
     uint32_t *masks = reinterpret_cast<uint32_t *>(Mint + NT * 32);   // [NT / 2 + 1]
     uint32_t *accs = masks + (NT / 2 + 1);                // [NT] accepted swaps of this CTA per lower slot
+    // energy tables (use_tab): 16-byte aligned behind the scratch above
+    uint4 *idxT = reinterpret_cast<uint4 *>((reinterpret_cast<uintptr_t>(accs + NT) + 15) & ~(uintptr_t)15);   // [H]
+    uint32_t *JgT = reinterpret_cast<uint32_t *>(idxT + H);                                                     // [H][6]
 
     const int w = blockIdx.x / d.R, a = blockIdx.x % d.R;
     const int tid = threadIdx.x, nthr = blockDim.x;
@@ -191,6 +269,25 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
         for (int t = tid; t < NT; t += nthr) accs[t] = 0u;
     }
     __syncthreads();
+    if (A.use_tab && A.pt_every > 0) {                    // neighbour indices and couplings of the colour-0 sites, once per launch
+        const uint32_t *J0 = Jsm, *J1 = Jsm + 3 * H;
+        for (int n = tid; n < H; n += nthr) {
+            const int row = n / Lh, m = n - row * Lh;
+            const int z = row / L, y = row - z * L;
+            const int p = (y + z) & 1;
+            const int sd = row * Lh + (p ? (m + 1 == Lh ? 0 : m + 1) : (m == 0 ? Lh - 1 : m - 1));
+            const int xp = p ? sd : n, xm = p ? n : sd;
+            const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m, ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
+            const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m, zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
+            idxT[n] = make_uint4((uint32_t)xp | ((uint32_t)xm << 16), (uint32_t)yp | ((uint32_t)ym << 16),
+                                 (uint32_t)zp | ((uint32_t)zm << 16), 0u);
+            uint32_t *g = JgT + 6 * n;
+            g[0] = J0[n];          g[1] = J1[xm];
+            g[2] = J0[H + n];      g[3] = J1[H + ym];
+            g[4] = J0[2 * H + n];  g[5] = J1[2 * H + zm];
+        }
+        __syncthreads();
+    }
 
     const int q = tid % Q, g = tid / Q;
     const bool active = g < A.G;
@@ -359,7 +456,8 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
             const int lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
             for (int t = warp; t < NT; t += nwarp) {
                 int U, M;
-                ladder_energy<L>(S + t * N, Jsm, lane, U, M);
+                if (A.use_tab) ladder_energy_tab<L>(S + t * N, idxT, JgT, lane, U, M);
+                else ladder_energy<L>(S + t * N, Jsm, lane, U, M);
                 Uint[t * 32 + lane] = U;
                 Mint[t * 32 + lane] = M;
             }
@@ -430,6 +528,9 @@ size_t ladder_smem_bytes(int L, int NT)
     return (size_t)NT * N * 4 + 3 * N * 4 + (size_t)NT * 8 * sizeof(uint2) + (size_t)NT * 32 * 8 + (size_t)(NT / 2 + 1) * 4 + (size_t)NT * 4;
 }
 
+// + the energy tables of ladder_energy_tab: 16 (indices) + 24 (couplings) bytes per colour-0 site, 16-byte aligned
+static size_t ladder_tab_bytes(int L) { return 16 + (size_t)(L * L * L / 2) * 40; }
+
 bool ladder_supported(const sg_ctx *c)
 {
     const Dims &d = c->d;
@@ -487,7 +588,9 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchang
     A.G = G;
     int threads = (Q * G + 31) / 32 * 32;
     if (threads > maxt) return -1;
-    const size_t smem = ladder_smem_bytes(d.L, d.NT);
+    size_t smem = ladder_smem_bytes(d.L, d.NT);
+    A.use_tab = smem + ladder_tab_bytes(d.L) <= (size_t)227 * 1024 ? 1 : 0;
+    if (A.use_tab) smem += ladder_tab_bytes(d.L);
     const int grid = d.W * d.R;
     cudaError_t e;
     switch (d.L) {
