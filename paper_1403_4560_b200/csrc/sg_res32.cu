@@ -203,8 +203,8 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
     uint4 *S4 = reinterpret_cast<uint4 *>(smem);                           // [2][RQ]                  128 KB
     uint4 *ring = S4 + 2 * RQ;                                             // [16 warps][2 stages][6][32] 96 KB
     uint64_t *bars = reinterpret_cast<uint64_t *>(ring + R_WARPS * N_STAGES * CHUNK_U4);   // [16][2]
-    uint64_t *sysbar_p = bars + R_WARPS * N_STAGES;                        // load barrier of the system
-    int *sUM = reinterpret_cast<int *>(sysbar_p + 1);                      // [2][32], then [64]: swap mask of this CTA
+    uint64_t *sysbar_p = bars + R_WARPS * N_STAGES;                        // [8] load barriers of the system: one per 16 KB chunk
+    int *sUM = reinterpret_cast<int *>(sysbar_p + 8);                      // [2][32], then [64]: swap mask of this CTA
     const Dims &d = A.d;
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);        // warp-uniform for the compiler: uniform datapath
@@ -232,18 +232,18 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
         issue(0, 1);
     }
 
-    // ---- load the system (contiguous 128 KB): eight 16 KB bulk-async copies on one mbarrier
+    // ---- load the system (contiguous 128 KB): eight 16 KB bulk-async copies, each on its own mbarrier, issued in the
+    // order the first half sweep needs them (chunk k = colour k >> 2, planes 8 (k & 3) .. 8 (k & 3) + 7): the first
+    // warp steps start as soon as their three chunks have landed instead of after the whole system
     const uint32_t sysbar = smem_u32(sysbar_p);
     if (tid == 0) {
-        mbar_init(sysbar, 1);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) mbar_init(sysbar + 8 * i, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(sysbar), "r"(RN * 4) : "memory");
+        constexpr int order[8] = {0, 4, 7, 5, 1, 6, 2, 3};
 #pragma unroll
         for (int i = 0; i < 8; ++i)
-            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                             S_s + i * 16384),
-                         "l"(reinterpret_cast<const char *>(gS) + i * 16384), "r"(16384), "r"(sysbar)
-                         : "memory");
+            bulk_load(S_s + order[i] * 16384, reinterpret_cast<const char *>(gS) + order[i] * 16384, 16384, sysbar + 8 * order[i]);
     }
     if (tid < 64) sUM[tid] = 0;
     // ---- pending exchange: decide the swap of this slot's pair (warp 0; lane l = sample 32 w + l)
@@ -280,21 +280,19 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
     const uint32_t c3 = ctr3(3, a, t);
     const Geo32 geo = geo_of(wj, lane);
     const int pi = (wj >> 2) & 1;
-    __syncthreads();                                        // sysbar initialised, sUM zeroed, swap mask known
-    mbar_wait(sysbar, 0u);                                  // the system has landed (async-proxy writes visible)
+    __syncthreads();                                        // barriers initialised, sUM zeroed, swap mask known
     {
         const uint32_t xmask = (uint32_t)sUM[64];           // block-uniform
         if (xmask) {                                        // swap on load: take the partner's bits in the swapping lanes
+#pragma unroll
+            for (int i = 0; i < 8; ++i) mbar_wait(sysbar + 8 * i, 0u);     // the whole system has landed
             const uint4 *gP = reinterpret_cast<const uint4 *>(A.spins_in + (size_t)(sys - t + partner) * RN);
+            constexpr int LUT_SEL = (0xF0 & 0x55) | (0xCC & 0xAA);           // c ? b : a
 #pragma unroll 4
             for (int i = tid; i < 2 * RQ; i += R_THREADS) {
-                uint4 v = S4[i];
-                const uint4 pv = gP[i];
-                v.x ^= (v.x ^ pv.x) & xmask;
-                v.y ^= (v.y ^ pv.y) & xmask;
-                v.z ^= (v.z ^ pv.z) & xmask;
-                v.w ^= (v.w ^ pv.w) & xmask;
-                S4[i] = v;
+                const uint4 v = S4[i], pv = gP[i];
+                S4[i] = make_uint4(lop3<LUT_SEL>(v.x, pv.x, xmask), lop3<LUT_SEL>(v.y, pv.y, xmask),
+                                   lop3<LUT_SEL>(v.z, pv.z, xmask), lop3<LUT_SEL>(v.w, pv.w, xmask));
             }
             __syncthreads();
         }
@@ -314,6 +312,12 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
 #pragma unroll 1
         for (int it = 0; it < R_ITERS; ++it) {
             const int st = it & 1;
+            if (hs == 0) {                                  // first half sweep (colour 0): the chunks this step touches have landed?
+                const int Z = 2 * it + zhalf;
+                mbar_wait(sysbar + 8u * (uint32_t)(Z >> 2), 0u);                             // colour 0, planes 2 Z, 2 Z + 1
+                mbar_wait(sysbar + 8u * (uint32_t)(4 + (((2 * Z + 31) & 31) >> 3)), 0u);     // colour 1, plane 2 Z - 1
+                mbar_wait(sysbar + 8u * (uint32_t)(4 + (((2 * Z + 2) & 31) >> 3)), 0u);      // colour 1, plane 2 Z + 2
+            }
             mbar_wait(bar_s + st * 8, (uint32_t)(it >> 1) & 1u);      // use (8 hs + it) / 2 of the stage: parity = bit 1 of it
             const uint32_t jc = ring_s + st * CHUNK_BYTES + lane * 16;
             Quad6 Jq;
@@ -404,7 +408,7 @@ __global__ void __launch_bounds__(256) k_pack_J_res32(Dims d, const uint32_t *__
     Jp[idx] = make_uint4(v[0], v[1], v[2], v[3]);
 }
 
-constexpr size_t RES32_SMEM = (size_t)RN * 4 + (size_t)R_WARPS * N_STAGES * CHUNK_BYTES + R_WARPS * N_STAGES * 8 + 8 + 68 * 4;
+constexpr size_t RES32_SMEM = (size_t)RN * 4 + (size_t)R_WARPS * N_STAGES * CHUNK_BYTES + R_WARPS * N_STAGES * 8 + 8 * 8 + 68 * 4;
 
 }  // namespace
 
