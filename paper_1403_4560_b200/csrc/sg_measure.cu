@@ -214,16 +214,22 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
     if (tid < 2 * L) twsm[tid] = tw[tid];
     __syncthreads();
 
-    // ---- phase 0: D = S^a xor S^b, canonical order
-    for (int item = tid; item < P * N; item += nthr) {
-        const int pair = item / N, k = item - pair * N;            // k = colour * H + n
+    // ---- phase 0: D = S^a xor S^b, canonical order (every replica's word is loaded once and used by all its pairs)
+    for (int k = tid; k < N; k += nthr) {                              // k = colour * H + n
         const int c = k / H, n = k - c * H;
         const int row = n / Lh, m = n - row * Lh;
         const int z = row / L, y = row - z * L;
         const int x = 2 * m + ((c + y + z) & 1);
-        const uint32_t *A = spins + (((size_t)w * d.R + pa[pair]) * d.NT + t) * N;
-        const uint32_t *B = spins + (((size_t)w * d.R + pb[pair]) * d.NT + t) * N;
-        Dsm[pair * N + x + L * (y + L * z)] = A[k] ^ B[k];
+        const int site = x + L * (y + L * z);
+        uint32_t sr[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+            sr[a] = a < d.R ? spins[(((size_t)w * d.R + a) * d.NT + t) * N + k] : 0u;
+#pragma unroll
+        for (int pair = 0; pair < 6; ++pair) {
+            constexpr int PA[6] = {0, 0, 0, 1, 1, 2}, PB[6] = {1, 2, 3, 2, 3, 3};
+            if (pair < P) Dsm[pair * N + site] = sr[PA[pair]] ^ sr[PB[pair]];
+        }
     }
     for (int i = tid; i < P * C::PLW; i += nthr) PL[i] = 0u;
     __syncthreads();
@@ -407,8 +413,10 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
         if (s >= d.n_samples) continue;
         const size_t o = ((size_t)s * d.NT + t) * SG_NMOM + j;
         const double v = OUT[l * OUT_LD + j];
-        mo.acc[o] += v;
-        if (mo.acc_win) mo.acc_win[o] += v;
+        // one addition per address and launch: the reduction instruction gives the same result as load-add-store
+        // without waiting for the load
+        atomicAdd(&mo.acc[o], v);
+        if (mo.acc_win) atomicAdd(&mo.acc_win[o], v);
     }
 }
 
