@@ -158,64 +158,76 @@ __global__ void __launch_bounds__(512, 1) k_gladder(const __grid_constant__ GLad
         }
         // ---- exchange step (R12, R14), all in shared memory
         if (A.pt_every > 0 && ((uint64_t)A.sweep0 + (uint64_t)sw + 1) % (uint64_t)A.pt_every == 0) {
-            // Energies: threads stride over the colour-0 sites (their six bonds cover every bond once); the six
-            // fixed-point couplings of a site are converted once and used for a chunk of 16 systems, whose partial
-            // sums live in registers; warp shuffle + one shared-memory atomic per (warp, system) finish the sums.
+            // Energies (R14): thread (q, g) — the mapping of the sweep — takes the quad q of colour 0 (the six bonds of every
+            // colour-0 site cover each bond once) for its systems t = g, g + G, ...  The 24 fixed-point couplings of the quad
+            // are converted once and stay in registers; per system the spins come as six words, a bond's contribution is
+            // selected by the sign byte of S_i xor S_j (one PRMT), and only D = sum over the DIFFERING bonds is accumulated:
+            // E_fix = -sum J S_i S_j = 2 D - sum J.  Exact in int64 in any order.  One warp shuffle reduction and one
+            // shared-memory atomic per (warp, system) finish the sums.
             const int lane = tid & 31;
-            const float *J0 = Jsm, *J1 = Jsm + 3 * H;
             for (int t = tid; t < NT; t += nthr) { Efix[t] = 0; Msum[t] = 0; }
             __syncthreads();
-            constexpr int TCH = 16;
-            for (int t0 = 0; t0 < NT; t0 += TCH) {
-                long long acc[TCH];
-                int mm[TCH];
+            if (active) {
+                const float *Jown = Jsm, *Joth = Jsm + 3 * H;                          // colour 0
+                const int r = q / QR, kq = q % QR;
+                const int y = r % L, z = r / L;
+                const int p = (y + z) & 1;
+                const int q_yp = (y + 1 == L) ? q - (L - 1) * QR : q + QR;
+                const int q_ym = (y == 0) ? q + (L - 1) * QR : q - QR;
+                const int q_zp = (z + 1 == L) ? q - (L - 1) * L * QR : q + L * QR;
+                const int q_zm = (z == 0) ? q + (L - 1) * L * QR : q - L * QR;
+                const int m_out = p ? (4 * kq + 4 == Lh ? 0 : 4 * kq + 4) : (kq == 0 ? Lh - 1 : 4 * kq - 1);
+                const int side_idx = r * Lh + m_out;
+                long long jf[6][4], jtot = 0;                                          // [+x, -x, +y, -y, +z, -z][element]
+                {
+                    const float4 jx = reinterpret_cast<const float4 *>(Jown)[q];
+                    const float4 jox = reinterpret_cast<const float4 *>(Joth)[q];
+                    const float4 jy = reinterpret_cast<const float4 *>(Jown + H)[q];
+                    const float4 joy = reinterpret_cast<const float4 *>(Joth + H)[q_ym];
+                    const float4 jz = reinterpret_cast<const float4 *>(Jown + 2 * H)[q];
+                    const float4 joz = reinterpret_cast<const float4 *>(Joth + 2 * H)[q_zm];
+                    const float jside = Joth[side_idx];
+                    const float Jv[6][4] = {{jx.x, jx.y, jx.z, jx.w},
+                                            {p ? jox.x : jside, p ? jox.y : jox.x, p ? jox.z : jox.y, p ? jox.w : jox.z},
+                                            {jy.x, jy.y, jy.z, jy.w}, {joy.x, joy.y, joy.z, joy.w},
+                                            {jz.x, jz.y, jz.z, jz.w}, {joz.x, joz.y, joz.z, joz.w}};
 #pragma unroll
-                for (int k = 0; k < TCH; ++k) { acc[k] = 0; mm[k] = 0; }
-                for (int n = tid; n < H; n += nthr) {
-                    const int row = n / Lh, mi = n - row * Lh;
-                    const int z = row / L, y = row - z * L;
-                    const int p = (y + z) & 1;
-                    const int sd = row * Lh + (p ? (mi + 1 == Lh ? 0 : mi + 1) : (mi == 0 ? Lh - 1 : mi - 1));
-                    const int xp = p ? sd : n, xm = p ? n : sd;
-                    const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + mi, ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + mi;
-                    const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + mi, zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + mi;
-                    const long long jf0 = __double2ll_rz(__dmul_rn((double)J0[n], 4294967296.0));
-                    const long long jf1 = __double2ll_rz(__dmul_rn((double)J1[xm], 4294967296.0));
-                    const long long jf2 = __double2ll_rz(__dmul_rn((double)J0[H + n], 4294967296.0));
-                    const long long jf3 = __double2ll_rz(__dmul_rn((double)J1[H + ym], 4294967296.0));
-                    const long long jf4 = __double2ll_rz(__dmul_rn((double)J0[2 * H + n], 4294967296.0));
-                    const long long jf5 = __double2ll_rz(__dmul_rn((double)J1[2 * H + zm], 4294967296.0));
+                    for (int k = 0; k < 6; ++k)
 #pragma unroll
-                    for (int k = 0; k < TCH; ++k) {
-                        const int t = t0 + k;
-                        if (t < NT) {
-                            const int8_t *s0 = S + (size_t)t * N, *s1 = s0 + H;
-                            const int si = s0[n];
-                            mm[k] += si + s1[n];
-                            long long a8 = 0;
-                            a8 += (si ^ s1[xp]) < 0 ? -jf0 : jf0;          // J_fix * S_i * S_j, S = +-1
-                            a8 += (si ^ s1[xm]) < 0 ? -jf1 : jf1;
-                            a8 += (si ^ s1[yp]) < 0 ? -jf2 : jf2;
-                            a8 += (si ^ s1[ym]) < 0 ? -jf3 : jf3;
-                            a8 += (si ^ s1[zp]) < 0 ? -jf4 : jf4;
-                            a8 += (si ^ s1[zm]) < 0 ? -jf5 : jf5;
-                            acc[k] -= a8;
+                        for (int e = 0; e < 4; ++e) {
+                            jf[k][e] = __double2ll_rz(__dmul_rn((double)Jv[k][e], 4294967296.0));
+                            jtot += jf[k][e];
                         }
-                    }
                 }
+#pragma unroll 1
+                for (int t = g; t < NT; t += A.G) {
+                    const uint32_t *Sa = S32 + ((size_t)t * N) / 4;                    // colour 0
+                    const uint32_t *So = S32 + ((size_t)t * N + H) / 4;
+                    const uint32_t sv = Sa[q];
+                    const uint32_t o0 = So[q], oyp = So[q_yp], oym = So[q_ym], ozp = So[q_zp], ozm = So[q_zm];
+                    const uint32_t sb = (uint32_t)(uint8_t)S[(size_t)t * N + H + side_idx];
+                    const uint32_t wxp = p ? ((o0 >> 8) | (sb << 24)) : o0;
+                    const uint32_t wxm = p ? o0 : ((o0 << 8) | sb);
+                    const uint32_t dw[6] = {sv ^ wxp, sv ^ wxm, sv ^ oyp, sv ^ oym, sv ^ ozp, sv ^ ozm};   // byte sign bit: S_i != S_j
+                    long long D = 0;
 #pragma unroll
-                for (int k = 0; k < TCH; ++k) {
-                    if (t0 + k < NT) {                                     // uniform
-                        long long e = acc[k];
-                        int m = mm[k];
-                        for (int o = 16; o; o >>= 1) {
-                            e += __shfl_xor_sync(0xffffffffu, e, o);
-                            m += __shfl_xor_sync(0xffffffffu, m, o);
+                    for (int k = 0; k < 6; ++k)
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            uint32_t m32;                                          // sign of byte e replicated over the word: -1 iff S_i != S_j
+                            asm("prmt.b32 %0, %1, %2, %3;" : "=r"(m32) : "r"(dw[k]), "r"(0u), "r"(0x8888u | (0x1111u * (unsigned)e)));
+                            const long long m = (long long)(int)m32;
+                            D += jf[k][e] & m;
                         }
-                        if (lane == 0) {
-                            atomicAdd(reinterpret_cast<unsigned long long *>(&Efix[t0 + k]), (unsigned long long)e);
-                            atomicAdd(&Msum[t0 + k], m);
-                        }
+                    long long ev = 2 * D - jtot;
+                    int mv = __dp4a((int)sv, 0x01010101, __dp4a((int)o0, 0x01010101, 0));
+                    for (int o = 16; o; o >>= 1) {
+                        ev += __shfl_xor_sync(0xffffffffu, ev, o);
+                        mv += __shfl_xor_sync(0xffffffffu, mv, o);
+                    }
+                    if (lane == 0) {
+                        atomicAdd(reinterpret_cast<unsigned long long *>(&Efix[t]), (unsigned long long)ev);
+                        atomicAdd(&Msum[t], mv);
                     }
                 }
             }
