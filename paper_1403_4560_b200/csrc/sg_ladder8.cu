@@ -46,12 +46,10 @@ constexpr int PW1 = PU1 + PM1;              // words per (system, thread) in the
 
 // 4:1 adder stage over the reduction buffer: in[sys][PU+PM][n_in] -> out[sys][PU+2+PM+2][n_in/4]
 template <int PU, int PM>
-__device__ __forceinline__ void reduce4(const uint32_t *__restrict__ in, uint32_t *__restrict__ out, int n_sys,
-                                        int n_in, int tid, int nthr)
+__device__ __forceinline__ void reduce4_item(const uint32_t *__restrict__ in, uint32_t *__restrict__ out, int sys, int n_in, int c)
 {
     const int n_out = n_in >> 2;
-    for (int item = tid; item < n_sys * n_out; item += nthr) {
-        const int sys = item / n_out, c = item - sys * n_out;
+    {
         const uint32_t *src = in + (size_t)sys * (PU + PM) * n_in + 4 * c;
         uint32_t a[PU], b[PU], ab[PU + 1], cd[PU + 1], u[PU + 2];
 #pragma unroll
@@ -76,6 +74,14 @@ __device__ __forceinline__ void reduce4(const uint32_t *__restrict__ in, uint32_
 #pragma unroll
         for (int k = 0; k < PM + 2; ++k) dst[(PU + 2 + k) * n_out] = m[k];
     }
+}
+
+template <int PU, int PM>
+__device__ __forceinline__ void reduce4(const uint32_t *__restrict__ in, uint32_t *__restrict__ out, int n_sys,
+                                        int n_in, int tid, int nthr)
+{
+    const int n_out = n_in >> 2;
+    for (int item = tid; item < n_sys * n_out; item += nthr) reduce4_item<PU, PM>(in, out, item / n_out, n_in, item % n_out);
 }
 
 template <int P, bool ENERGY, bool BS>
@@ -168,8 +174,6 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
     uint32_t *red1 = red0 + NT * PW1 * 64;                 // [NT][13][16]
     uint32_t *red2 = red0;                                 // [NT][17][4]   (red0 is dead after stage 2)
     uint32_t *red3 = red1;                                 // [NT][21][1]   (red1 is dead after stage 3)
-    int *Uint = reinterpret_cast<int *>(red0 + NT * 17 * 4);   // [NT][32]  (behind red2, inside red0's area)
-    int *Mint = Uint + NT * 32;                            // [NT][32]
 
     const int w = blockIdx.x / d.R, a = blockIdx.x % d.R;
     const int tid = threadIdx.x, nthr = blockDim.x;
@@ -284,62 +288,61 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
             __syncthreads();
             reduce4<9, 8>(red2, red3, NT, 4, tid, nthr);
             __syncthreads();
-            {
-                const int lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
-                for (int t = warp; t < NT; t += nwarp) {
-                    const uint32_t x = lane < 21 ? red3[t * 21 + lane] : 0u;      // 11 planes of U, 10 of M
-                    const uint32_t v = transpose32(x, lane);
-                    Uint[t * 32 + lane] = (int)(v & 0x7ffu);
-                    Mint[t * 32 + lane] = 2 * (int)((v >> 11) & 0x3ffu) - N;
-                }
-            }
-            __syncthreads();
-            // ---- decisions: one thread per (pair, lane)
+            // ---- decisions and swaps: one WARP per pair.  The warp turns the count planes of its two systems into per-lane
+            // integers itself (one bit transpose each), decides (lane l = sample 32 w + l) and, knowing the mask from its own
+            // ballot, swaps the two configurations at once — no transpose phase, no barrier between decision and swap.
             const int e1 = (int)(exchange & 1u);
             const int npairs = (NT - e1) / 2;
-            for (int item = tid; item < npairs * 32; item += nthr) {       // whole warps: npairs*32 is a multiple of 32
-                const int pair = item >> 5, lane = item & 31;
-                const int t = e1 + 2 * pair;
-                const int s = w * 32 + lane;
-                const int U0 = Uint[t * 32 + lane], U1 = Uint[(t + 1) * 32 + lane];
-                const int M0 = Mint[t * 32 + lane], M1 = Mint[(t + 1) * 32 + lane];
-                const double Et = __dsub_rn((double)(2 * U0 - 3 * N), __dmul_rn(A.h, (double)M0));
-                const double Eu = __dsub_rn((double)(2 * U1 - 3 * N), __dmul_rn(A.h, (double)M1));
-                const double x = __dmul_rn(__dsub_rn(A.tab[t].beta, A.tab[t + 1].beta), __dsub_rn(Et, Eu));
-                const uint4 r = philox_rk8(0u, (uint32_t)exchange, (uint32_t)(s + d.s_first), ctr3(4, a, t), A.rk);
-                const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
-                const uint32_t mask = __ballot_sync(0xffffffffu, accept && s < d.n_samples);
-                if (lane == 0) { masks[pair] = mask; accs[t] += (uint32_t)__popc(mask); }
+            {
+                const int lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
+                for (int pair = warp; pair < npairs; pair += nwarp) {
+                    const int t = e1 + 2 * pair;
+                    const int s = w * 32 + lane;
+                    const uint32_t v0 = transpose32(lane < 21 ? red3[t * 21 + lane] : 0u, lane);            // 11 planes of U, 10 of M
+                    const uint32_t v1 = transpose32(lane < 21 ? red3[(t + 1) * 21 + lane] : 0u, lane);
+                    const int U0 = (int)(v0 & 0x7ffu), U1 = (int)(v1 & 0x7ffu);
+                    const int M0 = 2 * (int)((v0 >> 11) & 0x3ffu) - N, M1 = 2 * (int)((v1 >> 11) & 0x3ffu) - N;
+                    const double Et = __dsub_rn((double)(2 * U0 - 3 * N), __dmul_rn(A.h, (double)M0));
+                    const double Eu = __dsub_rn((double)(2 * U1 - 3 * N), __dmul_rn(A.h, (double)M1));
+                    const double x = __dmul_rn(__dsub_rn(A.tab[t].beta, A.tab[t + 1].beta), __dsub_rn(Et, Eu));
+                    const uint4 r = philox_rk8(0u, (uint32_t)exchange, (uint32_t)(s + d.s_first), ctr3(4, a, t), A.rk);
+                    const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
+                    const uint32_t mask = __ballot_sync(0xffffffffu, accept && s < d.n_samples);
+                    if (lane == 0) { masks[pair] = mask; accs[t] += (uint32_t)__popc(mask); }
+                    if (mask != 0u) {                                         // masked swap (layout independent: same slot in both systems)
+#pragma unroll
+                        for (int k = lane; k < 128; k += 32) {
+                            uint4 *X = reinterpret_cast<uint4 *>(S + t * N) + k;
+                            uint4 *Y = reinterpret_cast<uint4 *>(S + (t + 1) * N) + k;
+                            uint4 xv = *X, yv = *Y;
+                            uint32_t dd;
+                            dd = (xv.x ^ yv.x) & mask; xv.x ^= dd; yv.x ^= dd;
+                            dd = (xv.y ^ yv.y) & mask; xv.y ^= dd; yv.y ^= dd;
+                            dd = (xv.z ^ yv.z) & mask; xv.z ^= dd; yv.z ^= dd;
+                            dd = (xv.w ^ yv.w) & mask; xv.w ^= dd; yv.w ^= dd;
+                            *X = xv;
+                            *Y = yv;
+                        }
+                    }
+                }
             }
-            __syncthreads();
             if (sw == A.n_sweeps - 1) {
                 // the launch ends here: publish the energies the decisions used, permuted like the configurations
-                for (int item = tid; item < NT * 32; item += nthr) {
-                    const int t = item >> 5, lane = item & 31;
+                __syncthreads();                                              // masks of all pairs
+                const int lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
+                for (int t = warp; t < NT; t += nwarp) {
                     const int p = t - e1;
                     int src = t;
                     if (p >= 0 && (p >> 1) < npairs && ((masks[p >> 1] >> lane) & 1u)) src = (p & 1) ? t - 1 : t + 1;
+                    // per-lane integers of both candidate systems (the transposes need the whole warp), then the lane's choice
+                    const uint32_t vt = transpose32(lane < 21 ? red3[t * 21 + lane] : 0u, lane);
+                    const int other = (p >= 0 && (p >> 1) < npairs) ? ((p & 1) ? t - 1 : t + 1) : t;
+                    const uint32_t vo = transpose32(lane < 21 ? red3[other * 21 + lane] : 0u, lane);
+                    const uint32_t v = src == t ? vt : vo;
                     const size_t o = ((size_t)(w * 32 + lane) * d.R + a) * NT + t;
-                    A.U[o] = (int64_t)Uint[src * 32 + lane];
-                    A.M[o] = Mint[src * 32 + lane];
+                    A.U[o] = (int64_t)(v & 0x7ffu);
+                    A.M[o] = 2 * (int)((v >> 11) & 0x3ffu) - N;
                 }
-            }
-            // ---- masked swap of the two configurations (layout independent: same slot in both systems)
-            for (int item = tid; item < npairs * 128; item += nthr) {
-                const int pair = item >> 7, k = item & 127;
-                const uint32_t mask = masks[pair];
-                if (mask == 0u) continue;
-                const int t = e1 + 2 * pair;
-                uint4 *X = reinterpret_cast<uint4 *>(S + t * N) + k;
-                uint4 *Y = reinterpret_cast<uint4 *>(S + (t + 1) * N) + k;
-                uint4 xv = *X, yv = *Y;
-                uint32_t dd;
-                dd = (xv.x ^ yv.x) & mask; xv.x ^= dd; yv.x ^= dd;
-                dd = (xv.y ^ yv.y) & mask; xv.y ^= dd; yv.y ^= dd;
-                dd = (xv.z ^ yv.z) & mask; xv.z ^= dd; yv.z ^= dd;
-                dd = (xv.w ^ yv.w) & mask; xv.w ^= dd; yv.w ^= dd;
-                *X = xv;
-                *Y = yv;
             }
             exchange += 1;
             __syncthreads();
