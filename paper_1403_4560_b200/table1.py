@@ -21,9 +21,9 @@ import numpy as np
 from . import estimators, workloads
 
 
-def run_size(sg, L, n_samples, n_sweeps, h, n_temps, beta_lo, beta_hi, meas_every, seed):
+def run_size(sg, L, n_samples, n_sweeps, h, n_temps, beta_lo, beta_hi, meas_every, seed, kind=None):
     temps = workloads.ladder(1.0 / beta_hi, 1.0 / beta_lo, n_temps)
-    sim = sg.Simulation(L, h, n_samples, 2, temps, sg.PMJ, seed)
+    sim = sg.Simulation(L, h, n_samples, 2, temps, sg.PMJ if kind is None else kind, seed)
     t0 = time.perf_counter()
     half = n_sweeps // 2
     sim.sg_run(half, 1, 0)
@@ -47,13 +47,17 @@ def main():
     ap.add_argument("--beta-hi", type=float, default=1.8)
     ap.add_argument("--meas-every", type=int, default=64)
     ap.add_argument("--seed", type=int, default=1403)
+    ap.add_argument("--packing", default="samples", choices=["samples", "temperatures"],
+                    help="samples: 32 disorder samples per word (default); temperatures: the paper's own packing "
+                         "(SG_PMJ_TPACK, PAPER.md:68) — same trajectories, for few samples")
     ap.add_argument("--json", default="", help="also write the curves to this file")
     args = ap.parse_args()
     from . import sg
     curves = {}
     for L in args.L:
         temps, out, n_meas, dt, rate = run_size(sg, L, args.samples, args.sweeps, args.h, args.temps, args.beta_lo,
-                                                args.beta_hi, args.meas_every, args.seed)
+                                                args.beta_hi, args.meas_every, args.seed,
+                                                sg.PMJ_TPACK if args.packing == "temperatures" else sg.PMJ)
         print("# L = %d, %d samples x 2 replicas x %d temperatures, h = %g, %d sweeps (PT every sweep), %d measurements, "
               "%.1f s, %.0f flips/ns" % (L, args.samples, args.temps, args.h, args.sweeps, n_meas, dt, rate))
         print("#  beta       T      g_std     +-     xi_L/L     +-       R12      +-   chi(k1)")
