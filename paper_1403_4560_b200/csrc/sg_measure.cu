@@ -243,8 +243,15 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
         uint32_t ones = 0, twos = 0, fours = 0, hi[C::HI];
 #pragma unroll
         for (int k = 0; k < C::HI; ++k) hi[k] = 0;
+        // The bins of one histogram (consecutive threads, b = 0 .. L-1) walk their L^2 sites in the same order, and except
+        // for the x histogram their addresses differ by multiples of L words: with the walk as written they would meet in
+        // the same shared-memory bank at every step.  Thread b therefore starts the loop whose stride is one word (the x
+        // direction) at offset b: the sites counted are the same, the banks of a step are all different.
+        const int skew_u = g.su == 1 ? b : 0, skew_v = g.sv == 1 ? b : 0;
 #pragma unroll 1
-        for (int u = 0; u < L; ++u) {
+        for (int uu = 0; uu < L; ++uu) {
+            int u = uu + skew_u;
+            if (u >= L) u -= L;
             int dd = (g.ku * u + g.kb) % L;
             if (dd < 0) dd += L;
             const uint32_t *base = Dp + u * g.su + dd * g.sd;
@@ -252,7 +259,11 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
             for (int v0 = 0; v0 < L; v0 += 8) {
                 uint32_t x[8];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) x[j] = (v0 + j < L) ? base[(v0 + j) * g.sv] : 0u;
+                for (int j = 0; j < 8; ++j) {
+                    int v = v0 + j + skew_v;
+                    if (v >= L) v -= L;
+                    x[j] = (v0 + j < L) ? base[v * g.sv] : 0u;
+                }
                 uint32_t tA, tB, fA, fB, e;
                 csa(tA, ones, ones, x[0], x[1]);
                 csa(tB, ones, ones, x[2], x[3]);
