@@ -5,6 +5,45 @@
 
 namespace sg {
 
+// R9: the moments of one measurement of (sample s, slot t) from its pair records r[pair][SG_REC], added to the
+// accumulators (and to the current logarithmic-binning window, if any)
+__device__ __forceinline__ void add_records(const Dims &d, const double (&r)[6][SG_REC], int s, int t, const MeasOut &mo)
+{
+    double a[SG_NMOM];
+    for (int j = 0; j < SG_NMOM; ++j) a[j] = 0.0;
+    for (int p = 0; p < d.P; ++p) {
+        const double v = r[p][0];
+        a[0] += v; a[1] += v * v; a[2] += v * v * v; a[3] += (v * v) * (v * v);
+        for (int k = 0; k < SG_NK; ++k) {
+            const double re = r[p][1 + 2 * k], im = r[p][2 + 2 * k];
+            a[4 + 5 * k + 0] += re;
+            a[4 + 5 * k + 1] += im;
+            a[4 + 5 * k + 2] += re * re + im * im;
+        }
+    }
+    // pair -> (a, b)
+    int pa[6], pb[6];
+    {
+        int p = 0;
+        for (int x = 0; x < d.R; ++x)
+            for (int y = x + 1; y < d.R; ++y) { pa[p] = x; pb[p] = y; ++p; }
+    }
+    for (int p = 0; p < d.P; ++p)
+        for (int p2 = p + 1; p2 < d.P; ++p2) {
+            const int shared = (pa[p] == pa[p2]) + (pa[p] == pb[p2]) + (pb[p] == pa[p2]) + (pb[p] == pb[p2]);
+            const int slot = shared == 1 ? 3 : 4;
+            a[slot == 3 ? 64 : 65] += r[p][0] * r[p2][0];
+            for (int k = 0; k < SG_NK; ++k)
+                a[4 + 5 * k + slot] += r[p][1 + 2 * k] * r[p2][1 + 2 * k] + r[p][2 + 2 * k] * r[p2][2 + 2 * k];
+        }
+    double *A = mo.acc + ((size_t)s * d.NT + t) * SG_NMOM;
+    for (int j = 0; j < SG_NMOM; ++j) A[j] += a[j];
+    if (mo.acc_win) {
+        double *B = mo.acc_win + ((size_t)s * d.NT + t) * SG_NMOM;
+        for (int j = 0; j < SG_NMOM; ++j) B[j] += a[j];
+    }
+}
+
 // One thread per (sample of the chunk, slot): loops over the replica pairs.
 // hist: [ns_pad][NT][P][N_HIST][L] uint16 counts of differing sites per plane
 // rec : [ns][NT][P][SG_REC] (scratch, copied to the host by sg_measure when asked)
@@ -57,39 +96,7 @@ k_finalize(Dims d, const uint16_t *__restrict__ hist, const double *__restrict__
             for (int m = 0; m < L; ++m) D0 += hp[m];
             atomicAdd(&mo.pq[((size_t)s * d.NT + t) * mo.pq_bins + pq_bin(d.N - D0, d.N, mo.pq_bins)], 1u);
         }
-    double a[SG_NMOM];
-    for (int j = 0; j < SG_NMOM; ++j) a[j] = 0.0;
-    for (int p = 0; p < d.P; ++p) {
-        const double v = r[p][0];
-        a[0] += v; a[1] += v * v; a[2] += v * v * v; a[3] += (v * v) * (v * v);
-        for (int k = 0; k < SG_NK; ++k) {
-            const double re = r[p][1 + 2 * k], im = r[p][2 + 2 * k];
-            a[4 + 5 * k + 0] += re;
-            a[4 + 5 * k + 1] += im;
-            a[4 + 5 * k + 2] += re * re + im * im;
-        }
-    }
-    // pair -> (a, b)
-    int pa[6], pb[6];
-    {
-        int p = 0;
-        for (int x = 0; x < d.R; ++x)
-            for (int y = x + 1; y < d.R; ++y) { pa[p] = x; pb[p] = y; ++p; }
-    }
-    for (int p = 0; p < d.P; ++p)
-        for (int p2 = p + 1; p2 < d.P; ++p2) {
-            const int shared = (pa[p] == pa[p2]) + (pa[p] == pb[p2]) + (pb[p] == pa[p2]) + (pb[p] == pb[p2]);
-            const int slot = shared == 1 ? 3 : 4;
-            a[slot == 3 ? 64 : 65] += r[p][0] * r[p2][0];
-            for (int k = 0; k < SG_NK; ++k)
-                a[4 + 5 * k + slot] += r[p][1 + 2 * k] * r[p2][1 + 2 * k] + r[p][2 + 2 * k] * r[p2][2 + 2 * k];
-        }
-    double *A = mo.acc + ((size_t)s * d.NT + t) * SG_NMOM;
-    for (int j = 0; j < SG_NMOM; ++j) A[j] += a[j];
-    if (mo.acc_win) {
-        double *B = mo.acc_win + ((size_t)s * d.NT + t) * SG_NMOM;
-        for (int j = 0; j < SG_NMOM; ++j) B[j] += a[j];
-    }
+    add_records(d, r, s, t, mo);
 }
 
 MeasOut meas_out(const sg_ctx *c)
@@ -179,15 +186,20 @@ __device__ __forceinline__ BinGeom bin_geometry(int hh, int b)
     return g;
 }
 
-template <int L>
-__global__ void __launch_bounds__(256)
+// ONEPAIR (L = 32, where the differing-site words of one pair already fill 128 KB of shared memory): one CTA per
+// (word, slot, replica pair) runs phases 0-3 for its pair and writes the pair's records to `rec`; k_acc_from_rec then
+// adds the moments, which need all pairs of a (sample, slot) together.
+template <int L, bool ONEPAIR>
+__global__ void __launch_bounds__(ONEPAIR ? 288 : 256)
 k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restrict__ tw, int w0, int s0,
               double *__restrict__ rec, MeasOut mo)
 {
     using C = MeasureCfg<L>;
     constexpr int N = C::N, NB = C::NB, Lh = L / 2, H = N / 2;
     extern __shared__ __align__(16) unsigned char sm_raw[];
-    const int P = d.P;
+    const int P = ONEPAIR ? 1 : d.P;                       // pairs handled by this CTA
+    const int pair0 = ONEPAIR ? (int)(blockIdx.x % (unsigned)d.P) : 0;
+    const int bidx = ONEPAIR ? (int)(blockIdx.x / (unsigned)d.P) : (int)blockIdx.x;
     // region A: D words [P][N] during the counting phase, then records [P][SG_REC][32] doubles
     uint32_t *Dsm = reinterpret_cast<uint32_t *>(sm_raw);
     double *REC = reinterpret_cast<double *>(sm_raw);
@@ -197,8 +209,8 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
     __shared__ int pa[6], pb[6], couples[15], n_couples;      // couples: p | p2 << 4 | shared << 8
 
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
-    const int t = blockIdx.x % d.NT;
-    const int w = w0 + blockIdx.x / d.NT;
+    const int t = bidx % d.NT;
+    const int w = w0 + bidx / d.NT;
     if (tid == 0) {
         int p = 0;
         for (int a = 0; a < d.R; ++a)
@@ -215,6 +227,22 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
     __syncthreads();
 
     // ---- phase 0: D = S^a xor S^b, canonical order (every replica's word is loaded once and used by all its pairs)
+    if constexpr (ONEPAIR) {
+        const uint32_t *A = spins + (((size_t)w * d.R + pa[pair0]) * d.NT + t) * N;
+        const uint32_t *B = spins + (((size_t)w * d.R + pb[pair0]) * d.NT + t) * N;
+        for (int k4 = tid; k4 < N / 4; k4 += nthr) {                   // four consecutive compact entries = one row segment
+            const uint4 av = reinterpret_cast<const uint4 *>(A)[k4], bv = reinterpret_cast<const uint4 *>(B)[k4];
+            const uint32_t dv[4] = {av.x ^ bv.x, av.y ^ bv.y, av.z ^ bv.z, av.w ^ bv.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int k = 4 * k4 + e;
+                const int c = k / H, n = k - c * H;
+                const int row = n / Lh, m = n - row * Lh;
+                const int z = row / L, y = row - z * L;
+                Dsm[2 * m + ((c + y + z) & 1) + L * (y + L * z)] = dv[e];
+            }
+        }
+    } else
     for (int k = tid; k < N; k += nthr) {                              // k = colour * H + n
         const int c = k / H, n = k - c * H;
         const int row = n / Lh, m = n - row * Lh;
@@ -357,9 +385,10 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
             const int l = item / (P * SG_REC), rest = item - l * (P * SG_REC);
             const int pair = rest / SG_REC, j = rest - pair * SG_REC;
             const int sl = w * 32 + l - s0;
-            rec[(((size_t)sl * d.NT + t) * P + pair) * SG_REC + j] = REC[((size_t)pair * SG_REC + j) * 32 + l];
+            rec[(((size_t)sl * d.NT + t) * d.P + pair0 + pair) * SG_REC + j] = REC[((size_t)pair * SG_REC + j) * 32 + l];
         }
     }
+    if constexpr (ONEPAIR) return;                         // the moments are added by k_acc_from_rec
 
     // ---- phase 4: one thread per (moment j, sample l), l fastest: j is warp-uniform (no divergence,
     // conflict-free record reads); the sums are staged in shared memory (OUT aliases the plane words,
@@ -446,19 +475,53 @@ static int launch_measure_L(sg_ctx *c, int s0, int ns, bool want_rec)
     const Dims &d = c->d;
     const size_t smem = measure_smem<L>(d.P);
     if (attr_needed(c, ATTR_MEASURE + L / 2 - 2)) {      // L = 4..16 -> ids 11..17
-        if (cudaFuncSetAttribute(k_measure_pmj<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)measure_smem<L>(6)) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_measure_pmj<L, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)measure_smem<L>(6)) != cudaSuccess)
             return -1;
     }
     const int w0 = s0 >> 5, nw = (ns + 31) >> 5;
-    k_measure_pmj<L><<<(unsigned)(nw * d.NT), 256, smem, c->stream>>>(d, c->spins, c->twiddle, w0, s0,
-                                                                      want_rec ? c->rec : nullptr, meas_out(c));
+    k_measure_pmj<L, false><<<(unsigned)(nw * d.NT), 256, smem, c->stream>>>(d, c->spins, c->twiddle, w0, s0,
+                                                                             want_rec ? c->rec : nullptr, meas_out(c));
     return 1;
+}
+
+// one thread per (sample of the chunk, slot): records of all pairs -> moment accumulators
+__global__ void __launch_bounds__(128)
+k_acc_from_rec(Dims d, const double *__restrict__ rec, int s0, int ns, MeasOut mo)
+{
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= ns * d.NT) return;
+    const int t = tid % d.NT, sl = tid / d.NT;
+    if (s0 + sl >= d.n_samples) return;
+    double r[6][SG_REC];
+    for (int p = 0; p < d.P; ++p)
+        for (int j = 0; j < SG_REC; ++j) r[p][j] = rec[(((size_t)sl * d.NT + t) * d.P + p) * SG_REC + j];
+    add_records(d, r, s0 + sl, t, mo);
+}
+
+// L = 32: one CTA per (word, slot, pair) + the accumulation kernel (records always go through c->rec)
+static int launch_measure_32(sg_ctx *c, int s0, int ns)
+{
+    const Dims &d = c->d;
+    const size_t smem = measure_smem<32>(1);
+    if (attr_needed(c, ATTR_MEASURE32)) {
+        if (cudaFuncSetAttribute(k_measure_pmj<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return -1;
+    }
+    const int w0 = s0 >> 5, nw = (ns + 31) >> 5;
+    MeasOut mo = meas_out(c), none = mo;
+    none.acc = nullptr;                                   // (unused by the ONEPAIR instantiation; P(q) is counted there)
+    none.acc_win = nullptr;
+    k_measure_pmj<32, true><<<(unsigned)(nw * d.NT * d.P), 288, smem, c->stream>>>(d, c->spins, c->twiddle, w0, s0, c->rec, none);
+    mo.pq = nullptr;
+    const int n = nw * 32 * d.NT;
+    k_acc_from_rec<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(d, c->rec, s0, nw * 32, mo);
+    return 2;
 }
 
 bool measure_fused_supported(const sg_ctx *c)
 {
     const int L = c->d.L;
-    return c->path == SG_PATH_AUTO && is_packed(c) && (L == 4 || L == 6 || L == 8 || L == 10 || L == 12 || L == 16);
+    return c->path == SG_PATH_AUTO && is_packed(c) && (L == 4 || L == 6 || L == 8 || L == 10 || L == 12 || L == 16 || L == 32);
 }
 
 // samples [s0, s0+ns), s0 a multiple of 32: records (optional) and accumulators in one launch
@@ -471,6 +534,7 @@ int launch_measure_pmj(sg_ctx *c, int s0, int ns, bool want_rec)
     case 10: return launch_measure_L<10>(c, s0, ns, want_rec);
     case 12: return launch_measure_L<12>(c, s0, ns, want_rec);
     case 16: return launch_measure_L<16>(c, s0, ns, want_rec);
+    case 32: return launch_measure_32(c, s0, ns);
     default: return -1;
     }
 }
