@@ -407,10 +407,22 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         if constexpr (Lh % 2 == 0) {
                             // even rows: elements (0,1) and (2,3) sit in one row at an even index, so every neighbour
                             // except the side one is an aligned 64-bit pair
+                            // a z-plane is a whole number of quads when L is a multiple of 4: the same-index and the +-z neighbours of
+                            // the quad are then one aligned 128-bit load each
+                            constexpr bool QZ = (L * Lh) % 4 == 0;
+                            if constexpr (QZ) {
+                                const uint4 a0 = *reinterpret_cast<const uint4 *>(So + ix[0][0]);
+                                const uint4 a4 = *reinterpret_cast<const uint4 *>(So + ix[0][4]);
+                                const uint4 a5 = *reinterpret_cast<const uint4 *>(So + ix[0][5]);
+                                v[0][0] = a0.x; v[1][0] = a0.y; v[2][0] = a0.z; v[3][0] = a0.w;
+                                v[0][4] = a4.x; v[1][4] = a4.y; v[2][4] = a4.z; v[3][4] = a4.w;
+                                v[0][5] = a5.x; v[1][5] = a5.y; v[2][5] = a5.z; v[3][5] = a5.w;
+                            }
 #pragma unroll
                             for (int e = 0; e < 4; e += 2) {
 #pragma unroll
                                 for (int k = 0; k < 6; ++k) {
+                                    if (QZ && (k == 0 || k >= 4)) continue;
                                     if (k == 1) {
                                         v[e][1] = So[ix[e][1]];
                                         v[e + 1][1] = So[ix[e + 1][1]];
