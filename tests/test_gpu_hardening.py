@@ -323,6 +323,39 @@ def test_shard_equals_slice_of_unsharded_pool(sg):
         whole.close(); part.close()
 
 
+def test_two_devices_sum_equals_one_device_pool(sg):
+    """SURVEY.md §8e on hardware, when two GPUs are visible (skipped otherwise): two contexts on two devices, each with
+    its shard of a 128-sample pool (global keys through sg_set_first_sample), give moment sums equal to the single-device
+    run of the whole pool to 1e-12, and the same spins.  Also exercises the per-context kernel attributes on a second device."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    temps = W.ladder(0.8, 1.6, 6)
+    for kind, L, ns in ((sg.PMJ, 8, 128), (sg.PMJ, 32, 64), (sg.GAUSS, 8, 6)):
+        half = ns // 2
+        with torch.cuda.device(0):
+            whole = sg.Simulation(L, 0.2, ns, 4, temps, kind, 17, device="cuda:0")
+            lo = sg.Simulation(L, 0.2, half, 4, temps, kind, 17, device="cuda:0")
+        with torch.cuda.device(1):
+            hi = sg.Simulation(L, 0.2, ns - half, 4, temps, kind, 17, device="cuda:1")
+            hi.sg_set_first_sample(half)
+            hi.sg_reset()
+        for sim, dev in ((whole, 0), (lo, 0), (hi, 1)):
+            with torch.cuda.device(dev):
+                sim.sg_run(12, 2, 4)
+        with torch.cuda.device(0):
+            m_all, n_all = whole.sg_get_moments()
+            m_lo, _ = lo.sg_get_moments()
+            s_all = whole.sg_get_spins()
+        with torch.cuda.device(1):
+            m_hi, n_hi = hi.sg_get_moments()
+            s_hi = hi.sg_get_spins()
+        assert n_all == n_hi == 3
+        assert np.array_equal(s_all[half:], s_hi)
+        assert close(m_lo.sum(axis=0) + m_hi.sum(axis=0), m_all.sum(axis=0))
+        whole.close(); lo.close(); hi.close()
+
+
 def test_sweep_counter_guard(sg):
     sim = sg.Simulation(4, 0.1, 1, 2, [1.0, 2.0])
     sim.sg_sweep(1)
