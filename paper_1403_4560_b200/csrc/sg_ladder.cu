@@ -85,8 +85,15 @@ struct Geo {
     static constexpr int Lh = L / 2, N = L * L * L, H = N / 2, Q = H / 4;
     static constexpr bool VEC = (Lh % 4) == 0;
     static constexpr int QR = VEC ? Lh / 4 : 1;     // quads per row (vector path)
+    // Rows of an even number of words that are not whole quads (L = 4, 12): every colour block of H words is kept in
+    // shared memory as two arrays of 64-bit pairs, [low pairs of the quads][high pairs of the quads].  A lane's quad is
+    // then two unit-stride 64-bit accesses, and so is every +-y / +-z neighbour (they start at an even word, i.e. on a
+    // pair, but not on a quad): no shared-memory bank conflicts, where 64-bit pairs at a 16-byte stride had 2-way ones.
+    static constexpr bool PAIR = !VEC && (Lh % 2) == 0;
+    // position of compact index n (< H) inside its colour block
+    static __host__ __device__ constexpr int pos(int n) { return PAIR ? ((n >> 1) & 1) * (H / 2) + ((n >> 2) << 1) + (n & 1) : n; }
     // launch bounds: L=8 runs two 320-thread CTAs per SM (256 ladders of config 2 on 148 SMs)
-    static constexpr int MAXT = L == 8 ? 320 : 512;
+    static constexpr int MAXT = L == 8 ? 320 : VEC ? 512 : 384;
     static constexpr int MINB = L == 8 ? 2 : 1;
 };
 
@@ -116,10 +123,11 @@ __device__ __forceinline__ void ladder_energy(const uint32_t *__restrict__ Ssys,
         const int xp = p ? sd : n, xm = p ? n : sd;
         const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m, ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
         const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m, zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
-        const uint32_t sa = s0[n], sb = s1[n];
-        const uint32_t u0 = xor3(sa, s1[xp], J0[n]), u1 = xor3(sa, s1[xm], J1[xm]);
-        const uint32_t u2 = xor3(sa, s1[yp], J0[H + n]), u3 = xor3(sa, s1[ym], J1[H + ym]);
-        const uint32_t u4 = xor3(sa, s1[zp], J0[2 * H + n]), u5 = xor3(sa, s1[zm], J1[2 * H + zm]);
+        constexpr auto P = Geo<L>::pos;                               // shared-memory position of a compact index
+        const uint32_t sa = s0[P(n)], sb = s1[P(n)];
+        const uint32_t u0 = xor3(sa, s1[P(xp)], J0[P(n)]), u1 = xor3(sa, s1[P(xm)], J1[P(xm)]);
+        const uint32_t u2 = xor3(sa, s1[P(yp)], J0[H + P(n)]), u3 = xor3(sa, s1[P(ym)], J1[H + P(ym)]);
+        const uint32_t u4 = xor3(sa, s1[P(zp)], J0[2 * H + P(n)]), u5 = xor3(sa, s1[P(zm)], J1[2 * H + P(zm)]);
         const uint32_t a0 = xor3(u0, u1, u2), c0 = maj3(u0, u1, u2);
         const uint32_t a1 = xor3(u3, u4, u5), c1 = maj3(u3, u4, u5);
         const uint32_t kk = a0 & a1;
@@ -177,7 +185,7 @@ __device__ __forceinline__ void ladder_energy_tab(const uint32_t *__restrict__ S
                 const uint2 j01 = *reinterpret_cast<const uint2 *>(JgT + 6 * n);
                 const uint2 j23 = *reinterpret_cast<const uint2 *>(JgT + 6 * n + 2);
                 const uint2 j45 = *reinterpret_cast<const uint2 *>(JgT + 6 * n + 4);
-                const uint32_t sa = s0[n];
+                const uint32_t sa = s0[ii.w];                         // ii.w = position of n in its colour block
                 const uint32_t u0 = xor3(sa, s1[ii.x & 0xffffu], j01.x), u1 = xor3(sa, s1[ii.x >> 16], j01.y);
                 const uint32_t u2 = xor3(sa, s1[ii.y & 0xffffu], j23.x), u3 = xor3(sa, s1[ii.y >> 16], j23.y);
                 const uint32_t u4 = xor3(sa, s1[ii.z & 0xffffu], j45.x), u5 = xor3(sa, s1[ii.z >> 16], j45.y);
@@ -188,7 +196,7 @@ __device__ __forceinline__ void ladder_energy_tab(const uint32_t *__restrict__ S
                 w[e][1] = xor3(c0, c1, kk);
                 w[e][2] = maj3(c0, c1, kk);
                 sw[2 * e] = sa;
-                sw[2 * e + 1] = s1[n];
+                sw[2 * e + 1] = s1[ii.w];
             } else {
                 w[e][0] = w[e][1] = w[e][2] = 0u;
                 sw[2 * e] = sw[2 * e + 1] = 0u;
@@ -248,11 +256,27 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     // ---- load the ladder, the couplings and the threshold constants
     {
         const uint4 *src = reinterpret_cast<const uint4 *>(gS);
-        uint4 *dst = reinterpret_cast<uint4 *>(S);
-        for (int i = tid; i < NT * N / 4; i += nthr) dst[i] = src[i];
         const uint4 *js = reinterpret_cast<const uint4 *>(gJ);
-        uint4 *jd = reinterpret_cast<uint4 *>(Jsm);
-        for (int i = tid; i < 3 * N / 4; i += nthr) jd[i] = js[i];
+        if constexpr (G_::PAIR) {                              // quad i of a colour block -> its low and high pair
+            uint2 *dst = reinterpret_cast<uint2 *>(S), *jd = reinterpret_cast<uint2 *>(Jsm);
+            for (int i = tid; i < NT * N / 4; i += nthr) {
+                const int blk = i / Q, qd = i - blk * Q;
+                const uint4 v = src[i];
+                dst[blk * (2 * Q) + qd] = make_uint2(v.x, v.y);
+                dst[blk * (2 * Q) + Q + qd] = make_uint2(v.z, v.w);
+            }
+            for (int i = tid; i < 3 * N / 4; i += nthr) {
+                const int blk = i / Q, qd = i - blk * Q;
+                const uint4 v = js[i];
+                jd[blk * (2 * Q) + qd] = make_uint2(v.x, v.y);
+                jd[blk * (2 * Q) + Q + qd] = make_uint2(v.z, v.w);
+            }
+        } else {
+            uint4 *dst = reinterpret_cast<uint4 *>(S);
+            for (int i = tid; i < NT * N / 4; i += nthr) dst[i] = src[i];
+            uint4 *jd = reinterpret_cast<uint4 *>(Jsm);
+            for (int i = tid; i < 3 * N / 4; i += nthr) jd[i] = js[i];
+        }
         for (int t = tid; t < NT; t += nthr) {                 // acceptance constants (SlotK of sg_accept.cuh)
             uint32_t lo[7], hi[7], kw[10];
             for (int c = 0; c < 7; ++c) {
@@ -279,12 +303,13 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
             const int xp = p ? sd : n, xm = p ? n : sd;
             const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m, ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
             const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m, zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
-            idxT[n] = make_uint4((uint32_t)xp | ((uint32_t)xm << 16), (uint32_t)yp | ((uint32_t)ym << 16),
-                                 (uint32_t)zp | ((uint32_t)zm << 16), 0u);
+            constexpr auto P = G_::pos;
+            idxT[n] = make_uint4((uint32_t)P(xp) | ((uint32_t)P(xm) << 16), (uint32_t)P(yp) | ((uint32_t)P(ym) << 16),
+                                 (uint32_t)P(zp) | ((uint32_t)P(zm) << 16), (uint32_t)P(n));
             uint32_t *g = JgT + 6 * n;
-            g[0] = J0[n];          g[1] = J1[xm];
-            g[2] = J0[H + n];      g[3] = J1[H + ym];
-            g[4] = J0[2 * H + n];  g[5] = J1[2 * H + zm];
+            g[0] = J0[P(n)];          g[1] = J1[P(xm)];
+            g[2] = J0[H + P(n)];      g[3] = J1[H + P(ym)];
+            g[4] = J0[2 * H + P(n)];  g[5] = J1[2 * H + P(zm)];
         }
         __syncthreads();
     }
@@ -373,36 +398,157 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                                                  A.mone);
                         reinterpret_cast<uint4 *>(Sa)[q] = make_uint4(out[0], out[1], out[2], out[3]);
                     }
-                } else {
-                    // generic lattice (rows of L/2 words are not whole quads): per-element neighbour indices and the
-                    // 24 coupling words of the quad are computed / loaded once per half sweep and shared by all
-                    // systems of the group
-                    int ix[4][6];
+                }
+            }
+            if constexpr (!G_::VEC) {
+                // generic lattice (rows of L/2 words are not whole quads).  Work item = (block of 32 quads, system); the
+                // NB * NT items of a half sweep are dealt out in contiguous ranges so that the four warp schedulers get the
+                // same number of items (warp w runs on scheduler w % 4).  Per-element neighbour indices and the 24 coupling
+                // words of the quad are computed / loaded when the block of a warp changes (at most twice per half sweep).
+                constexpr int NB = (Q + 31) / 32;
+                const uint32_t time = 2u * (A.sweep0 + (uint32_t)sw) + (uint32_t)colour;
+                const uint32_t *Jown = Jsm + (colour * 3) * H;
+                const uint32_t *Joth = Jsm + ((1 - colour) * 3) * H;
+                const int lane_ = tid & 31, warp_ = tid >> 5, NW = nthr >> 5;
+                const int rank = (warp_ & 3) * (NW >> 2) + (warp_ >> 2);
+                const int I = NB * NT;
+                const int i1 = (rank + 1) * I / NW;
+                int qq = 0;
+                bool qa = false;
+                if constexpr (G_::PAIR) {
+                    // pair layout (Geo::PAIR): per 64-bit pair h of the quad, the positions of its +-y / +-z neighbour
+                    // pairs and of the ONE word beyond the pair that its side (x) neighbours need, the row parity as a
+                    // mask, and the 24 coupling words of the quad
+                    constexpr int Q2 = 2 * Q;
+                    int ip[2][6];
                     uint32_t Jq[4][6];
+                    // one work item: system t of the current block (Sa / So = its own / the other colour block)
+                    auto item = [&](const int t, uint32_t *__restrict__ Sa, const uint32_t *__restrict__ So) {
+                        const uint4 r4 = philox_rk((uint32_t)qq, time, wglob, ctr3(3, a, t), A.rk);
+                        SlotK K;
+                        {
+                            const uint4 *k4 = reinterpret_cast<const uint4 *>(thr + t * 8);
+                            const uint4 k0 = k4[0], k1 = k4[1], k2 = k4[2];
+                            K.lo[0] = k0.x; K.lo[1] = k0.y; K.lo[2] = k0.z; K.lo[3] = k0.w;
+                            K.lo[4] = k1.x; K.lo[5] = k1.y; K.lo[6] = k1.z; K.b3c = k1.w;
+                            K.nc = k2.x; K.ec = k2.y;
+                        }
+                        const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const int n = 4 * q + e;
-                        const int row = n / Lh, m = n - row * Lh;
-                        const int z = row / L, y = row - z * L;
-                        const int p = (colour + y + z) & 1;
-                        const int sd = row * Lh + (p ? (m + 1 == Lh ? 0 : m + 1) : (m == 0 ? Lh - 1 : m - 1));
-                        const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m;
-                        const int ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
-                        const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m;
-                        const int zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
-                        // slot 0: the x-neighbour at the same compact index (its bond if p, own bond else); slot 1: the one
-                        // at the side index (own bond if p, its bond else)
-                        ix[e][0] = n; ix[e][1] = sd; ix[e][2] = yp; ix[e][3] = ym; ix[e][4] = zp; ix[e][5] = zm;
-                        Jq[e][0] = p ? Joth[n] : Jown[n];
-                        Jq[e][1] = p ? Jown[n] : Joth[sd];
-                        Jq[e][2] = Jown[H + n];      Jq[e][3] = Joth[H + ym];
-                        Jq[e][4] = Jown[2 * H + n];  Jq[e][5] = Joth[2 * H + zm];
-                    }
+                        for (int hh = 0; hh < 2; ++hh) {
+                            const int o = hh * Q2 + 2 * qq;
+                            const uint2 sv = *reinterpret_cast<const uint2 *>(Sa + o);
+                            const uint2 a0 = *reinterpret_cast<const uint2 *>(So + o);
+                            const uint2 vyp = *reinterpret_cast<const uint2 *>(So + ip[hh][0]);
+                            const uint2 vym = *reinterpret_cast<const uint2 *>(So + ip[hh][1]);
+                            const uint2 vzp = *reinterpret_cast<const uint2 *>(So + ip[hh][2]);
+                            const uint2 vzm = *reinterpret_cast<const uint2 *>(So + ip[hh][3]);
+                            const uint32_t sd0 = So[ip[hh][4]], sd1 = So[ip[hh][5]];
+                            const int e0 = 2 * hh, e1 = 2 * hh + 1;
+                            const uint32_t o0 = flip_word_k<BS>(sv.x, amask, xor3(sv.x, a0.x, Jq[e0][0]), xor3(sv.x, sd0, Jq[e0][1]),
+                                                                xor3(sv.x, vyp.x, Jq[e0][2]), xor3(sv.x, vym.x, Jq[e0][3]),
+                                                                xor3(sv.x, vzp.x, Jq[e0][4]), xor3(sv.x, vzm.x, Jq[e0][5]), rr[e0], K,
+                                                                A.one, A.mone);
+                            const uint32_t o1 = flip_word_k<BS>(sv.y, amask, xor3(sv.y, a0.y, Jq[e1][0]), xor3(sv.y, sd1, Jq[e1][1]),
+                                                                xor3(sv.y, vyp.y, Jq[e1][2]), xor3(sv.y, vym.y, Jq[e1][3]),
+                                                                xor3(sv.y, vzp.y, Jq[e1][4]), xor3(sv.y, vzm.y, Jq[e1][5]), rr[e1], K,
+                                                                A.one, A.mone);
+                            if (qa) *reinterpret_cast<uint2 *>(Sa + o) = make_uint2(o0, o1);
+                        }
+                    };
+                    const int i0 = rank * I / NW;
+                    int b = i0 / NT, t = i0 - b * NT;
 #pragma unroll 1
-                    for (int t = g; t < NT; t += A.G) {
+                    for (int i = i0; i < i1;) {
+                        if (t == NT) { t = 0; ++b; }
+                        {
+                            qq = 32 * b + lane_;
+                            qa = qq < Q;
+                            if (!qa) qq = Q - 1;
+#pragma unroll
+                            for (int hh = 0; hh < 2; ++hh) {
+                                const int n = 4 * qq + 2 * hh, o = hh * Q2 + 2 * qq;
+                                const int row = n / Lh, m = n - row * Lh;
+                                const int z = row / L, y = row - z * L;
+                                const int p = (colour + y + z) & 1;
+                                const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m;
+                                const int ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
+                                const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m;
+                                const int zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
+                                // p: the side neighbours are m + 1 (the pair's own second word, and the word after the pair);
+                                // else m - 1 (the word before the pair, and the pair's own first word); periodic in the row
+                                const int sdn = G_::pos(p ? (m + 2 == Lh ? row * Lh : n + 2) : (m == 0 ? row * Lh + Lh - 1 : n - 1));
+                                ip[hh][0] = G_::pos(yp); ip[hh][1] = G_::pos(ym); ip[hh][2] = G_::pos(zp); ip[hh][3] = G_::pos(zm);
+                                ip[hh][4] = p ? o + 1 : sdn;
+                                ip[hh][5] = p ? sdn : o;
+                                const uint2 jx = *reinterpret_cast<const uint2 *>(Jown + o);
+                                const uint2 jox = *reinterpret_cast<const uint2 *>(Joth + o);
+                                const uint2 jy = *reinterpret_cast<const uint2 *>(Jown + H + o);
+                                const uint2 joy = *reinterpret_cast<const uint2 *>(Joth + H + ip[hh][1]);
+                                const uint2 jz = *reinterpret_cast<const uint2 *>(Jown + 2 * H + o);
+                                const uint2 joz = *reinterpret_cast<const uint2 *>(Joth + 2 * H + ip[hh][3]);
+                                const uint32_t jsd = Joth[sdn];
+                                // slot 0: the x-neighbour at the same compact index (its bond if p, own bond else); slot 1: the side one
+                                Jq[2 * hh][0] = p ? jox.x : jx.x;      Jq[2 * hh + 1][0] = p ? jox.y : jx.y;
+                                Jq[2 * hh][1] = p ? jx.x : jsd;        Jq[2 * hh + 1][1] = p ? jx.y : jox.x;
+                                Jq[2 * hh][2] = jy.x;   Jq[2 * hh + 1][2] = jy.y;
+                                Jq[2 * hh][3] = joy.x;  Jq[2 * hh + 1][3] = joy.y;
+                                Jq[2 * hh][4] = jz.x;   Jq[2 * hh + 1][4] = jz.y;
+                                Jq[2 * hh][5] = joz.x;  Jq[2 * hh + 1][5] = joz.y;
+                            }
+                        }
+                        // the systems t .. tend - 1 of this block, two per trip (the second one at a compile-time offset)
+                        const int tend = min(NT, t + (i1 - i));
+                        i += tend - t;
                         uint32_t *Sa = S + t * N + colour * H;
                         const uint32_t *So = S + t * N + (1 - colour) * H;
-                        const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[q];
+#pragma unroll 1
+                        for (; t + 1 < tend; t += 2, Sa += 2 * N, So += 2 * N) {
+                            item(t, Sa, So);
+                            item(t + 1, Sa + N, So + N);
+                        }
+                        if (t < tend) {
+                            item(t, Sa, So);
+                            ++t;
+                        }
+                    }
+                } else {
+                    int bcur = -1;
+                    int ix[4][6];
+                    uint32_t Jq[4][6];
+                    const int i0 = rank * I / NW;
+                    int b = i0 / NT, t = i0 - b * NT;
+#pragma unroll 1
+                    for (int i = i0; i < i1; ++i, ++t) {
+                        if (t == NT) { t = 0; ++b; }
+                        if (b != bcur) {
+                            bcur = b;
+                            qq = 32 * b + lane_;
+                            qa = qq < Q;
+                            if (!qa) qq = Q - 1;
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                const int n = 4 * qq + e;
+                                const int row = n / Lh, m = n - row * Lh;
+                                const int z = row / L, y = row - z * L;
+                                const int p = (colour + y + z) & 1;
+                                const int sd = row * Lh + (p ? (m + 1 == Lh ? 0 : m + 1) : (m == 0 ? Lh - 1 : m - 1));
+                                const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m;
+                                const int ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
+                                const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m;
+                                const int zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
+                                // slot 0: the x-neighbour at the same compact index (its bond if p, own bond else); slot 1: the one
+                                // at the side index (own bond if p, its bond else)
+                                ix[e][0] = n; ix[e][1] = sd; ix[e][2] = yp; ix[e][3] = ym; ix[e][4] = zp; ix[e][5] = zm;
+                                Jq[e][0] = p ? Joth[n] : Jown[n];
+                                Jq[e][1] = p ? Jown[n] : Joth[sd];
+                                Jq[e][2] = Jown[H + n];      Jq[e][3] = Joth[H + ym];
+                                Jq[e][4] = Jown[2 * H + n];  Jq[e][5] = Joth[2 * H + zm];
+                            }
+                        }
+                        uint32_t *Sa = S + t * N + colour * H;
+                        const uint32_t *So = S + t * N + (1 - colour) * H;
+                        const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[qq];
                         uint32_t v[4][6];
                         if constexpr (Lh % 2 == 0) {
                             // even rows: elements (0,1) and (2,3) sit in one row at an even index, so every neighbour
@@ -439,7 +585,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
 #pragma unroll
                                 for (int k = 0; k < 6; ++k) v[e][k] = So[ix[e][k]];
                         }
-                        const uint4 r4 = philox_rk((uint32_t)q, time, wglob, ctr3(3, a, t), A.rk);
+                        const uint4 r4 = philox_rk((uint32_t)qq, time, wglob, ctr3(3, a, t), A.rk);
                         SlotK K;
                         {
                             const uint4 *k4 = reinterpret_cast<const uint4 *>(thr + t * 8);
@@ -457,7 +603,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                                                  xor3(s[e], v[e][2], Jq[e][2]), xor3(s[e], v[e][3], Jq[e][3]),
                                                  xor3(s[e], v[e][4], Jq[e][4]), xor3(s[e], v[e][5], Jq[e][5]), rr[e], K, A.one,
                                                  A.mone);
-                        reinterpret_cast<uint4 *>(Sa)[q] = make_uint4(out[0], out[1], out[2], out[3]);
+                        if (qa) reinterpret_cast<uint4 *>(Sa)[qq] = make_uint4(out[0], out[1], out[2], out[3]);
                     }
                 }
             }
@@ -528,8 +674,17 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
         if (accs[t]) atomicAdd(&A.pt_acc[t], (unsigned long long)accs[t]);
     {
         uint4 *dst = reinterpret_cast<uint4 *>(gS);
-        const uint4 *src = reinterpret_cast<const uint4 *>(S);
-        for (int i = tid; i < NT * N / 4; i += nthr) dst[i] = src[i];
+        if constexpr (G_::PAIR) {
+            const uint2 *src = reinterpret_cast<const uint2 *>(S);
+            for (int i = tid; i < NT * N / 4; i += nthr) {
+                const int blk = i / Q, qd = i - blk * Q;
+                const uint2 lo = src[blk * (2 * Q) + qd], hi = src[blk * (2 * Q) + Q + qd];
+                dst[i] = make_uint4(lo.x, lo.y, hi.x, hi.y);
+            }
+        } else {
+            const uint4 *src = reinterpret_cast<const uint4 *>(S);
+            for (int i = tid; i < NT * N / 4; i += nthr) dst[i] = src[i];
+        }
     }
 }
 
@@ -593,12 +748,19 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchang
     A.pt_acc = c->pt_acc;
     const int Q = d.N / 8;
     // groups: as many as fit in <= 512 threads, at most NT, preferring a divisor of NT
-    const int maxt = d.L == 8 ? 320 : 512;
+    const int maxt = d.L == 8 ? 320 : ((d.L / 2) % 4 == 0 ? 512 : 384);
     int G = std::max(1, std::min(d.NT, maxt / Q));
     for (int gtry = G; gtry >= 1 && gtry * 2 > G; --gtry)
         if (d.NT % gtry == 0) { G = gtry; break; }
     A.G = G;
     int threads = (Q * G + 31) / 32 * 32;
+    if ((d.L / 2) % 4 != 0) {
+        // generic lattices: balanced warp items (block of 32 quads, system); a multiple of four warps, at most 12
+        const int items = (Q + 31) / 32 * d.NT;
+        // (measured at C3: 12 warps with 130 registers beat 16 with 116 and 20 with 96 - the kernel is bound by ALU-pipe
+        // and issue throughput, not by latency)
+        threads = 32 * std::min(12, (items + 3) / 4 * 4);
+    }
     if (threads > maxt) return -1;
     size_t smem = ladder_smem_bytes(d.L, d.NT);
     A.use_tab = smem + ladder_tab_bytes(d.L) <= (size_t)227 * 1024 ? 1 : 0;
