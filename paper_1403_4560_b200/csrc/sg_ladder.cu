@@ -34,6 +34,7 @@ struct LadderArgs {
     int32_t *M;
     unsigned long long *pt_acc;
     int use_tab;              // shared memory has room for the energy tables (neighbour indices + gathered couplings)
+    int use_spw;              // pair layout: room for the offset table of the system-per-warp exchange half sweep
 };
 
 __device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -229,7 +230,8 @@ __device__ __forceinline__ void ladder_energy_tab(const uint32_t *__restrict__ S
     M = 2 * (int)bs_warp_total(bigM, PM, lane) - N;
 }
 
-template <int L, bool BS>
+// PT = false: the instantiation for launches without exchanges (pt_every == 0), all exchange code compiled out
+template <int L, bool BS, bool PT>
 __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const __grid_constant__ LadderArgs A)
 {
     using G_ = Geo<L>;
@@ -247,6 +249,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     // energy tables (use_tab): 16-byte aligned behind the scratch above
     uint4 *idxT = reinterpret_cast<uint4 *>((reinterpret_cast<uintptr_t>(accs + NT) + 15) & ~(uintptr_t)15);   // [H]
     uint32_t *JgT = reinterpret_cast<uint32_t *>(idxT + H);                                                     // [H][6]
+    uint2 *spwT = reinterpret_cast<uint2 *>(idxT);        // [9][Q] byte offsets of the colour-1 quads (use_spw; instead of idxT / JgT)
 
     const int w = blockIdx.x / d.R, a = blockIdx.x % d.R;
     const int tid = threadIdx.x, nthr = blockDim.x;
@@ -293,7 +296,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
         for (int t = tid; t < NT; t += nthr) accs[t] = 0u;
     }
     __syncthreads();
-    if (A.use_tab && A.pt_every > 0) {                    // neighbour indices and couplings of the colour-0 sites, once per launch
+    if (PT && A.use_tab && !A.use_spw && A.pt_every > 0) {      // neighbour indices and couplings of the colour-0 sites, once per launch
         const uint32_t *J0 = Jsm, *J1 = Jsm + 3 * H;
         for (int n = tid; n < H; n += nthr) {
             const int row = n / Lh, m = n - row * Lh;
@@ -312,6 +315,42 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
             g[4] = J0[2 * H + P(n)];  g[5] = J1[2 * H + P(zm)];
         }
         __syncthreads();
+    }
+
+    if constexpr (G_::PAIR) {
+        if (PT && A.use_spw && A.pt_every > 0) {
+            // Offsets (bytes) for the colour-1 half sweep that precedes an exchange, where a WARP owns two systems and its
+            // lanes walk the quads, so nothing can be hoisted into registers.  Per pair hh of quad qd, relative to the
+            // other-colour block of the system: +y, -y, +z, -z neighbour pairs and the two side words; relative to the
+            // couplings: the pair of slot 0 and the two words of slot 1 (see the block-item path below for the selection).
+            constexpr int Q2 = 2 * Q;
+            for (int qd = tid; qd < Q; qd += nthr) {
+#pragma unroll
+                for (int hh = 0; hh < 2; ++hh) {
+                    const int n = 4 * qd + 2 * hh, o = hh * Q2 + 2 * qd;
+                    const int row = n / Lh, m = n - row * Lh;
+                    const int z = row / L, y = row - z * L;
+                    const int p = (1 + y + z) & 1;
+                    const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m;
+                    const int ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
+                    const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m;
+                    const int zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
+                    const int sdn = G_::pos(p ? (m + 2 == Lh ? row * Lh : n + 2) : (m == 0 ? row * Lh + Lh - 1 : n - 1));
+                    constexpr int JOWN = 3 * H, JOTH = 0;               // colour 1 owns the second coupling block
+                    uint32_t e[9];
+                    e[0] = 4u * G_::pos(yp); e[1] = 4u * G_::pos(ym); e[2] = 4u * G_::pos(zp); e[3] = 4u * G_::pos(zm);
+                    e[4] = 4u * (p ? o + 1 : sdn);
+                    e[5] = 4u * (p ? sdn : o);
+                    e[6] = 4u * (p ? JOTH + o : JOWN + o);
+                    e[7] = 4u * (p ? JOWN + o : JOTH + sdn);
+                    e[8] = 4u * (p ? JOWN + o + 1 : JOTH + o);
+                    uint32_t *T = reinterpret_cast<uint32_t *>(spwT);   // word k of pair hh of quad qd: T[((k * Q) + qd) * 2 + hh]
+#pragma unroll
+                    for (int k = 0; k < 9; ++k) T[(k * Q + qd) * 2 + hh] = e[k];
+                }
+            }
+            __syncthreads();
+        }
     }
 
     const int q = tid % Q, g = tid / Q;
@@ -456,6 +495,173 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                             if (qa) *reinterpret_cast<uint2 *>(Sa + o) = make_uint2(o0, o1);
                         }
                     };
+                    // The same work item with the energy bookkeeping of the exchange step (colour 1 only): U = sum over the
+                    // colour-1 sites of their unsatisfied-bond counts AFTER the update (every bond has one colour-1 end; a flip
+                    // turns n into 6 - n), spin count = the four new words + the four other-colour words at the same compact
+                    // index; both added to the lane's running bit-sliced totals.
+                    constexpr int PU = NB * 24 < 32 ? 5 : NB * 24 < 64 ? 6 : NB * 24 < 128 ? 7 : NB * 24 < 256 ? 8 : 9;
+                    constexpr int PM = NB * 8 < 16 ? 4 : NB * 8 < 32 ? 5 : NB * 8 < 64 ? 6 : 7;
+                    static_assert(NB * 24 < 512 && NB * 8 < 128, "plane counts");
+                    auto itemE = [&](const int t, uint32_t *__restrict__ Sa, const uint32_t *__restrict__ So, uint32_t (&aU)[PU],
+                                     uint32_t (&aM)[PM]) {
+                        const uint4 r4 = philox_rk((uint32_t)qq, time, wglob, ctr3(3, a, t), A.rk);
+                        SlotK K;
+                        {
+                            const uint4 *k4 = reinterpret_cast<const uint4 *>(thr + t * 8);
+                            const uint4 k0 = k4[0], k1 = k4[1], k2 = k4[2];
+                            K.lo[0] = k0.x; K.lo[1] = k0.y; K.lo[2] = k0.z; K.lo[3] = k0.w;
+                            K.lo[4] = k1.x; K.lo[5] = k1.y; K.lo[6] = k1.z; K.b3c = k1.w;
+                            K.nc = k2.x; K.ec = k2.y;
+                        }
+                        const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
+                        uint32_t wpl[4][3], outw[4], othw[4];
+#pragma unroll
+                        for (int hh = 0; hh < 2; ++hh) {
+                            const int o = hh * Q2 + 2 * qq;
+                            const uint2 sv = *reinterpret_cast<const uint2 *>(Sa + o);
+                            const uint2 a0 = *reinterpret_cast<const uint2 *>(So + o);
+                            const uint2 vyp = *reinterpret_cast<const uint2 *>(So + ip[hh][0]);
+                            const uint2 vym = *reinterpret_cast<const uint2 *>(So + ip[hh][1]);
+                            const uint2 vzp = *reinterpret_cast<const uint2 *>(So + ip[hh][2]);
+                            const uint2 vzm = *reinterpret_cast<const uint2 *>(So + ip[hh][3]);
+                            const uint32_t sdw[2] = {So[ip[hh][4]], So[ip[hh][5]]};
+                            const uint32_t sw2[2] = {sv.x, sv.y}, a02[2] = {a0.x, a0.y}, yp2[2] = {vyp.x, vyp.y}, ym2[2] = {vym.x, vym.y};
+                            const uint32_t zp2[2] = {vzp.x, vzp.y}, zm2[2] = {vzm.x, vzm.y};
+#pragma unroll
+                            for (int j = 0; j < 2; ++j) {
+                                const int e = 2 * hh + j;
+                                const uint32_t sx = sw2[j];
+                                uint32_t n0, n1, n2;
+                                const uint32_t acc = accept_word<BS>(xor3(sx, a02[j], Jq[e][0]), xor3(sx, sdw[j], Jq[e][1]),
+                                                                     xor3(sx, yp2[j], Jq[e][2]), xor3(sx, ym2[j], Jq[e][3]),
+                                                                     xor3(sx, zp2[j], Jq[e][4]), xor3(sx, zm2[j], Jq[e][5]),
+                                                                     ~(sx ^ amask), rr[e], K, A.one, A.mone, n0, n1, n2);
+                                outw[e] = sx ^ acc;
+                                othw[e] = a02[j];
+                                // 6 - n: bit 0 = n0; bit 1 set for n in {0, 3, 4}; bit 2 set for n in {0, 1, 2}
+                                const uint32_t f1 = (~n2 & ~(n1 ^ n0)) | (n2 & ~n1 & ~n0);
+                                const uint32_t f2 = ~n2 & ~(n1 & n0);
+                                wpl[e][0] = n0;
+                                wpl[e][1] = (acc & f1) | (~acc & n1);
+                                wpl[e][2] = (acc & f2) | (~acc & n2);
+                            }
+                            *reinterpret_cast<uint2 *>(Sa + o) = make_uint2(outw[2 * hh], outw[2 * hh + 1]);
+                        }
+                        uint32_t ab[4], cd[4], U5[5];
+                        bs_sum<3>(wpl[0], wpl[1], ab);
+                        bs_sum<3>(wpl[2], wpl[3], cd);
+                        bs_sum<4>(ab, cd, U5);
+                        bs_add(aU, U5);
+                        const uint32_t x1 = xor3(outw[0], outw[1], outw[2]), y1 = maj3(outw[0], outw[1], outw[2]);
+                        const uint32_t x2 = xor3(outw[3], othw[0], othw[1]), y2 = maj3(outw[3], othw[0], othw[1]);
+                        const uint32_t x3 = xor3(x1, x2, othw[2]), y3 = maj3(x1, x2, othw[2]);
+                        const uint32_t ones = x3 ^ othw[3], y4 = x3 & othw[3];
+                        const uint32_t t1 = xor3(y1, y2, y3), g1 = maj3(y1, y2, y3);
+                        const uint32_t twos = t1 ^ y4, g2 = t1 & y4;
+                        const uint32_t M4[4] = {ones, twos, g1 ^ g2, g1 & g2};
+                        bs_add(aM, M4);
+                    };
+                    const bool pt_due_now = PT && A.use_spw && colour == 1 && A.pt_every > 0 &&
+                                            ((uint64_t)A.sweep0 + (uint64_t)sw + 1) % (uint64_t)A.pt_every == 0;
+                    if (pt_due_now) {
+                        // ---- colour-1 half sweep + exchange, one WARP per pair of neighbouring slots: the lanes walk the quads
+                        // of both systems (offsets and couplings from the table / shared memory), keep the energy counts in
+                        // registers, and the warp then decides and swaps its own two systems: no pass over the ladder and no
+                        // CTA barrier between the half sweep, the decisions and the swaps.
+                        const int e1 = (int)(exchange & 1u);
+                        const int npairs = (NT - e1) / 2;
+                        const bool left_lo = e1 == 1, left_hi = ((NT - e1) & 1) != 0;      // slots without a partner this time
+                        const int ntask = npairs + ((left_lo || left_hi) ? 1 : 0);
+                        const bool last = sw == A.n_sweeps - 1;
+                        const uint32_t *Tw = reinterpret_cast<const uint32_t *>(spwT);
+                        for (int task = warp_; task < ntask; task += NW) {
+                            const bool paired = task < npairs;
+                            int tA, tB;
+                            if (paired) { tA = e1 + 2 * task; tB = tA + 1; }
+                            else if (left_lo && left_hi) { tA = NT - 1; tB = 0; }
+                            else { tA = left_lo ? 0 : NT - 1; tB = tA; }
+                            const bool two = tB != tA;
+                            const int offB = (tB - tA) * N;
+                            uint32_t *SaA = S + tA * N + H;
+                            const uint32_t *SoA = S + tA * N;
+                            uint32_t aU0[PU], aM0[PM], aU1[PU], aM1[PM];
+#pragma unroll
+                            for (int k = 0; k < PU; ++k) aU0[k] = aU1[k] = 0u;
+#pragma unroll
+                            for (int k = 0; k < PM; ++k) aM0[k] = aM1[k] = 0u;
+#pragma unroll 1
+                            for (int kb = 0; kb < NB; ++kb) {
+                                qq = 32 * kb + lane_;
+                                qa = true;
+                                if (qq < Q) {
+#pragma unroll
+                                    for (int hh = 0; hh < 2; ++hh) {
+                                        const int o = hh * Q2 + 2 * qq;
+                                        uint32_t ee[9];
+#pragma unroll
+                                        for (int k = 0; k < 9; ++k) ee[k] = Tw[(k * Q + qq) * 2 + hh];
+#pragma unroll
+                                        for (int k = 0; k < 6; ++k) ip[hh][k] = (int)(ee[k] >> 2);
+                                        const char *Jb = reinterpret_cast<const char *>(Jsm);
+                                        const uint2 j0 = *reinterpret_cast<const uint2 *>(Jb + ee[6]);
+                                        const uint32_t j1a = *reinterpret_cast<const uint32_t *>(Jb + ee[7]);
+                                        const uint32_t j1b = *reinterpret_cast<const uint32_t *>(Jb + ee[8]);
+                                        const uint2 jy = *reinterpret_cast<const uint2 *>(Jsm + 3 * H + H + o);
+                                        const uint2 joy = *reinterpret_cast<const uint2 *>(Jb + 4 * H + ee[1]);
+                                        const uint2 jz = *reinterpret_cast<const uint2 *>(Jsm + 3 * H + 2 * H + o);
+                                        const uint2 joz = *reinterpret_cast<const uint2 *>(Jb + 8 * H + ee[3]);
+                                        Jq[2 * hh][0] = j0.x;   Jq[2 * hh + 1][0] = j0.y;
+                                        Jq[2 * hh][1] = j1a;    Jq[2 * hh + 1][1] = j1b;
+                                        Jq[2 * hh][2] = jy.x;   Jq[2 * hh + 1][2] = jy.y;
+                                        Jq[2 * hh][3] = joy.x;  Jq[2 * hh + 1][3] = joy.y;
+                                        Jq[2 * hh][4] = jz.x;   Jq[2 * hh + 1][4] = jz.y;
+                                        Jq[2 * hh][5] = joz.x;  Jq[2 * hh + 1][5] = joz.y;
+                                    }
+                                    itemE(tA, SaA, SoA, aU0, aM0);
+                                    if (two) itemE(tB, SaA + offB, SoA + offB, aU1, aM1);
+                                }
+                            }
+                            __syncwarp();
+                            const int U0 = (int)bs_warp_total(aU0, PU, lane_), M0 = 2 * (int)bs_warp_total(aM0, PM, lane_) - N;
+                            const int U1 = (int)bs_warp_total(aU1, PU, lane_), M1 = 2 * (int)bs_warp_total(aM1, PM, lane_) - N;
+                            uint32_t mask = 0u;
+                            if (paired) {
+                                const int smp = w * 32 + lane_;
+                                const double Et = __dsub_rn((double)(2 * U0 - 3 * N), __dmul_rn(A.h, (double)M0));
+                                const double Eu = __dsub_rn((double)(2 * U1 - 3 * N), __dmul_rn(A.h, (double)M1));
+                                const double x = __dmul_rn(__dsub_rn(A.tab[tA].beta, A.tab[tB].beta), __dsub_rn(Et, Eu));
+                                const uint4 r = philox_rk(0u, (uint32_t)exchange, (uint32_t)(smp + d.s_first), ctr3(4, a, tA), A.rk);
+                                const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
+                                mask = __ballot_sync(0xffffffffu, accept && smp < d.n_samples);
+                                if (lane_ == 0) accs[tA] += (uint32_t)__popc(mask);
+                                if (mask != 0u) {                             // masked swap of the warp's own two systems
+                                    for (int k = lane_; k < N / 4; k += 32) {
+                                        uint4 *X = reinterpret_cast<uint4 *>(S + tA * N) + k;
+                                        uint4 *Y = reinterpret_cast<uint4 *>(S + tB * N) + k;
+                                        uint4 xv = *X, yv = *Y;
+                                        uint32_t dd;
+                                        dd = (xv.x ^ yv.x) & mask; xv.x ^= dd; yv.x ^= dd;
+                                        dd = (xv.y ^ yv.y) & mask; xv.y ^= dd; yv.y ^= dd;
+                                        dd = (xv.z ^ yv.z) & mask; xv.z ^= dd; yv.z ^= dd;
+                                        dd = (xv.w ^ yv.w) & mask; xv.w ^= dd; yv.w ^= dd;
+                                        *X = xv;
+                                        *Y = yv;
+                                    }
+                                }
+                            }
+                            if (last) {                                       // publish the energies, permuted like the configurations
+                                const bool swp = (mask >> lane_) & 1u;
+                                const size_t oA = ((size_t)(w * 32 + lane_) * d.R + a) * NT + tA;
+                                A.U[oA] = (int64_t)(swp ? U1 : U0);
+                                A.M[oA] = swp ? M1 : M0;
+                                if (two) {
+                                    const size_t oB = ((size_t)(w * 32 + lane_) * d.R + a) * NT + tB;
+                                    A.U[oB] = (int64_t)(swp ? U0 : U1);
+                                    A.M[oB] = swp ? M0 : M1;
+                                }
+                            }
+                        }
+                    } else {
                     const int i0 = rank * I / NW;
                     int b = i0 / NT, t = i0 - b * NT;
 #pragma unroll 1
@@ -511,6 +717,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                             item(t, Sa, So);
                             ++t;
                         }
+                    }
                     }
                 } else {
                     int bcur = -1;
@@ -610,7 +817,10 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
             __syncthreads();
         }
         // ---- exchange step (R12), all in shared memory
-        if (A.pt_every > 0 && ((uint64_t)A.sweep0 + (uint64_t)sw + 1) % (uint64_t)A.pt_every == 0) {
+        const bool pt_due = PT && A.pt_every > 0 && ((uint64_t)A.sweep0 + (uint64_t)sw + 1) % (uint64_t)A.pt_every == 0;
+        if (pt_due && G_::PAIR && A.use_spw) {
+            exchange += 1;                                 // done by the warps of the colour-1 half sweep above
+        } else if (pt_due) {
             const int lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
             for (int t = warp; t < NT; t += nwarp) {
                 int U, M;
@@ -710,13 +920,21 @@ template <int L>
 static cudaError_t launch_l(sg_ctx *c, const LadderArgs &A, int threads, size_t smem, cudaStream_t st, int grid)
 {
     if (attr_needed(c, ATTR_LADDER + L / 2 - 2)) {       // L = 4..16 -> ids 1..7
-        cudaError_t e = cudaFuncSetAttribute(k_ladder_pmj<L, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(k_ladder_pmj<L, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
+        const void *f[4] = {(const void *)k_ladder_pmj<L, false, false>, (const void *)k_ladder_pmj<L, false, true>,
+                            (const void *)k_ladder_pmj<L, true, false>, (const void *)k_ladder_pmj<L, true, true>};
+        for (int i = 0; i < 4; ++i) {
+            cudaError_t e = cudaFuncSetAttribute(f[i], cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+            if (e != cudaSuccess) return e;
+        }
     }
-    if (A.d.bs_accept) k_ladder_pmj<L, true><<<grid, threads, smem, st>>>(A);
-    else k_ladder_pmj<L, false><<<grid, threads, smem, st>>>(A);
+    const bool pt = A.pt_every > 0;
+    if (A.d.bs_accept) {
+        if (pt) k_ladder_pmj<L, true, true><<<grid, threads, smem, st>>>(A);
+        else k_ladder_pmj<L, true, false><<<grid, threads, smem, st>>>(A);
+    } else {
+        if (pt) k_ladder_pmj<L, false, true><<<grid, threads, smem, st>>>(A);
+        else k_ladder_pmj<L, false, false><<<grid, threads, smem, st>>>(A);
+    }
     return cudaGetLastError();
 }
 
@@ -763,7 +981,11 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchang
     }
     if (threads > maxt) return -1;
     size_t smem = ladder_smem_bytes(d.L, d.NT);
-    A.use_tab = smem + ladder_tab_bytes(d.L) <= (size_t)227 * 1024 ? 1 : 0;
+    const bool pair = (d.L / 2) % 4 != 0 && (d.L / 2) % 2 == 0;                 // Geo<L>::PAIR
+    const size_t spw_bytes = 16 + (size_t)Q * 72;                               // 9 offset pairs per quad
+    A.use_spw = pair && smem + spw_bytes <= (size_t)227 * 1024 ? 1 : 0;
+    A.use_tab = !A.use_spw && smem + ladder_tab_bytes(d.L) <= (size_t)227 * 1024 ? 1 : 0;
+    if (A.use_spw) smem += spw_bytes;
     if (A.use_tab) smem += ladder_tab_bytes(d.L);
     const int grid = d.W * d.R;
     cudaError_t e;
