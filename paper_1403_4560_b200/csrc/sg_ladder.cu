@@ -34,6 +34,8 @@ struct LadderArgs {
     int32_t *M;
     unsigned long long *pt_acc;
     int use_tab;              // shared memory has room for the energy tables (neighbour indices + gathered couplings)
+    int n_full;               // CTAs [0, n_full) own a whole ladder; launches without exchanges may split the last ladders
+                              // of the grid into two CTAs each (half of the slots) so that the last wave fills the SMs
     int use_spw;              // pair layout: room for the offset table of the system-per-warp exchange half sweep
 };
 
@@ -251,9 +253,18 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     uint32_t *JgT = reinterpret_cast<uint32_t *>(idxT + H);                                                     // [H][6]
     uint2 *spwT = reinterpret_cast<uint2 *>(idxT);        // [9][Q] byte offsets of the colour-1 quads (use_spw; instead of idxT / JgT)
 
-    const int w = blockIdx.x / d.R, a = blockIdx.x % d.R;
+    int lad = blockIdx.x, tlo = 0, ntl = NT;               // this CTA: slots [tlo, tlo + ntl) of ladder `lad`
+    if constexpr (!PT && G_::PAIR) {
+        if ((int)blockIdx.x >= A.n_full) {
+            const int idx = (int)blockIdx.x - A.n_full;
+            lad = A.n_full + (idx >> 1);
+            tlo = (idx & 1) ? NT / 2 : 0;
+            ntl = (idx & 1) ? NT - NT / 2 : NT / 2;
+        }
+    }
+    const int w = lad / d.R, a = lad % d.R;
     const int tid = threadIdx.x, nthr = blockDim.x;
-    uint32_t *gS = A.spins + ((size_t)(w * d.R + a) * NT) * N;
+    uint32_t *gS = A.spins + ((size_t)(w * d.R + a) * NT + tlo) * N;
     const uint32_t *gJ = A.J + (size_t)w * 3 * N;
 
     // ---- load the ladder, the couplings and the threshold constants
@@ -262,7 +273,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
         const uint4 *js = reinterpret_cast<const uint4 *>(gJ);
         if constexpr (G_::PAIR) {                              // quad i of a colour block -> its low and high pair
             uint2 *dst = reinterpret_cast<uint2 *>(S), *jd = reinterpret_cast<uint2 *>(Jsm);
-            for (int i = tid; i < NT * N / 4; i += nthr) {
+            for (int i = tid; i < ntl * N / 4; i += nthr) {
                 const int blk = i / Q, qd = i - blk * Q;
                 const uint4 v = src[i];
                 dst[blk * (2 * Q) + qd] = make_uint2(v.x, v.y);
@@ -450,7 +461,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                 const uint32_t *Joth = Jsm + ((1 - colour) * 3) * H;
                 const int lane_ = tid & 31, warp_ = tid >> 5, NW = nthr >> 5;
                 const int rank = (warp_ & 3) * (NW >> 2) + (warp_ >> 2);
-                const int I = NB * NT;
+                const int I = NB * ntl;                  // (ntl = NT unless this CTA owns half a ladder)
                 const int i1 = (rank + 1) * I / NW;
                 int qq = 0;
                 bool qa = false;
@@ -663,10 +674,10 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         }
                     } else {
                     const int i0 = rank * I / NW;
-                    int b = i0 / NT, t = i0 - b * NT;
+                    int b = i0 / ntl, t = i0 - b * ntl;         // t: index among this CTA's slots
 #pragma unroll 1
                     for (int i = i0; i < i1;) {
-                        if (t == NT) { t = 0; ++b; }
+                        if (t == ntl) { t = 0; ++b; }
                         {
                             qq = 32 * b + lane_;
                             qa = qq < Q;
@@ -704,17 +715,17 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                             }
                         }
                         // the systems t .. tend - 1 of this block, two per trip (the second one at a compile-time offset)
-                        const int tend = min(NT, t + (i1 - i));
+                        const int tend = min(ntl, t + (i1 - i));
                         i += tend - t;
                         uint32_t *Sa = S + t * N + colour * H;
                         const uint32_t *So = S + t * N + (1 - colour) * H;
 #pragma unroll 1
                         for (; t + 1 < tend; t += 2, Sa += 2 * N, So += 2 * N) {
-                            item(t, Sa, So);
-                            item(t + 1, Sa + N, So + N);
+                            item(tlo + t, Sa, So);
+                            item(tlo + t + 1, Sa + N, So + N);
                         }
                         if (t < tend) {
-                            item(t, Sa, So);
+                            item(tlo + t, Sa, So);
                             ++t;
                         }
                     }
@@ -886,7 +897,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
         uint4 *dst = reinterpret_cast<uint4 *>(gS);
         if constexpr (G_::PAIR) {
             const uint2 *src = reinterpret_cast<const uint2 *>(S);
-            for (int i = tid; i < NT * N / 4; i += nthr) {
+            for (int i = tid; i < ntl * N / 4; i += nthr) {
                 const int blk = i / Q, qd = i - blk * Q;
                 const uint2 lo = src[blk * (2 * Q) + qd], hi = src[blk * (2 * Q) + Q + qd];
                 dst[i] = make_uint4(lo.x, lo.y, hi.x, hi.y);
@@ -987,7 +998,20 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchang
     A.use_tab = !A.use_spw && smem + ladder_tab_bytes(d.L) <= (size_t)227 * 1024 ? 1 : 0;
     if (A.use_spw) smem += spw_bytes;
     if (A.use_tab) smem += ladder_tab_bytes(d.L);
-    const int grid = d.W * d.R;
+    int grid = d.W * d.R;
+    A.n_full = grid;
+    if (pair && pt_every == 0 && d.NT >= 2) {
+        // plain sweeps, one CTA per SM: if the last wave of ladders fills at most half of the SMs, each of its ladders
+        // goes to two CTAs (C3: 512 ladders on 148 SMs = 3 waves + 68 -> 136 half ladders: 3.5 instead of 4 wave times)
+        int dev = 0, n_sm = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        const int tail = n_sm > 0 ? grid % n_sm : 0;
+        if (grid > n_sm && tail > 0 && 2 * tail <= n_sm) {
+            A.n_full = grid - tail;
+            grid = A.n_full + 2 * tail;
+        }
+    }
     cudaError_t e;
     switch (d.L) {
     case 4: e = launch_l<4>(c, A, threads, smem, c->stream, grid); break;
