@@ -136,7 +136,7 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void *src, uint32_
 template <int P, bool ENERGY, bool BS>
 __device__ __forceinline__ void quad_update(uint32_t sa, uint32_t so, uint32_t qb, const Geo32 &g, const Quad6 &Jq,
                                             const uint4 r4, const SlotK &K, uint32_t amask, uint32_t one, uint32_t mone,
-                                            int lane, uint32_t (&accU)[8], uint32_t (&accM)[7])
+                                            int lane, uint32_t (&accU)[8], uint32_t (&accM)[7], uint4 *gst)
 {
     const uint4 sv = lds128(sa + qb);
     const uint4 o0 = lds128(so + qb);
@@ -178,6 +178,12 @@ __device__ __forceinline__ void quad_update(uint32_t sa, uint32_t so, uint32_t q
         }
     }
     sts128(sa + qb, make_uint4(out[0], out[1], out[2], out[3]));
+    if (gst) {
+        // last half sweep of the launch (colour 1): this quad and the colour-0 quad at the same index are final, so they
+        // go to global memory from the registers now and the write-back overlaps the rest of the half sweep
+        gst[RQ] = make_uint4(out[0], out[1], out[2], out[3]);
+        gst[0] = o0;
+    }
     if (ENERGY) {
         uint32_t ab[4], cd[4], U5[5];
         bs_sum<3>(w[0], w[1], ab);
@@ -329,7 +335,7 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
             Jq.zm = lds128(jc + 2560);
             const uint32_t qb = geo.tb + 4096u * (uint32_t)(2 * it + zhalf);
             quad_update<P, ENERGY, BS>(sa, so, qb, geo, Jq, philox_rk8(qb >> 4, time, wglob, c3, A.rk), K, amask, A.one,
-                                   A.mone, lane, accU, accM);
+                                   A.mone, lane, accU, accM, hs == n_half - 1 ? gO + (qb >> 4) : nullptr);
             // Refill the stage two steps ahead only now: every lane has CONSUMED its coupling registers, so the
             // shared-memory loads of the stage have completed (a load that is merely issued could still be in the
             // LSU queue when the bulk copy, which runs on a different engine, overwrites the stage).
@@ -369,9 +375,8 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
         }
     }
 
-    // ---- write back (plain vector stores: a bulk-async store would hold the CTA until its completion — measured slower)
-#pragma unroll 8
-    for (int i = 0; i < 2 * RQ / R_THREADS; ++i) gO[i * R_THREADS + tid] = S4[i * R_THREADS + tid];
+    // (the state went back to global memory quad by quad during the last half sweep, see quad_update; a bulk-async
+    // store at this point would hold the CTA until its completion — measured slower, as was a plain store loop)
 }
 
 // canonical couplings J[w][colour][dir][H] -> packed copy (see above); one thread per packed uint4
