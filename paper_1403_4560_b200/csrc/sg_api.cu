@@ -48,7 +48,9 @@ Layout make_layout(int L, int n_samples, int R, int NT, int kind)
     lo.tps = lo.J6 = 0;
     if (kind != SG_GAUSS) {
         lo.spins = take((size_t)W * R * NT * N * 4);
-        lo.spins_alt = (kind == SG_PMJ && L == 32) ? take((size_t)W * R * NT * N * 4) : 0;   // k_res32_pmj reads one buffer, writes the other
+        // second state buffer: k_res32_pmj reads one buffer and writes the other; so do the ladder launches of sg_run (L <= 16)
+        // that a measurement follows
+        lo.spins_alt = (kind == SG_PMJ && (L == 32 || L <= 16)) ? take((size_t)W * R * NT * N * 4) : 0;
         lo.J = take((size_t)W * 3 * N * 4);
         lo.Jp = (kind == SG_PMJ && L == 32) ? take(res32_packed_bytes(W)) : 0;
         if (kind == SG_PMJ_TPACK) {
@@ -408,7 +410,11 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     char *b = (char *)c->ws;
     c->spins = (uint32_t *)(b + lo.spins);
     c->spins8 = (int8_t *)(b + lo.spins);
-    c->spins_alt = (coupling_kind == SG_PMJ && L == 32) ? (uint32_t *)(b + lo.spins_alt) : nullptr;
+    c->spins_alt = (coupling_kind == SG_PMJ && (L == 32 || L <= 16)) ? (uint32_t *)(b + lo.spins_alt) : nullptr;
+    c->stream2 = nullptr;
+    c->ev_state = nullptr;
+    c->ev_read[0] = c->ev_read[1] = nullptr;
+    c->read_pending[0] = c->read_pending[1] = false;
     c->J = (uint32_t *)(b + lo.J);
     c->Jg = (float *)(b + lo.J);
     c->Jp = (coupling_kind == SG_PMJ && L == 32) ? (uint4 *)(b + lo.Jp) : nullptr;
@@ -502,23 +508,82 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
         return check_launch(c, "run kernels");
     }
     if (ladder8_supported(c) || ladder_supported(c) || gladder_supported(c)) {
-        // sweeps and the exchanges between them are fused in one launch; launches end at measurements
+        // sweeps and the exchanges between them are fused in one launch; launches end at measurements.
+        // +-J: a launch that a measurement follows leaves the state in the SECOND buffer; the measurement then runs on a
+        // stream of its own and reads that buffer while the next launch (which reads it too) fills the first one again -
+        // measurement CTAs take the SMs and shared memory the ladder CTAs leave free (C3: the last, 46 % full wave).
+        const bool overlap = meas_every > 0 && c->kind == SG_PMJ && c->spins_alt && measure_fused_supported(c) &&
+                             (ladder8_supported(c) || ladder_supported(c));
+        if (overlap && !c->stream2) {
+            if ((rc = check_cuda(c, cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking), "stream2"))) return rc;
+            cudaEventCreateWithFlags(&c->ev_state, cudaEventDisableTiming);
+            cudaEventCreateWithFlags(&c->ev_read[0], cudaEventDisableTiming);
+            cudaEventCreateWithFlags(&c->ev_read[1], cudaEventDisableTiming);
+        }
+        auto buf_id = [&](const uint32_t *p) { return p == std::min(c->spins, c->spins_alt) ? 0 : 1; };
+        // An overlapped measurement is SUBMITTED after the next ladder launch, so that the ladder CTAs are placed first
+        // and the measurement CTAs fill what is left; it still sees the buffer and the sweep counter it belongs to.
+        bool deferred = false;
+        uint32_t *def_buf = nullptr;
+        uint64_t def_sweeps = 0;
+        auto submit_deferred = [&]() -> int {
+            if (!deferred) return SG_OK;
+            deferred = false;
+            int r = check_cuda(c, cudaStreamWaitEvent(c->stream2, c->ev_state, 0), "wait state");
+            if (r) return r;
+            uint32_t *cur = c->spins;
+            const uint64_t cur_sweeps = c->sweeps;
+            c->spins = def_buf;
+            c->sweeps = def_sweeps;
+            std::swap(c->stream, c->stream2);
+            r = do_measure(c, nullptr);
+            std::swap(c->stream, c->stream2);
+            c->spins = cur;
+            c->sweeps = cur_sweeps;
+            if (r) return r;
+            if ((r = check_cuda(c, cudaEventRecord(c->ev_read[buf_id(def_buf)], c->stream2), "record measurement"))) return r;
+            c->read_pending[buf_id(def_buf)] = true;
+            return SG_OK;
+        };
         while (left > 0) {
             uint64_t run = (uint64_t)left;
             if (meas_every > 0) run = std::min<uint64_t>(run, (uint64_t)meas_every - c->sweeps % (uint64_t)meas_every);
-            const int k = ladder8_supported(c) ? launch_ladder8_pmj(c, c->sweeps, c->exchanges, (int)run, pt_every)
+            const bool meas_after = meas_every > 0 && (c->sweeps + run) % (uint64_t)meas_every == 0;
+            uint32_t *out = overlap && meas_after ? c->spins_alt : c->spins;
+            if (overlap && deferred && out == def_buf)               // (a launch in place on the buffer a deferred measurement reads)
+                if ((rc = submit_deferred())) return rc;
+            if (overlap && c->read_pending[buf_id(out)]) {          // a measurement may still be reading the buffer this launch writes
+                if ((rc = check_cuda(c, cudaStreamWaitEvent(c->stream, c->ev_read[buf_id(out)], 0), "wait measurement"))) return rc;
+                c->read_pending[buf_id(out)] = false;
+            }
+            const int k = ladder8_supported(c) ? launch_ladder8_pmj(c, c->sweeps, c->exchanges, (int)run, pt_every, out)
                           : gladder_supported(c) ? launch_gladder(c, c->sweeps, (int)run, c->exchanges, pt_every)
-                                                 : launch_ladder_pmj(c, c->sweeps, (int)run, c->exchanges, pt_every);
+                                                 : launch_ladder_pmj(c, c->sweeps, (int)run, c->exchanges, pt_every, out);
             if (k < 0) return check_launch(c, "ladder kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "ladder kernel launch failed");
+            if (out != c->spins) std::swap(c->spins, c->spins_alt);
             c->launches += k;
             if (pt_every > 0) c->exchanges += (c->sweeps + run) / (uint64_t)pt_every - c->sweeps / (uint64_t)pt_every;
             c->sweeps += run;
             // the kernel publishes its own energies when an exchange follows its last sweep
             c->um_fresh = pt_every > 0 && c->sweeps % (uint64_t)pt_every == 0;
             left -= (int)run;
-            if (meas_every > 0 && c->sweeps % (uint64_t)meas_every == 0)
-                if ((rc = do_measure(c, nullptr))) return rc;
+            if ((rc = submit_deferred())) return rc;                // the measurement of the state the launch above started from
+            if (meas_after) {
+                if (overlap) {
+                    if ((rc = check_cuda(c, cudaEventRecord(c->ev_state, c->stream), "record state"))) return rc;
+                    deferred = true;
+                    def_buf = c->spins;
+                    def_sweeps = c->sweeps;
+                } else if ((rc = do_measure(c, nullptr))) return rc;
+            }
         }
+        if ((rc = submit_deferred())) return rc;
+        if (overlap)                                                  // everything after sg_run is ordered after the measurements
+            for (int b = 0; b < 2; ++b)
+                if (c->read_pending[b]) {
+                    if ((rc = check_cuda(c, cudaStreamWaitEvent(c->stream, c->ev_read[b], 0), "join measurement"))) return rc;
+                    c->read_pending[b] = false;
+                }
         return check_launch(c, "run kernels");
     }
     while (left > 0) {
@@ -552,6 +617,13 @@ int sg_destroy(sg_ctx *c)
 {
     if (!c) return SG_EINVAL;
     cudaStreamSynchronize(c->stream);
+    if (c->stream2) {
+        cudaStreamSynchronize(c->stream2);
+        cudaEventDestroy(c->ev_state);
+        cudaEventDestroy(c->ev_read[0]);
+        cudaEventDestroy(c->ev_read[1]);
+        cudaStreamDestroy(c->stream2);
+    }
     if (c->own_ws) cudaFree(c->ws);
     if (c->pq) cudaFree(c->pq);
     if (c->acc_win) cudaFree(c->acc_win);

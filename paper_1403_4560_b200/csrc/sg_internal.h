@@ -56,6 +56,10 @@ struct sg_ctx {
     double h;
     uint64_t seed;
     cudaStream_t stream;
+    cudaStream_t stream2;               // measurements that overlap the next ladder launch (sg_run); created lazily
+    cudaEvent_t ev_state;               // main stream: the state a measurement reads is complete
+    cudaEvent_t ev_read[2];             // stream2: the last measurement reading buffer b (0: lower address) has finished
+    bool read_pending[2];
     std::vector<double> temps, beta;
     std::vector<uint64_t> thr;          // [NT][7][2]
     std::string err;
@@ -71,7 +75,9 @@ struct sg_ctx {
     size_t ws_bytes;
     bool own_ws;
     uint32_t *spins;                    // PMJ: [W][R][NT][2][H] colour-compacted words (the CURRENT state)
-    uint32_t *spins_alt;                // PMJ, L = 32: second state buffer; k_res32_pmj reads `spins`, writes `spins_alt`, then they swap
+    uint32_t *spins_alt;                // PMJ, L = 32: second state buffer; k_res32_pmj reads `spins`, writes `spins_alt`, then they swap.
+                                        // PMJ, L <= 16: the ladder launches of sg_run do the same when a measurement follows them, so that
+                                        // the measurement (on `stream2`) can read one buffer while the next launch fills the other
     uint32_t *J;                        // PMJ: [W][2][3][H]
     uint32_t *tps;                      // SG_PMJ_TPACK: [S][R][NW][2][H] temperature-packed state (sg_tpack.cu)
     uint8_t *J6;                        // SG_PMJ_TPACK: [S][2][H] six bond bits per site
@@ -111,11 +117,12 @@ int launch_init_gauss(sg_ctx *c);
 int launch_sweep_pmj(sg_ctx *c, uint64_t sweep);            // both colours
 int launch_sweep_gauss(sg_ctx *c, uint64_t sweep);
 bool ladder_supported(const sg_ctx *c);                    // shared-memory-resident ladder kernel usable?
-int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0 = 0, int pt_every = 0);   // 1 launch (-1 on error)
+// spins_out: where the launch leaves the state (nullptr = in place)
+int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0 = 0, int pt_every = 0, uint32_t *spins_out = nullptr);   // 1 launch (-1 on error)
 bool gladder_supported(const sg_ctx *c);                   // Gaussian ladder kernel (L = 8, 16) with fused exchanges
 int launch_gladder(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0 = 0, int pt_every = 0);   // 1 launch (-1 on error)
 bool ladder8_supported(const sg_ctx *c);                   // L = 8 kernel with fused parallel tempering
-int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_sweeps, int pt_every);
+int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_sweeps, int pt_every, uint32_t *spins_out = nullptr);
 bool res32_supported(const sg_ctx *c);                     // L = 32: one system resident per SM, couplings streamed from L2
 size_t res32_packed_bytes(int W);
 int launch_pack_J_res32(sg_ctx *c);                        // J -> Jp

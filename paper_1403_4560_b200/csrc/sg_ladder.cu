@@ -17,7 +17,8 @@ namespace sg {
 
 struct LadderArgs {
     Dims d;
-    uint32_t *spins;
+    uint32_t *spins;          // state the launch starts from
+    uint32_t *spins_out;      // where it leaves the state (the same buffer, or the second one: see sg_run)
     const uint32_t *J;
     const SlotTab *tab;
     uint32_t rk[20];          // Philox round keys: rk[2r] = k0 + r*0x9E3779B9, rk[2r+1] = k1 + r*0xBB67AE85
@@ -265,6 +266,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     const int w = lad / d.R, a = lad % d.R;
     const int tid = threadIdx.x, nthr = blockDim.x;
     uint32_t *gS = A.spins + ((size_t)(w * d.R + a) * NT + tlo) * N;
+    uint32_t *gOut = A.spins_out + ((size_t)(w * d.R + a) * NT + tlo) * N;
     const uint32_t *gJ = A.J + (size_t)w * 3 * N;
 
     // ---- load the ladder, the couplings and the threshold constants
@@ -894,7 +896,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     for (int t = tid; t < NT; t += nthr)
         if (accs[t]) atomicAdd(&A.pt_acc[t], (unsigned long long)accs[t]);
     {
-        uint4 *dst = reinterpret_cast<uint4 *>(gS);
+        uint4 *dst = reinterpret_cast<uint4 *>(gOut);
         if constexpr (G_::PAIR) {
             const uint2 *src = reinterpret_cast<const uint2 *>(S);
             for (int i = tid; i < ntl * N / 4; i += nthr) {
@@ -951,12 +953,13 @@ static cudaError_t launch_l(sg_ctx *c, const LadderArgs &A, int threads, size_t 
 
 // n_sweeps consecutive sweeps starting at global sweep index `sweep0`, with the exchanges that fall due fused in
 // (pt_every > 0; first exchange index exchange0); returns kernels launched (or -1)
-int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0, int pt_every)
+int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0, int pt_every, uint32_t *spins_out)
 {
     const Dims &d = c->d;
     LadderArgs A;
     A.d = d;
     A.spins = c->spins;
+    A.spins_out = spins_out ? spins_out : c->spins;
     A.J = c->J;
     A.tab = c->tab;
     for (int r = 0; r < 10; ++r) {

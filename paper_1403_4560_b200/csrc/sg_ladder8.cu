@@ -22,7 +22,8 @@ namespace sg {
 
 struct Ladder8Args {
     Dims d;
-    uint32_t *spins;
+    uint32_t *spins;          // state the launch starts from
+    uint32_t *spins_out;      // where it leaves the state (the same buffer, or the second one: see sg_run)
     const uint32_t *J;
     const SlotTab *tab;
     const double *exp_tab;
@@ -178,6 +179,7 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
     const int w = blockIdx.x / d.R, a = blockIdx.x % d.R;
     const int tid = threadIdx.x, nthr = blockDim.x;
     uint32_t *gS = A.spins + ((size_t)(w * d.R + a) * NT) * N;
+    uint32_t *gOut = A.spins_out + ((size_t)(w * d.R + a) * NT) * N;
     const uint32_t *gJ = A.J + (size_t)w * 3 * N;
 
     // ---- load (global compact order -> slot order)
@@ -354,7 +356,7 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
     // ---- write back (slot order -> global compact order)
     for (int i = tid; i < NT * 128; i += nthr) {
         const int qq = i & 63, tc = i >> 6;
-        reinterpret_cast<uint4 *>(gS)[i] = reinterpret_cast<const uint4 *>(S)[tc * 64 + slot_of_row(qq & 7, qq >> 3)];
+        reinterpret_cast<uint4 *>(gOut)[i] = reinterpret_cast<const uint4 *>(S)[tc * 64 + slot_of_row(qq & 7, qq >> 3)];
     }
 }
 
@@ -375,7 +377,7 @@ bool ladder8_supported(const sg_ctx *c)
 
 // n_sweeps sweeps (global indices sweep0...) with the exchanges that fall due (pt_every; 0 = none).
 // Returns kernels launched (1) or -1.  The caller advances its sweep / exchange counters.
-int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_sweeps, int pt_every)
+int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_sweeps, int pt_every, uint32_t *spins_out)
 {
     if (attr_needed(c, ATTR_LADDER8)) {
         bool ok = true;
@@ -388,6 +390,7 @@ int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_swe
     Ladder8Args A;
     A.d = d;
     A.spins = c->spins;
+    A.spins_out = spins_out ? spins_out : c->spins;
     A.J = c->J;
     A.tab = c->tab;
     A.exp_tab = c->exp64_tab;
