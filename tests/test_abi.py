@@ -44,7 +44,11 @@ def test_workspace_bytes_and_validation_without_gpu():
     assert lib.sg_workspace_bytes(4, 1, 3, 8, 0) == 0          # replicas not in {2,4}
     assert lib.sg_workspace_bytes(4, 1, 4, 0, 0) == 0
     assert lib.sg_workspace_bytes(4, 1, 4, 8, 3) == 0          # unknown coupling_kind (0, 1, 2 exist)
-    assert lib.sg_workspace_bytes(4, 1, 4, 8, 2) > lib.sg_workspace_bytes(4, 1, 4, 8, 0)   # SG_PMJ_TPACK adds its own state copy
+    # SG_PMJ_TPACK keeps the sample-packed state AND its own temperature-packed copy; SG_PMJ (L <= 16, L = 32) keeps a
+    # second sample-packed buffer instead (overlapped measurements / swap on load): both exceed one state (4096 B here)
+    one_state = 1 * 4 * 8 * 64 * 4
+    assert lib.sg_workspace_bytes(4, 1, 4, 8, 2) > one_state and lib.sg_workspace_bytes(4, 1, 4, 8, 0) > 2 * one_state
+    assert lib.sg_workspace_bytes(4, 1, 4, 8, 2) != lib.sg_workspace_bytes(4, 1, 4, 8, 0)
     c1 = lib.sg_workspace_bytes(4, 1, 4, 8, 0)
     assert c1 >= 8 * 1024 and c1 % 256 == 0
     # config 5: 2 x ~4.3 GB bit-packed state (double-buffered for the L = 32 kernel) + couplings + scratch, far below 180 GB
