@@ -412,6 +412,8 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     c->spins8 = (int8_t *)(b + lo.spins);
     c->spins_alt = (coupling_kind == SG_PMJ && (L == 32 || L <= 16)) ? (uint32_t *)(b + lo.spins_alt) : nullptr;
     c->stream2 = nullptr;
+    c->stream_hi = nullptr;
+    c->ev_join = nullptr;
     c->ev_state = nullptr;
     c->ev_read[0] = c->ev_read[1] = nullptr;
     c->read_pending[0] = c->read_pending[1] = false;
@@ -515,7 +517,13 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
         const bool overlap = meas_every > 0 && c->kind == SG_PMJ && c->spins_alt && measure_fused_supported(c) &&
                              (ladder8_supported(c) || ladder_supported(c));
         if (overlap && !c->stream2) {
-            if ((rc = check_cuda(c, cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking), "stream2"))) return rc;
+            // the ladder launches of an overlapped run go to a HIGH-priority stream of the library, the measurements to a
+            // low-priority one: the block scheduler then places a measurement CTA only where no ladder CTA fits
+            int lo_pri = 0, hi_pri = 0;
+            cudaDeviceGetStreamPriorityRange(&lo_pri, &hi_pri);
+            if ((rc = check_cuda(c, cudaStreamCreateWithPriority(&c->stream_hi, cudaStreamNonBlocking, hi_pri), "stream_hi"))) return rc;
+            if ((rc = check_cuda(c, cudaStreamCreateWithPriority(&c->stream2, cudaStreamNonBlocking, lo_pri), "stream2"))) return rc;
+            cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming);
             cudaEventCreateWithFlags(&c->ev_state, cudaEventDisableTiming);
             cudaEventCreateWithFlags(&c->ev_read[0], cudaEventDisableTiming);
             cudaEventCreateWithFlags(&c->ev_read[1], cudaEventDisableTiming);
@@ -545,6 +553,13 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
             c->read_pending[buf_id(def_buf)] = true;
             return SG_OK;
         };
+        cudaStream_t user_stream = c->stream;
+        if (overlap) {                                              // the library's streams start where the caller's stream is
+            if ((rc = check_cuda(c, cudaEventRecord(c->ev_join, user_stream), "record entry"))) return rc;
+            if ((rc = check_cuda(c, cudaStreamWaitEvent(c->stream_hi, c->ev_join, 0), "wait entry"))) return rc;
+            c->stream = c->stream_hi;
+        }
+        auto run_loop = [&]() -> int {
         while (left > 0) {
             uint64_t run = (uint64_t)left;
             if (meas_every > 0) run = std::min<uint64_t>(run, (uint64_t)meas_every - c->sweeps % (uint64_t)meas_every);
@@ -584,6 +599,15 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
                     if ((rc = check_cuda(c, cudaStreamWaitEvent(c->stream, c->ev_read[b], 0), "join measurement"))) return rc;
                     c->read_pending[b] = false;
                 }
+        return SG_OK;
+        };
+        rc = run_loop();
+        if (overlap) {                                              // ... and the caller's stream continues after both
+            c->stream = user_stream;
+            if (!rc) rc = check_cuda(c, cudaEventRecord(c->ev_join, c->stream_hi), "record exit");
+            if (!rc) rc = check_cuda(c, cudaStreamWaitEvent(user_stream, c->ev_join, 0), "wait exit");
+        }
+        if (rc) return rc;
         return check_launch(c, "run kernels");
     }
     while (left > 0) {
@@ -623,6 +647,9 @@ int sg_destroy(sg_ctx *c)
         cudaEventDestroy(c->ev_read[0]);
         cudaEventDestroy(c->ev_read[1]);
         cudaStreamDestroy(c->stream2);
+        cudaStreamSynchronize(c->stream_hi);
+        cudaStreamDestroy(c->stream_hi);
+        cudaEventDestroy(c->ev_join);
     }
     if (c->own_ws) cudaFree(c->ws);
     if (c->pq) cudaFree(c->pq);

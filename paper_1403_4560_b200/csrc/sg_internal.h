@@ -57,7 +57,9 @@ struct sg_ctx {
     uint64_t seed;
     cudaStream_t stream;
     cudaStream_t stream2;               // measurements that overlap the next ladder launch (sg_run); created lazily
-    cudaEvent_t ev_state;               // main stream: the state a measurement reads is complete
+    cudaStream_t stream_hi;             // the ladder launches of such a run (high priority; joined with `stream` at both ends of sg_run)
+    cudaEvent_t ev_join;
+    cudaEvent_t ev_state;               // ladder stream: the state a measurement reads is complete
     cudaEvent_t ev_read[2];             // stream2: the last measurement reading buffer b (0: lower address) has finished
     bool read_pending[2];
     std::vector<double> temps, beta;

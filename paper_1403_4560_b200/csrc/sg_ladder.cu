@@ -586,7 +586,6 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         const bool left_lo = e1 == 1, left_hi = ((NT - e1) & 1) != 0;      // slots without a partner this time
                         const int ntask = npairs + ((left_lo || left_hi) ? 1 : 0);
                         const bool last = sw == A.n_sweeps - 1;
-                        const uint32_t *Tw = reinterpret_cast<const uint32_t *>(spwT);
                         for (int task = warp_; task < ntask; task += NW) {
                             const bool paired = task < npairs;
                             int tA, tB;
@@ -607,12 +606,15 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                                 qq = 32 * kb + lane_;
                                 qa = true;
                                 if (qq < Q) {
+                                    uint2 tk[9];                              // entry k of both pairs of the quad: one 64-bit load
+#pragma unroll
+                                    for (int k = 0; k < 9; ++k) tk[k] = spwT[k * Q + qq];
 #pragma unroll
                                     for (int hh = 0; hh < 2; ++hh) {
                                         const int o = hh * Q2 + 2 * qq;
                                         uint32_t ee[9];
 #pragma unroll
-                                        for (int k = 0; k < 9; ++k) ee[k] = Tw[(k * Q + qq) * 2 + hh];
+                                        for (int k = 0; k < 9; ++k) ee[k] = hh ? tk[k].y : tk[k].x;
 #pragma unroll
                                         for (int k = 0; k < 6; ++k) ip[hh][k] = (int)(ee[k] >> 2);
                                         const char *Jb = reinterpret_cast<const char *>(Jsm);
