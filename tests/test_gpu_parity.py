@@ -382,3 +382,103 @@ def test_fuzzed_shapes_run_vs_oracle(sg, O, case):
         assert close(mom[s], want)
     assert sim.sg_get_counters()[0] == n1 + n2
     sim.close()
+
+
+# ---- round 2, last session: pair layout / warp-per-pair exchange (L = 4, 12), half ladders in the last wave, overlapped
+# measurements
+
+
+@pytest.mark.parametrize("L,h,NT,R,pt_every,n_samples", [(12, 0.1, 1, 2, 1, 32), (12, -0.2, 2, 2, 1, 33), (12, 0.3, 3, 4, 1, 32),
+                                                       (12, 0.1, 6, 2, 2, 64), (12, 0.0, 7, 4, 1, 32), (4, 0.3, 2, 2, 1, 40),
+                                                       (4, -0.3, 9, 4, 1, 32), (4, 0.2, 20, 2, 3, 65)])
+def test_pair_layout_ladder_odd_and_tiny_ladders(sg, O, L, h, NT, R, pt_every, n_samples):
+    """k_ladder_pmj<4 | 12> (pair layout; exchange half sweep by one warp per pair of slots): ladders with one slot, an
+    odd number of slots (a slot without a partner at both parities of the exchange), more pairs than warps, 2 and 4
+    replicas, h = 0 (carry-chain compare) — spins, the kernel's own (U, M) after an exchange, accepted-swap counts and
+    moments vs the oracle."""
+    temps = W.ladder(0.6, 1.7, NT)
+    samples = sorted({0, n_samples - 1, n_samples // 2})
+    sim, orc = make_pair(sg, O, L, h, n_samples, R, temps, 0, 77, samples)
+    n = 12 if pt_every == 1 else 12 * pt_every // 2
+    sim.sg_run(n, pt_every, 4)
+    for o in orc.values():
+        o.run(n, pt_every, 4)
+    check_state(sim, orc, "pair-layout ladder")
+    if n % pt_every == 0 and NT > 1:
+        Uc, Mc = sim.sg_get_energies_cached()          # the kernel's own energies, permuted by the last exchange
+        for s, o in orc.items():
+            Uo, Mo = o.energies()
+            assert np.array_equal(Uc[s], Uo) and np.array_equal(Mc[s], Mo)
+    mom, nm = sim.sg_get_moments()
+    assert nm == n // 4
+    for s, o in orc.items():
+        assert close(mom[s], o.moments()[0])
+    sim.sg_sweep(3)                                    # instantiation without exchange code, from the same state
+    for o in orc.values():
+        o.sweep(3)
+    check_state(sim, orc, "pair-layout ladder + plain sweeps")
+    sim.close()
+
+
+@pytest.mark.parametrize("L,NT,R,n_samples", [(4, 4, 4, 39 * 32), (12, 2, 2, 77 * 32)])
+def test_half_ladders_in_the_last_wave(sg, O, L, NT, R, n_samples):
+    """Plain sweeps with more ladders than SMs and a last wave that fills at most half of them (156 / 154 ladders on 148
+    SMs): its ladders are split over two CTAs.  Samples of the first, a middle and the LAST words (the split ones) vs the
+    oracle, and the whole pool vs the generic path by state hash."""
+    temps = W.ladder(0.5, 1.8, NT)
+    nw = (n_samples + 31) // 32
+    samples = sorted({0, 31, 32 * (nw // 2) + 7, 32 * (nw - 2) + 1, 32 * (nw - 1), n_samples - 1})
+    sim, orc = make_pair(sg, O, L, 0.2, n_samples, R, temps, 0, 5, samples)
+    sim.sg_sweep(5)
+    for o in orc.values():
+        o.sweep(5)
+    check_state(sim, orc, "half ladders")
+    h_fast = sim.sg_get_state_hash()
+    sim.close()
+    gen = sg.Simulation(L, 0.2, n_samples, R, temps, 0, 5)
+    gen.sg_set_kernel_path(sg.PATH_GENERIC)
+    gen.sg_sweep(5)
+    assert np.array_equal(gen.sg_get_state_hash(), h_fast)
+    gen.close()
+
+
+@pytest.mark.parametrize("L,NT,R,n_samples", [(8, 6, 4, 64), (12, 4, 4, 32), (4, 5, 2, 33), (16, 3, 2, 32)])
+def test_overlapped_measurements_equal_serial_ones(sg, O, L, NT, R, n_samples):
+    """sg_run with a measurement cadence overlaps every measurement with the next ladder launch (second state buffer,
+    two library streams).  Run segments that start and end between measurements, interleaved with other calls, must give
+    the moments, the state and the records of the same schedule done with sg_run(.., 0) + sg_measure (no overlap), and
+    both must equal the oracle."""
+    temps = W.ladder(0.5, 1.9, NT)
+    samples = sorted({0, n_samples - 1})
+    a, orc = make_pair(sg, O, L, 0.25, n_samples, R, temps, 0, 9, samples)
+    b = sg.Simulation(L, 0.25, n_samples, R, temps, 0, 9)
+    segs = [21, 3, 8, 1, 16, 7]                      # measurement every 8 sweeps: after sweeps 8, 16, 24, 32, 40, 48, 56
+    for i, n in enumerate(segs):
+        a.sg_run(n, 1, 8)
+        if i == 2:
+            a.sg_get_spins(0, 1)                     # a reader between two overlapped runs
+    done = 0
+    for n in segs:
+        left = n
+        while left:
+            step = min(left, 8 - done % 8)
+            b.sg_run(step, 1, 0)
+            done += step
+            left -= step
+            if done % 8 == 0:
+                b.sg_measure(False)
+    for o in orc.values():
+        o.run(sum(segs), 1, 8)
+    check_state(a, orc, "overlapped measurements")
+    assert np.array_equal(a.sg_get_state_hash(), b.sg_get_state_hash())
+    ma, na = a.sg_get_moments()
+    mb, nb = b.sg_get_moments()
+    assert na == nb == sum(segs) // 8
+    assert np.array_equal(ma, mb), "overlapped and serial measurements accumulate different moments"
+    for s, o in orc.items():
+        assert close(ma[s], o.moments()[0])
+    ra = a.sg_measure()                              # records from the current buffer after an overlapped run
+    rb = b.sg_measure()
+    assert np.array_equal(ra, rb)
+    a.close()
+    b.close()
