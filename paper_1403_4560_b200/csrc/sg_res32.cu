@@ -123,6 +123,15 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         "D_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
 }
 
+// true in exactly one lane of a converged warp (elect.sync): the bulk-copy issue below stays a warp-uniform region —
+// with `lane == 0` ptxas wraps the uniform-operand UBLKCP in an ELECT loop over the active lanes
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
+
 // one lane: arm the barrier with the byte count and start the bulk copy global -> shared
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
 {
@@ -340,7 +349,7 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
             // shared-memory loads of the stage have completed (a load that is merely issued could still be in the
             // LSU queue when the bulk copy, which runs on a different engine, overwrites the stage).
             __syncwarp();
-            if (lane == 0) {
+            if (elect_one()) {
                 if (it + 2 < R_ITERS) issue(hs, it + 2);
                 else if (hs + 1 < n_half) issue(hs + 1, it + 2 - R_ITERS);
             }
