@@ -178,7 +178,10 @@ __global__ void __launch_bounds__(512, 1) k_gladder(const __grid_constant__ GLad
                 const int q_zm = (z == 0) ? q + (L - 1) * L * QR : q - L * QR;
                 const int m_out = p ? (4 * kq + 4 == Lh ? 0 : 4 * kq + 4) : (kq == 0 ? Lh - 1 : 4 * kq - 1);
                 const int side_idx = r * Lh + m_out;
-                long long jf[6][4], jtot = 0;                                          // [+x, -x, +y, -y, +z, -z][element]
+                // -J_fix of the 24 bonds as DOUBLES: |J_fix| < 2^36 and every partial sum of a system stays below 2^53, so the
+                // additions below are exact (= the int64 sum in any order, R14).  S_i S_j = -1 flips the sign bit of the
+                // addend (one shift + one LOP3 on the high word) and the sum runs on the FP64 pipe, not on the ALU pipe.
+                double njf[6][4];                                                      // [+x, -x, +y, -y, +z, -z][element]
                 {
                     const float4 jx = reinterpret_cast<const float4 *>(Jown)[q];
                     const float4 jox = reinterpret_cast<const float4 *>(Joth)[q];
@@ -194,10 +197,8 @@ __global__ void __launch_bounds__(512, 1) k_gladder(const __grid_constant__ GLad
 #pragma unroll
                     for (int k = 0; k < 6; ++k)
 #pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            jf[k][e] = __double2ll_rz(__dmul_rn((double)Jv[k][e], 4294967296.0));
-                            jtot += jf[k][e];
-                        }
+                        for (int e = 0; e < 4; ++e)
+                            njf[k][e] = -(double)__double2ll_rz(__dmul_rn((double)Jv[k][e], 4294967296.0));
                 }
 #pragma unroll 1
                 for (int t = g; t < NT; t += A.G) {
@@ -209,17 +210,16 @@ __global__ void __launch_bounds__(512, 1) k_gladder(const __grid_constant__ GLad
                     const uint32_t wxp = p ? ((o0 >> 8) | (sb << 24)) : o0;
                     const uint32_t wxm = p ? o0 : ((o0 << 8) | sb);
                     const uint32_t dw[6] = {sv ^ wxp, sv ^ wxm, sv ^ oyp, sv ^ oym, sv ^ ozp, sv ^ ozm};   // byte sign bit: S_i != S_j
-                    long long D = 0;
+                    double ed[4] = {0.0, 0.0, 0.0, 0.0};                               // four chains (exact, so the order is free)
 #pragma unroll
                     for (int k = 0; k < 6; ++k)
 #pragma unroll
                         for (int e = 0; e < 4; ++e) {
-                            uint32_t m32;                                          // sign of byte e replicated over the word: -1 iff S_i != S_j
-                            asm("prmt.b32 %0, %1, %2, %3;" : "=r"(m32) : "r"(dw[k]), "r"(0u), "r"(0x8888u | (0x1111u * (unsigned)e)));
-                            const long long m = (long long)(int)m32;
-                            D += jf[k][e] & m;
+                            const uint32_t sgn = sgn_of(dw[k], e);                     // 0x80000000 iff S_i != S_j
+                            const double term = __hiloint2double(__double2hiint(njf[k][e]) ^ (int)sgn, __double2loint(njf[k][e]));
+                            ed[e] = __dadd_rn(ed[e], term);                            // -J S_i S_j
                         }
-                    long long ev = 2 * D - jtot;
+                    long long ev = __double2ll_rz(__dadd_rn(__dadd_rn(ed[0], ed[1]), __dadd_rn(ed[2], ed[3])));
                     int mv = __dp4a((int)sv, 0x01010101, __dp4a((int)o0, 0x01010101, 0));
                     for (int o = 16; o; o >>= 1) {
                         ev += __shfl_xor_sync(0xffffffffu, ev, o);
