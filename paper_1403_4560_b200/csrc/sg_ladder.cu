@@ -37,6 +37,9 @@ struct LadderArgs {
     int use_tab;              // shared memory has room for the energy tables (neighbour indices + gathered couplings)
     int n_full;               // CTAs [0, n_full) own a whole ladder; launches without exchanges may split the last ladders
                               // of the grid into two CTAs each (half of the slots) so that the last wave fills the SMs
+    int nt_res;               // slots resident in one CTA: NT, or ceil(NT / 2) when every ladder is split over two CTAs (`split`)
+    int split;                // 1: every ladder is split (launches with exchanges: the two CTAs form a cluster and the slot pair
+                              // across them exchanges through distributed shared memory)
     int use_spw;              // pair layout: room for the offset table of the system-per-warp exchange half sweep
 };
 
@@ -233,6 +236,30 @@ __device__ __forceinline__ void ladder_energy_tab(const uint32_t *__restrict__ S
     M = 2 * (int)bs_warp_total(bigM, PM, lane) - N;
 }
 
+// ---- thread-block cluster helpers (split ladders): barrier over both CTAs, loads from the partner's shared memory
+__device__ __forceinline__ void cluster_sync()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t dsmem_addr(const void *p, int rank)
+{
+    uint32_t a = (uint32_t)__cvta_generic_to_shared(p), r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ uint32_t ld_dsmem(const void *p, int rank)
+{
+    uint32_t v;
+    asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(dsmem_addr(p, rank)) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint4 ld_dsmem4(const void *p, int rank)
+{
+    uint4 v;
+    asm volatile("ld.shared::cluster.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(dsmem_addr(p, rank)) : "memory");
+    return v;
+}
+
 // PT = false: the instantiation for launches without exchanges (pt_every == 0), all exchange code compiled out
 template <int L, bool BS, bool PT>
 __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const __grid_constant__ LadderArgs A)
@@ -242,8 +269,8 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     extern __shared__ __align__(16) uint32_t smem[];
     const Dims &d = A.d;
     const int NT = d.NT;
-    uint32_t *S = smem;                                   // [NT][2][H]
-    uint32_t *Jsm = S + (size_t)NT * N;                   // [2][3][H]
+    uint32_t *S = smem;                                   // [nt_res][2][H]: the slots this CTA owns
+    uint32_t *Jsm = S + (size_t)A.nt_res * N;             // [2][3][H]
     uint2 *thr = reinterpret_cast<uint2 *>(Jsm + 3 * N);  // [NT][8]
     int *Uint = reinterpret_cast<int *>(thr + NT * 8);    // [NT][32]   exchange scratch (pt_every > 0 only)
     int *Mint = Uint + NT * 32;                           // [NT][32]
@@ -254,15 +281,18 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     uint32_t *JgT = reinterpret_cast<uint32_t *>(idxT + H);                                                     // [H][6]
     uint2 *spwT = reinterpret_cast<uint2 *>(idxT);        // [9][Q] byte offsets of the colour-1 quads (use_spw; instead of idxT / JgT)
 
-    int lad = blockIdx.x, tlo = 0, ntl = NT;               // this CTA: slots [tlo, tlo + ntl) of ladder `lad`
-    if constexpr (!PT && G_::PAIR) {
-        if ((int)blockIdx.x >= A.n_full) {
-            const int idx = (int)blockIdx.x - A.n_full;
-            lad = A.n_full + (idx >> 1);
-            tlo = (idx & 1) ? NT / 2 : 0;
-            ntl = (idx & 1) ? NT - NT / 2 : NT / 2;
-        }
+    // this CTA: slots [tlo, tlo + ntl) of ladder `lad`.  CTAs [0, n_full) own whole ladders, the rest come in pairs that
+    // share a ladder (first half of the slots rounded up, second half)
+    int lad = blockIdx.x, tlo = 0, ntl = NT, half = 0;
+    if ((int)blockIdx.x >= A.n_full) {
+        const int idx = (int)blockIdx.x - A.n_full;
+        lad = A.n_full + (idx >> 1);
+        half = idx & 1;
+        const int nt0 = (NT + 1) / 2;
+        tlo = half ? nt0 : 0;
+        ntl = half ? NT - nt0 : nt0;
     }
+    const bool split_pt = PT && A.split != 0;              // the partner CTA (cluster rank 1 - half) holds the other slots
     const int w = lad / d.R, a = lad % d.R;
     const int tid = threadIdx.x, nthr = blockDim.x;
     uint32_t *gS = A.spins + ((size_t)(w * d.R + a) * NT + tlo) * N;
@@ -289,7 +319,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
             }
         } else {
             uint4 *dst = reinterpret_cast<uint4 *>(S);
-            for (int i = tid; i < NT * N / 4; i += nthr) dst[i] = src[i];
+            for (int i = tid; i < ntl * N / 4; i += nthr) dst[i] = src[i];
             uint4 *jd = reinterpret_cast<uint4 *>(Jsm);
             for (int i = tid; i < 3 * N / 4; i += nthr) jd[i] = js[i];
         }
@@ -417,9 +447,10 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         Jzm[0] = joz.x; Jzm[1] = joz.y; Jzm[2] = joz.z; Jzm[3] = joz.w;
                     }
 #pragma unroll 1
-                    for (int t = g; t < NT; t += A.G) {
-                        uint32_t *Sa = S + t * N + colour * H;
-                        const uint32_t *So = S + t * N + (1 - colour) * H;
+                    for (int tl = g; tl < ntl; tl += A.G) {
+                        const int t = tlo + tl;
+                        uint32_t *Sa = S + tl * N + colour * H;
+                        const uint32_t *So = S + tl * N + (1 - colour) * H;
                         const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[q];
                         const uint4 o0 = reinterpret_cast<const uint4 *>(So)[q];
                         const uint4 oyp = reinterpret_cast<const uint4 *>(So)[q_yp];
@@ -739,10 +770,11 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                     int ix[4][6];
                     uint32_t Jq[4][6];
                     const int i0 = rank * I / NW;
-                    int b = i0 / NT, t = i0 - b * NT;
+                    int b = i0 / ntl, tl = i0 - b * ntl;        // tl: index among this CTA's slots
 #pragma unroll 1
-                    for (int i = i0; i < i1; ++i, ++t) {
-                        if (t == NT) { t = 0; ++b; }
+                    for (int i = i0; i < i1; ++i, ++tl) {
+                        if (tl == ntl) { tl = 0; ++b; }
+                        const int t = tlo + tl;
                         if (b != bcur) {
                             bcur = b;
                             qq = 32 * b + lane_;
@@ -768,45 +800,15 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                                 Jq[e][4] = Jown[2 * H + n];  Jq[e][5] = Joth[2 * H + zm];
                             }
                         }
-                        uint32_t *Sa = S + t * N + colour * H;
-                        const uint32_t *So = S + t * N + (1 - colour) * H;
+                        uint32_t *Sa = S + tl * N + colour * H;
+                        const uint32_t *So = S + tl * N + (1 - colour) * H;
                         const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[qq];
                         uint32_t v[4][6];
-                        if constexpr (Lh % 2 == 0) {
-                            // even rows: elements (0,1) and (2,3) sit in one row at an even index, so every neighbour
-                            // except the side one is an aligned 64-bit pair
-                            // a z-plane is a whole number of quads when L is a multiple of 4: the same-index and the +-z neighbours of
-                            // the quad are then one aligned 128-bit load each
-                            constexpr bool QZ = (L * Lh) % 4 == 0;
-                            if constexpr (QZ) {
-                                const uint4 a0 = *reinterpret_cast<const uint4 *>(So + ix[0][0]);
-                                const uint4 a4 = *reinterpret_cast<const uint4 *>(So + ix[0][4]);
-                                const uint4 a5 = *reinterpret_cast<const uint4 *>(So + ix[0][5]);
-                                v[0][0] = a0.x; v[1][0] = a0.y; v[2][0] = a0.z; v[3][0] = a0.w;
-                                v[0][4] = a4.x; v[1][4] = a4.y; v[2][4] = a4.z; v[3][4] = a4.w;
-                                v[0][5] = a5.x; v[1][5] = a5.y; v[2][5] = a5.z; v[3][5] = a5.w;
-                            }
+                        // (rows of an odd number of words: nothing is aligned beyond the quad itself)
 #pragma unroll
-                            for (int e = 0; e < 4; e += 2) {
+                        for (int e = 0; e < 4; ++e)
 #pragma unroll
-                                for (int k = 0; k < 6; ++k) {
-                                    if (QZ && (k == 0 || k >= 4)) continue;
-                                    if (k == 1) {
-                                        v[e][1] = So[ix[e][1]];
-                                        v[e + 1][1] = So[ix[e + 1][1]];
-                                    } else {
-                                        const uint2 pr = *reinterpret_cast<const uint2 *>(So + ix[e][k]);
-                                        v[e][k] = pr.x;
-                                        v[e + 1][k] = pr.y;
-                                    }
-                                }
-                            }
-                        } else {
-#pragma unroll
-                            for (int e = 0; e < 4; ++e)
-#pragma unroll
-                                for (int k = 0; k < 6; ++k) v[e][k] = So[ix[e][k]];
-                        }
+                            for (int k = 0; k < 6; ++k) v[e][k] = So[ix[e][k]];
                         const uint4 r4 = philox_rk((uint32_t)qq, time, wglob, ctr3(3, a, t), A.rk);
                         SlotK K;
                         {
@@ -837,19 +839,35 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
             exchange += 1;                                 // done by the warps of the colour-1 half sweep above
         } else if (pt_due) {
             const int lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
-            for (int t = warp; t < NT; t += nwarp) {
+            for (int tl = warp; tl < ntl; tl += nwarp) {               // energies of the slots this CTA owns
                 int U, M;
-                if (A.use_tab) ladder_energy_tab<L>(S + t * N, idxT, JgT, lane, U, M);
-                else ladder_energy<L>(S + t * N, Jsm, lane, U, M);
-                Uint[t * 32 + lane] = U;
-                Mint[t * 32 + lane] = M;
+                if (A.use_tab) ladder_energy_tab<L>(S + tl * N, idxT, JgT, lane, U, M);
+                else ladder_energy<L>(S + tl * N, Jsm, lane, U, M);
+                Uint[(tlo + tl) * 32 + lane] = U;
+                Mint[(tlo + tl) * 32 + lane] = M;
             }
-            __syncthreads();
             const int e1 = (int)(exchange & 1u);
             const int npairs = (NT - e1) / 2;
-            for (int item = tid; item < npairs * 32; item += nthr) {       // whole warps
+            // split ladder: the pair (tb, tb + 1) lies across the two CTAs of the cluster (tb = last slot of the first
+            // half); it is exchanged this time iff tb has the parity of the exchange
+            const int tb = (NT + 1) / 2 - 1;
+            const bool cross = split_pt && tb >= e1 && ((tb - e1) & 1) == 0 && tb + 1 < NT;
+            const int t_mine = half ? tb + 1 : tb, t_other = half ? tb : tb + 1;      // the cross pair's slots: mine, the partner's
+            __syncthreads();
+            if (cross) {
+                // the partner's energies of its slot of the cross pair -> my copy of the tables (distributed shared memory)
+                cluster_sync();
+                if (tid < 32) {
+                    Uint[t_other * 32 + tid] = (int)ld_dsmem(Uint + t_other * 32 + tid, 1 - half);
+                    Mint[t_other * 32 + tid] = (int)ld_dsmem(Mint + t_other * 32 + tid, 1 - half);
+                }
+                __syncthreads();
+            }
+            const int t_end = tlo + ntl;
+            for (int item = tid; item < npairs * 32; item += nthr) {       // whole warps; a cross pair is decided by both CTAs
                 const int pair = item >> 5, ln = item & 31;
                 const int t = e1 + 2 * pair;
+                if (t + 1 < tlo || t >= t_end) continue;                   // neither slot is mine (warp-uniform)
                 const int smp = w * 32 + ln;
                 const int U0 = Uint[t * 32 + ln], U1 = Uint[(t + 1) * 32 + ln];
                 const int M0 = Mint[t * 32 + ln], M1 = Mint[(t + 1) * 32 + ln];
@@ -859,12 +877,15 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                 const uint4 r = philox_rk(0u, (uint32_t)exchange, (uint32_t)(smp + d.s_first), ctr3(4, a, t), A.rk);
                 const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
                 const uint32_t mask = __ballot_sync(0xffffffffu, accept && smp < d.n_samples);
-                if (ln == 0) { masks[pair] = mask; accs[t] += (uint32_t)__popc(mask); }
+                if (ln == 0) {
+                    masks[pair] = mask;
+                    if (t >= tlo) accs[t] += (uint32_t)__popc(mask);       // counted by the CTA that owns the lower slot
+                }
             }
             __syncthreads();
             if (sw == A.n_sweeps - 1) {
-                for (int item = tid; item < NT * 32; item += nthr) {       // publish the energies, permuted like the configurations
-                    const int t = item >> 5, ln = item & 31;
+                for (int item = tid; item < ntl * 32; item += nthr) {      // publish the energies, permuted like the configurations
+                    const int t = tlo + (item >> 5), ln = item & 31;
                     const int p = t - e1;
                     int src = t;
                     if (p >= 0 && (p >> 1) < npairs && ((masks[p >> 1] >> ln) & 1u)) src = (p & 1) ? t - 1 : t + 1;
@@ -873,13 +894,14 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                     A.M[o] = Mint[src * 32 + ln];
                 }
             }
-            for (int item = tid; item < npairs * (N / 4); item += nthr) {  // masked swap of the two configurations
+            for (int item = tid; item < npairs * (N / 4); item += nthr) {  // masked swap of the two configurations (both mine)
                 const int pair = item / (N / 4), k = item - pair * (N / 4);
+                const int t = e1 + 2 * pair;
+                if (t < tlo || t + 1 >= t_end) continue;
                 const uint32_t mask = masks[pair];
                 if (mask == 0u) continue;
-                const int t = e1 + 2 * pair;
-                uint4 *X = reinterpret_cast<uint4 *>(S + t * N) + k;
-                uint4 *Y = reinterpret_cast<uint4 *>(S + (t + 1) * N) + k;
+                uint4 *X = reinterpret_cast<uint4 *>(S + (t - tlo) * N) + k;
+                uint4 *Y = reinterpret_cast<uint4 *>(S + (t + 1 - tlo) * N) + k;
                 uint4 xv = *X, yv = *Y;
                 uint32_t dd;
                 dd = (xv.x ^ yv.x) & mask; xv.x ^= dd; yv.x ^= dd;
@@ -888,6 +910,31 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                 dd = (xv.w ^ yv.w) & mask; xv.w ^= dd; yv.w ^= dd;
                 *X = xv;
                 *Y = yv;
+            }
+            if (cross) {
+                // the cross pair: every thread merges the partner's lanes into its words of my slot — remote reads first,
+                // a cluster barrier (the partner reads MY old words meanwhile), then the local writes
+                const uint32_t mask = masks[(tb - e1) >> 1];
+                uint4 *X = reinterpret_cast<uint4 *>(S + (t_mine - tlo) * N);
+                const uint4 *Yr = reinterpret_cast<const uint4 *>(S + (t_other - (half ? 0 : tlo + ntl)) * N);   // its local address there
+                constexpr int PER = (N / 4 + Geo<L>::MAXT - 1) / Geo<L>::MAXT + 1;
+                uint4 keep[PER];
+                int n_keep = 0;
+                if (mask != 0u)
+#pragma unroll
+                    for (int j = 0; j < PER; ++j) {
+                        const int k = tid + j * nthr;
+                        if (k < N / 4) {
+                            const uint4 xv = X[k], yv = ld_dsmem4(Yr + k, 1 - half);
+                            keep[j] = make_uint4(xv.x ^ ((xv.x ^ yv.x) & mask), xv.y ^ ((xv.y ^ yv.y) & mask),
+                                                 xv.z ^ ((xv.z ^ yv.z) & mask), xv.w ^ ((xv.w ^ yv.w) & mask));
+                            n_keep = j + 1;
+                        }
+                    }
+                cluster_sync();
+#pragma unroll
+                for (int j = 0; j < PER; ++j)
+                    if (j < n_keep) X[tid + j * nthr] = keep[j];
             }
             exchange += 1;
             __syncthreads();
@@ -908,27 +955,33 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
             }
         } else {
             const uint4 *src = reinterpret_cast<const uint4 *>(S);
-            for (int i = tid; i < NT * N / 4; i += nthr) dst[i] = src[i];
+            for (int i = tid; i < ntl * N / 4; i += nthr) dst[i] = src[i];
         }
     }
 }
 
 // ------------------------------------------------------------------------------- host side
-size_t ladder_smem_bytes(int L, int NT)
+// nt_res slots resident in the CTA; the per-slot tables (thresholds, exchange scratch) cover all NT slots
+size_t ladder_smem_bytes(int L, int NT, int nt_res)
 {
     const size_t N = (size_t)L * L * L;
-    return (size_t)NT * N * 4 + 3 * N * 4 + (size_t)NT * 8 * sizeof(uint2) + (size_t)NT * 32 * 8 + (size_t)(NT / 2 + 1) * 4 + (size_t)NT * 4;
+    return (size_t)nt_res * N * 4 + 3 * N * 4 + (size_t)NT * 8 * sizeof(uint2) + (size_t)NT * 32 * 8 + (size_t)(NT / 2 + 1) * 4 + (size_t)NT * 4;
 }
 
 // + the energy tables of ladder_energy_tab: 16 (indices) + 24 (couplings) bytes per colour-0 site, 16-byte aligned
 static size_t ladder_tab_bytes(int L) { return 16 + (size_t)(L * L * L / 2) * 40; }
+
+// A ladder that does not fit in the shared memory of one SM is split over a cluster of two CTAs (first half of the slots
+// rounded up, second half); the slot pair across the two exchanges through distributed shared memory.
+static bool ladder_needs_split(const Dims &d) { return ladder_smem_bytes(d.L, d.NT, d.NT) > (size_t)227 * 1024; }
 
 bool ladder_supported(const sg_ctx *c)
 {
     const Dims &d = c->d;
     if (c->path != SG_PATH_AUTO || c->kind != SG_PMJ || !d.fast_accept) return false;
     if (d.L != 4 && d.L != 6 && d.L != 8 && d.L != 10 && d.L != 12 && d.L != 16) return false;
-    return ladder_smem_bytes(d.L, d.NT) <= (size_t)227 * 1024;
+    if (!ladder_needs_split(d)) return true;
+    return d.NT >= 2 && ladder_smem_bytes(d.L, d.NT, (d.NT + 1) / 2) <= (size_t)227 * 1024;
 }
 
 template <int L>
@@ -943,6 +996,23 @@ static cudaError_t launch_l(sg_ctx *c, const LadderArgs &A, int threads, size_t 
         }
     }
     const bool pt = A.pt_every > 0;
+    if (pt && A.split) {
+        // split ladders with exchanges: the two CTAs of a ladder are a thread-block cluster (distributed shared memory)
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)grid);
+        cfg.blockDim = dim3((unsigned)threads);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = 2;
+        at[0].val.clusterDim.y = 1;
+        at[0].val.clusterDim.z = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        return A.d.bs_accept ? cudaLaunchKernelEx(&cfg, k_ladder_pmj<L, true, true>, A)
+                             : cudaLaunchKernelEx(&cfg, k_ladder_pmj<L, false, true>, A);
+    }
     if (A.d.bs_accept) {
         if (pt) k_ladder_pmj<L, true, true><<<grid, threads, smem, st>>>(A);
         else k_ladder_pmj<L, true, false><<<grid, threads, smem, st>>>(A);
@@ -981,38 +1051,45 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchang
     A.M = c->M;
     A.pt_acc = c->pt_acc;
     const int Q = d.N / 8;
-    // groups: as many as fit in <= 512 threads, at most NT, preferring a divisor of NT
+    A.split = ladder_needs_split(d) ? 1 : 0;
+    A.nt_res = A.split ? (d.NT + 1) / 2 : d.NT;
+    // groups: as many as fit in <= 512 threads, at most the resident slots, preferring a divisor of their number
     const int maxt = d.L == 8 ? 320 : ((d.L / 2) % 4 == 0 ? 512 : 384);
-    int G = std::max(1, std::min(d.NT, maxt / Q));
+    int G = std::max(1, std::min(A.nt_res, maxt / Q));
     for (int gtry = G; gtry >= 1 && gtry * 2 > G; --gtry)
-        if (d.NT % gtry == 0) { G = gtry; break; }
+        if (A.nt_res % gtry == 0) { G = gtry; break; }
     A.G = G;
     int threads = (Q * G + 31) / 32 * 32;
     if ((d.L / 2) % 4 != 0) {
         // generic lattices: balanced warp items (block of 32 quads, system); a multiple of four warps, at most 12
-        const int items = (Q + 31) / 32 * d.NT;
+        const int items = (Q + 31) / 32 * A.nt_res;
         // (measured at C3: 12 warps with 130 registers beat 16 with 116 and 20 with 96 - the kernel is bound by ALU-pipe
         // and issue throughput, not by latency)
         threads = 32 * std::min(12, (items + 3) / 4 * 4);
     }
     if (threads > maxt) return -1;
-    size_t smem = ladder_smem_bytes(d.L, d.NT);
+    if (A.split && ((d.N / 4 + maxt - 1) / maxt + 1) * threads < d.N / 4) return -1;   // (cross-pair swap: PER quads per thread)
+    size_t smem = ladder_smem_bytes(d.L, d.NT, A.nt_res);
     const bool pair = (d.L / 2) % 4 != 0 && (d.L / 2) % 2 == 0;                 // Geo<L>::PAIR
     const size_t spw_bytes = 16 + (size_t)Q * 72;                               // 9 offset pairs per quad
-    A.use_spw = pair && smem + spw_bytes <= (size_t)227 * 1024 ? 1 : 0;
+    A.use_spw = pair && !A.split && smem + spw_bytes <= (size_t)227 * 1024 ? 1 : 0;
     A.use_tab = !A.use_spw && smem + ladder_tab_bytes(d.L) <= (size_t)227 * 1024 ? 1 : 0;
     if (A.use_spw) smem += spw_bytes;
     if (A.use_tab) smem += ladder_tab_bytes(d.L);
     int grid = d.W * d.R;
     A.n_full = grid;
-    if (pair && pt_every == 0 && d.NT >= 2) {
+    if (A.split) {
+        A.n_full = 0;
+        grid *= 2;
+    } else if (pt_every == 0 && d.NT >= 2) {
         // plain sweeps, one CTA per SM: if the last wave of ladders fills at most half of the SMs, each of its ladders
         // goes to two CTAs (C3: 512 ladders on 148 SMs = 3 waves + 68 -> 136 half ladders: 3.5 instead of 4 wave times)
         int dev = 0, n_sm = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        const int tail = n_sm > 0 ? grid % n_sm : 0;
-        if (grid > n_sm && tail > 0 && 2 * tail <= n_sm) {
+        const int slots = smem > (size_t)113 * 1024 ? n_sm : 0;                // only where one CTA fills an SM
+        const int tail = slots > 0 ? grid % slots : 0;
+        if (slots > 0 && grid > slots && tail > 0 && 2 * tail <= slots) {
             A.n_full = grid - tail;
             grid = A.n_full + 2 * tail;
         }

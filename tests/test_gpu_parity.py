@@ -482,3 +482,43 @@ def test_overlapped_measurements_equal_serial_ones(sg, O, L, NT, R, n_samples):
     assert np.array_equal(ra, rb)
     a.close()
     b.close()
+
+
+@pytest.mark.parametrize("L,NT,R,pt_every,n_samples", [(10, 56, 2, 1, 33), (12, 31, 2, 1, 32), (12, 40, 4, 2, 32), (16, 12, 2, 1, 32),
+                                                     (16, 13, 4, 1, 32), (16, 20, 2, 3, 64)])
+def test_ladders_split_over_a_cluster(sg, O, L, NT, R, pt_every, n_samples):
+    """Ladders that do not fit in the shared memory of one SM: two CTAs of a thread-block cluster own one half of the
+    slots each; the slot pair across them is decided by both from energies read through distributed shared memory and
+    swapped by remote reads + a cluster barrier + local writes.  Even and odd numbers of slots (the cross pair is
+    exchanged at one parity only), exchanges every 1 / 2 / 3 sweeps, plain sweeps from the same state (independent
+    halves) — spins, the kernel's own energies, accepted swaps and moments vs the oracle."""
+    temps = W.ladder(0.6, 1.8, NT)
+    samples = sorted({0, n_samples - 1})
+    sim, orc = make_pair(sg, O, L, 0.15, n_samples, R, temps, 0, 21, samples)
+    n = 6 * pt_every
+    sim.sg_run(n, pt_every, 3 * pt_every)
+    for o in orc.values():
+        o.run(n, pt_every, 3 * pt_every)
+    check_state(sim, orc, "split ladder")
+    Uc, Mc = sim.sg_get_energies_cached()
+    for s, o in orc.items():
+        Uo, Mo = o.energies()
+        assert np.array_equal(Uc[s], Uo) and np.array_equal(Mc[s], Mo), "split ladder: the kernel's own energies"
+    mom, nm = sim.sg_get_moments()
+    assert nm == 2
+    for s, o in orc.items():
+        assert close(mom[s], o.moments()[0])
+    prop, acc = sim.sg_get_pt_stats()
+    assert prop.sum() > 0 and acc.sum() > 0
+    sim.sg_sweep(2); sim.sg_run(3, 1, 0)
+    for o in orc.values():
+        o.sweep(2); o.run(3, 1, 0)
+    check_state(sim, orc, "split ladder + plain sweeps + odd exchange")
+    # the whole pool against the global-memory kernels
+    h_fast = sim.sg_get_state_hash()
+    sim.close()
+    gen = sg.Simulation(L, 0.15, n_samples, R, temps, 0, 21)
+    gen.sg_set_kernel_path(sg.PATH_GENERIC)
+    gen.sg_run(n, pt_every, 3 * pt_every); gen.sg_sweep(2); gen.sg_run(3, 1, 0)
+    assert np.array_equal(gen.sg_get_state_hash(), h_fast)
+    gen.close()
