@@ -106,7 +106,12 @@ int sg_measure(sg_ctx *ctx, double *out);
 /* Fused driver, bit-identical to the primitive sequence (R16):
  *   for s in 1..n_sweeps: sweep; if pt_every>0 and sweeps_done % pt_every == 0: exchange;
  *                                if meas_every>0 and sweeps_done % meas_every == 0: measure(NULL)
- * (sweeps_done = global sweep counter).  Asynchronous. */
+ * (sweeps_done = global sweep counter).  Asynchronous.
+ * Stream order: with a measurement cadence on the +-J ladder paths (L <= 16) the library runs the sweep launches and the
+ * measurements on two streams of its own so that a measurement overlaps the sweeps that follow it (DESIGN.md 5,
+ * "Overlapped measurements"); both are joined with the context's stream at entry and at exit, so for the caller sg_run
+ * behaves like any other call enqueued on `stream`: work enqueued before it is finished when it starts, and everything it
+ * did is finished before work enqueued after it starts. */
 int sg_run(sg_ctx *ctx, int n_sweeps, int pt_every, int meas_every);
 
 /* Block until all enqueued work of this context has finished. */
