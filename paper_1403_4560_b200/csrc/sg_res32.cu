@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(R_THREADS, 1) k_res32_pmj(const __grid_constan
         for (int k = 0; k < 8; ++k) accU[k] = 0;
 #pragma unroll
         for (int k = 0; k < 7; ++k) accM[k] = 0;
-#pragma unroll 1
+#pragma unroll 4
         for (int it = 0; it < R_ITERS; ++it) {
             const int st = it & 1;
             if (hs == 0) {                                  // first half sweep (colour 0): the chunks this step touches have landed?
