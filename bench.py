@@ -36,7 +36,7 @@ HBM_BYTES_PER_WORDSITE_LAUNCH = 8   # spin word read once + written once per LAU
 # `ncu --set full` capture named beside it; a pointer to profiles/, not re-measured by this run
 NCU_TRAFFIC = {"C2": (10.92e6, "profiles/r01_v3_resident_kernels.md"),
                "C3": (114.6e6, "profiles/r02c_kernels.md"),
-               "C5": (8.759e9, "profiles/r02c_kernels.md")}
+               "C5": (8.755e9, "profiles/r02c_kernels.md")}
 ALU_LANES_PER_SM = 64         # INT/LOP3 lanes per SM per clock (16 per SMSP x 4; B300_MICROARCH pipe table)
 N_SM = 148
 
