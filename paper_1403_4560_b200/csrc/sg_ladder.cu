@@ -98,7 +98,14 @@ struct Geo {
     // pair, but not on a quad): no shared-memory bank conflicts, where 64-bit pairs at a 16-byte stride had 2-way ones.
     static constexpr bool PAIR = !VEC && (Lh % 2) == 0;
     // position of compact index n (< H) inside its colour block
-    static __host__ __device__ constexpr int pos(int n) { return PAIR ? ((n >> 1) & 1) * (H / 2) + ((n >> 2) << 1) + (n & 1) : n; }
+    // Rows of an ODD number of words (L = 6, 10): nothing beyond the quad is aligned, every neighbour is a 32-bit access at
+    // a 16-byte stride over the lanes (4-way bank conflicts).  Planar layout: a colour block is kept as four arrays, word e
+    // of every quad; the lanes of a warp (consecutive quads, same e) then touch consecutive words for every neighbour.
+    static constexpr bool PLANAR = !VEC && !PAIR;
+    static __host__ __device__ constexpr int pos(int n)
+    {
+        return PAIR ? ((n >> 1) & 1) * (H / 2) + ((n >> 2) << 1) + (n & 1) : PLANAR ? (n & 3) * Q + (n >> 2) : n;
+    }
     // launch bounds: L=8 runs two 320-thread CTAs per SM (256 ladders of config 2 on 148 SMs)
     static constexpr int MAXT = L == 8 ? 320 : VEC ? 512 : 384;
     static constexpr int MINB = L == 8 ? 2 : 1;
@@ -316,6 +323,19 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                 const uint4 v = js[i];
                 jd[blk * (2 * Q) + qd] = make_uint2(v.x, v.y);
                 jd[blk * (2 * Q) + Q + qd] = make_uint2(v.z, v.w);
+            }
+        } else if constexpr (G_::PLANAR) {                      // quad i of a colour block -> word e to array e
+            for (int i = tid; i < ntl * N / 4; i += nthr) {
+                const int blk = i / Q, qd = i - blk * Q;
+                const uint4 v = src[i];
+                uint32_t *dst = S + blk * H + qd;
+                dst[0] = v.x; dst[Q] = v.y; dst[2 * Q] = v.z; dst[3 * Q] = v.w;
+            }
+            for (int i = tid; i < 3 * N / 4; i += nthr) {
+                const int blk = i / Q, qd = i - blk * Q;
+                const uint4 v = js[i];
+                uint32_t *dst = Jsm + blk * H + qd;
+                dst[0] = v.x; dst[Q] = v.y; dst[2 * Q] = v.z; dst[3 * Q] = v.w;
             }
         } else {
             uint4 *dst = reinterpret_cast<uint4 *>(S);
@@ -793,18 +813,18 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                                 const int zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
                                 // slot 0: the x-neighbour at the same compact index (its bond if p, own bond else); slot 1: the one
                                 // at the side index (own bond if p, its bond else)
-                                ix[e][0] = n; ix[e][1] = sd; ix[e][2] = yp; ix[e][3] = ym; ix[e][4] = zp; ix[e][5] = zm;
-                                Jq[e][0] = p ? Joth[n] : Jown[n];
-                                Jq[e][1] = p ? Jown[n] : Joth[sd];
-                                Jq[e][2] = Jown[H + n];      Jq[e][3] = Joth[H + ym];
-                                Jq[e][4] = Jown[2 * H + n];  Jq[e][5] = Joth[2 * H + zm];
+                                constexpr auto P = G_::pos;                    // planar layout: position of a compact index
+                                ix[e][0] = P(n); ix[e][1] = P(sd); ix[e][2] = P(yp); ix[e][3] = P(ym); ix[e][4] = P(zp); ix[e][5] = P(zm);
+                                Jq[e][0] = p ? Joth[P(n)] : Jown[P(n)];
+                                Jq[e][1] = p ? Jown[P(n)] : Joth[P(sd)];
+                                Jq[e][2] = Jown[H + P(n)];      Jq[e][3] = Joth[H + P(ym)];
+                                Jq[e][4] = Jown[2 * H + P(n)];  Jq[e][5] = Joth[2 * H + P(zm)];
                             }
                         }
                         uint32_t *Sa = S + tl * N + colour * H;
                         const uint32_t *So = S + tl * N + (1 - colour) * H;
-                        const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[qq];
+                        const uint4 sv = make_uint4(Sa[qq], Sa[Q + qq], Sa[2 * Q + qq], Sa[3 * Q + qq]);   // planar: word e in array e
                         uint32_t v[4][6];
-                        // (rows of an odd number of words: nothing is aligned beyond the quad itself)
 #pragma unroll
                         for (int e = 0; e < 4; ++e)
 #pragma unroll
@@ -827,7 +847,9 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                                                  xor3(s[e], v[e][2], Jq[e][2]), xor3(s[e], v[e][3], Jq[e][3]),
                                                  xor3(s[e], v[e][4], Jq[e][4]), xor3(s[e], v[e][5], Jq[e][5]), rr[e], K, A.one,
                                                  A.mone);
-                        if (qa) reinterpret_cast<uint4 *>(Sa)[qq] = make_uint4(out[0], out[1], out[2], out[3]);
+                        if (qa) {
+                            Sa[qq] = out[0]; Sa[Q + qq] = out[1]; Sa[2 * Q + qq] = out[2]; Sa[3 * Q + qq] = out[3];
+                        }
                     }
                 }
             }
@@ -952,6 +974,12 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                 const int blk = i / Q, qd = i - blk * Q;
                 const uint2 lo = src[blk * (2 * Q) + qd], hi = src[blk * (2 * Q) + Q + qd];
                 dst[i] = make_uint4(lo.x, lo.y, hi.x, hi.y);
+            }
+        } else if constexpr (G_::PLANAR) {
+            for (int i = tid; i < ntl * N / 4; i += nthr) {
+                const int blk = i / Q, qd = i - blk * Q;
+                const uint32_t *src = S + blk * H + qd;
+                dst[i] = make_uint4(src[0], src[Q], src[2 * Q], src[3 * Q]);
             }
         } else {
             const uint4 *src = reinterpret_cast<const uint4 *>(S);
