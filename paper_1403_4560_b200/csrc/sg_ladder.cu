@@ -267,10 +267,115 @@ __device__ __forceinline__ uint4 ld_dsmem4(const void *p, int rank)
     return v;
 }
 
-// PT = false: the instantiation for launches without exchanges (pt_every == 0), all exchange code compiled out
-template <int L, bool BS, bool PT>
+// ---- pieces of the exchange half sweep that one warp runs for its own pair of slots (pair and planar layouts)
+// one word-site with the energy bookkeeping: new word and the three planes of its unsatisfied-bond count AFTER the update
+template <bool BS>
+__device__ __forceinline__ uint32_t update_word_energy(uint32_t sx, uint32_t amask, uint32_t u0, uint32_t u1, uint32_t u2, uint32_t u3,
+                                                       uint32_t u4, uint32_t u5, uint32_t r, const SlotK &K, uint32_t one, uint32_t mone,
+                                                       uint32_t (&wpl)[3])
+{
+    uint32_t n0, n1, n2;
+    const uint32_t acc = accept_word<BS>(u0, u1, u2, u3, u4, u5, ~(sx ^ amask), r, K, one, mone, n0, n1, n2);
+    // a flip turns n into 6 - n: bit 0 = n0; bit 1 set for n in {0, 3, 4}; bit 2 set for n in {0, 1, 2}
+    const uint32_t f1 = (~n2 & ~(n1 ^ n0)) | (n2 & ~n1 & ~n0);
+    const uint32_t f2 = ~n2 & ~(n1 & n0);
+    wpl[0] = n0;
+    wpl[1] = (acc & f1) | (~acc & n1);
+    wpl[2] = (acc & f2) | (~acc & n2);
+    return sx ^ acc;
+}
+
+// the four count planes of a quad and its eight spin words (four new, four of the other colour) -> the lane's running totals
+template <int PU, int PM>
+__device__ __forceinline__ void energy_accumulate(const uint32_t (&wpl)[4][3], const uint32_t (&outw)[4], const uint32_t (&othw)[4],
+                                                  uint32_t (&aU)[PU], uint32_t (&aM)[PM])
+{
+    uint32_t ab[4], cd[4], U5[5];
+    bs_sum<3>(wpl[0], wpl[1], ab);
+    bs_sum<3>(wpl[2], wpl[3], cd);
+    bs_sum<4>(ab, cd, U5);
+    bs_add(aU, U5);
+    const uint32_t x1 = xor3(outw[0], outw[1], outw[2]), y1 = maj3(outw[0], outw[1], outw[2]);
+    const uint32_t x2 = xor3(outw[3], othw[0], othw[1]), y2 = maj3(outw[3], othw[0], othw[1]);
+    const uint32_t x3 = xor3(x1, x2, othw[2]), y3 = maj3(x1, x2, othw[2]);
+    const uint32_t ones = x3 ^ othw[3], y4 = x3 & othw[3];
+    const uint32_t t1 = xor3(y1, y2, y3), g1 = maj3(y1, y2, y3);
+    const uint32_t twos = t1 ^ y4, g2 = t1 & y4;
+    const uint32_t M4[4] = {ones, twos, g1 ^ g2, g1 & g2};
+    bs_add(aM, M4);
+}
+
+// which slots task `task` of exchange parity e1 covers: a pair (tA, tA + 1), or the slots without a partner this time
+__device__ __forceinline__ void spw_task(int task, int e1, int NT, int &tA, int &tB, bool &paired)
+{
+    const int npairs = (NT - e1) / 2;
+    const bool left_lo = e1 == 1, left_hi = ((NT - e1) & 1) != 0;
+    paired = task < npairs;
+    if (paired) { tA = e1 + 2 * task; tB = tA + 1; }
+    else if (left_lo && left_hi) { tA = NT - 1; tB = 0; }
+    else { tA = left_lo ? 0 : NT - 1; tB = tA; }
+}
+__device__ __forceinline__ int spw_ntask(int e1, int NT)
+{
+    return (NT - e1) / 2 + ((e1 == 1 || ((NT - e1) & 1) != 0) ? 1 : 0);
+}
+
+// after the warp's lanes walked both systems: per-lane totals, decision (R12), masked swap of the warp's own two systems,
+// accepted-swap count, and (last sweep of the launch) the energies, permuted like the configurations
+template <int L, int PU, int PM>
+__device__ __forceinline__ void spw_finish(const LadderArgs &A, uint32_t *S, uint32_t *accs, const uint32_t (&aU0)[PU],
+                                           const uint32_t (&aM0)[PM], const uint32_t (&aU1)[PU], const uint32_t (&aM1)[PM], int tA, int tB,
+                                           bool paired, bool last, int lane, int w, int a, uint64_t exchange)
+{
+    constexpr int N = L * L * L;
+    const Dims &d = A.d;
+    __syncwarp();
+    const int U0 = (int)bs_warp_total(aU0, PU, lane), M0 = 2 * (int)bs_warp_total(aM0, PM, lane) - N;
+    const int U1 = (int)bs_warp_total(aU1, PU, lane), M1 = 2 * (int)bs_warp_total(aM1, PM, lane) - N;
+    uint32_t mask = 0u;
+    if (paired) {
+        const int smp = w * 32 + lane;
+        const double Et = __dsub_rn((double)(2 * U0 - 3 * N), __dmul_rn(A.h, (double)M0));
+        const double Eu = __dsub_rn((double)(2 * U1 - 3 * N), __dmul_rn(A.h, (double)M1));
+        const double x = __dmul_rn(__dsub_rn(A.tab[tA].beta, A.tab[tB].beta), __dsub_rn(Et, Eu));
+        const uint4 r = philox_rk(0u, (uint32_t)exchange, (uint32_t)(smp + d.s_first), ctr3(4, a, tA), A.rk);
+        const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
+        mask = __ballot_sync(0xffffffffu, accept && smp < d.n_samples);
+        if (lane == 0) accs[tA] += (uint32_t)__popc(mask);
+        if (mask != 0u) {                             // masked swap (layout independent: the same position in both systems)
+            for (int k = lane; k < N / 4; k += 32) {
+                uint4 *X = reinterpret_cast<uint4 *>(S + tA * N) + k;
+                uint4 *Y = reinterpret_cast<uint4 *>(S + tB * N) + k;
+                uint4 xv = *X, yv = *Y;
+                uint32_t dd;
+                dd = (xv.x ^ yv.x) & mask; xv.x ^= dd; yv.x ^= dd;
+                dd = (xv.y ^ yv.y) & mask; xv.y ^= dd; yv.y ^= dd;
+                dd = (xv.z ^ yv.z) & mask; xv.z ^= dd; yv.z ^= dd;
+                dd = (xv.w ^ yv.w) & mask; xv.w ^= dd; yv.w ^= dd;
+                *X = xv;
+                *Y = yv;
+            }
+        }
+    }
+    if (last) {
+        const bool swp = (mask >> lane) & 1u;
+        const size_t oA = ((size_t)(w * 32 + lane) * d.R + a) * d.NT + tA;
+        A.U[oA] = (int64_t)(swp ? U1 : U0);
+        A.M[oA] = swp ? M1 : M0;
+        if (tB != tA) {
+            const size_t oB = ((size_t)(w * 32 + lane) * d.R + a) * d.NT + tB;
+            A.U[oB] = (int64_t)(swp ? U0 : U1);
+            A.M[oB] = swp ? M0 : M1;
+        }
+    }
+}
+
+// PTM: 0 = the instantiation for launches without exchanges (all exchange code compiled out), 1 = exchanges by the recount
+// path (any layout, split ladders), 2 = exchanges by the warp-per-pair half sweep (pair and planar layouts, A.use_spw)
+template <int L, bool BS, int PTM>
 __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const __grid_constant__ LadderArgs A)
 {
+    constexpr bool PT = PTM != 0, SPW = PTM == 2;
     using G_ = Geo<L>;
     constexpr int Lh = G_::Lh, N = G_::N, H = G_::H, Q = G_::Q;
     extern __shared__ __align__(16) uint32_t smem[];
@@ -359,7 +464,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
         for (int t = tid; t < NT; t += nthr) accs[t] = 0u;
     }
     __syncthreads();
-    if (PT && A.use_tab && !A.use_spw && A.pt_every > 0) {      // neighbour indices and couplings of the colour-0 sites, once per launch
+    if (PT && !SPW && A.use_tab && A.pt_every > 0) {      // neighbour indices and couplings of the colour-0 sites, once per launch
         const uint32_t *J0 = Jsm, *J1 = Jsm + 3 * H;
         for (int n = tid; n < H; n += nthr) {
             const int row = n / Lh, m = n - row * Lh;
@@ -381,7 +486,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     }
 
     if constexpr (G_::PAIR) {
-        if (PT && A.use_spw && A.pt_every > 0) {
+        if (SPW && A.pt_every > 0) {
             // Offsets (bytes) for the colour-1 half sweep that precedes an exchange, where a WARP owns two systems and its
             // lanes walk the quads, so nothing can be hoisted into registers.  Per pair hh of quad qd, relative to the
             // other-colour block of the system: +y, -y, +z, -z neighbour pairs and the two side words; relative to the
@@ -410,6 +515,37 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                     uint32_t *T = reinterpret_cast<uint32_t *>(spwT);   // word k of pair hh of quad qd: T[((k * Q) + qd) * 2 + hh]
 #pragma unroll
                     for (int k = 0; k < 9; ++k) T[(k * Q + qd) * 2 + hh] = e[k];
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    if constexpr (G_::PLANAR) {
+        if (SPW && A.pt_every > 0) {
+            // planar layout, exchange half sweep by one warp per pair of slots: positions of the six neighbours and the six
+            // coupling words of every colour-1 site, [element e][neighbour k][quad] (unit-stride over the lanes)
+            uint32_t *ixT = reinterpret_cast<uint32_t *>(spwT), *JgS = ixT + 24 * Q;
+            const uint32_t *Jown = Jsm + 3 * H, *Joth = Jsm;          // colour 1 owns the second coupling block
+            for (int i = tid; i < 4 * Q; i += nthr) {
+                const int e = i / Q, qd = i - e * Q;
+                const int n = 4 * qd + e;
+                const int row = n / Lh, m = n - row * Lh;
+                const int z = row / L, y = row - z * L;
+                const int p = (1 + y + z) & 1;
+                const int sd = row * Lh + (p ? (m + 1 == Lh ? 0 : m + 1) : (m == 0 ? Lh - 1 : m - 1));
+                const int yp = (z * L + (y + 1 == L ? 0 : y + 1)) * Lh + m;
+                const int ym = (z * L + (y == 0 ? L - 1 : y - 1)) * Lh + m;
+                const int zp = ((z + 1 == L ? 0 : z + 1) * L + y) * Lh + m;
+                const int zm = ((z == 0 ? L - 1 : z - 1) * L + y) * Lh + m;
+                constexpr auto P = G_::pos;
+                const int ixv[6] = {P(n), P(sd), P(yp), P(ym), P(zp), P(zm)};
+                const uint32_t jv[6] = {p ? Joth[P(n)] : Jown[P(n)], p ? Jown[P(n)] : Joth[P(sd)], Jown[H + P(n)], Joth[H + P(ym)],
+                                        Jown[2 * H + P(n)], Joth[2 * H + P(zm)]};
+#pragma unroll
+                for (int k = 0; k < 6; ++k) {
+                    ixT[(e * 6 + k) * Q + qd] = (uint32_t)ixv[k];
+                    JgS[(e * 6 + k) * Q + qd] = jv[k];
                 }
             }
             __syncthreads();
@@ -595,37 +731,17 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                             for (int j = 0; j < 2; ++j) {
                                 const int e = 2 * hh + j;
                                 const uint32_t sx = sw2[j];
-                                uint32_t n0, n1, n2;
-                                const uint32_t acc = accept_word<BS>(xor3(sx, a02[j], Jq[e][0]), xor3(sx, sdw[j], Jq[e][1]),
-                                                                     xor3(sx, yp2[j], Jq[e][2]), xor3(sx, ym2[j], Jq[e][3]),
-                                                                     xor3(sx, zp2[j], Jq[e][4]), xor3(sx, zm2[j], Jq[e][5]),
-                                                                     ~(sx ^ amask), rr[e], K, A.one, A.mone, n0, n1, n2);
-                                outw[e] = sx ^ acc;
+                                outw[e] = update_word_energy<BS>(sx, amask, xor3(sx, a02[j], Jq[e][0]), xor3(sx, sdw[j], Jq[e][1]),
+                                                                 xor3(sx, yp2[j], Jq[e][2]), xor3(sx, ym2[j], Jq[e][3]),
+                                                                 xor3(sx, zp2[j], Jq[e][4]), xor3(sx, zm2[j], Jq[e][5]), rr[e], K,
+                                                                 A.one, A.mone, wpl[e]);
                                 othw[e] = a02[j];
-                                // 6 - n: bit 0 = n0; bit 1 set for n in {0, 3, 4}; bit 2 set for n in {0, 1, 2}
-                                const uint32_t f1 = (~n2 & ~(n1 ^ n0)) | (n2 & ~n1 & ~n0);
-                                const uint32_t f2 = ~n2 & ~(n1 & n0);
-                                wpl[e][0] = n0;
-                                wpl[e][1] = (acc & f1) | (~acc & n1);
-                                wpl[e][2] = (acc & f2) | (~acc & n2);
                             }
                             *reinterpret_cast<uint2 *>(Sa + o) = make_uint2(outw[2 * hh], outw[2 * hh + 1]);
                         }
-                        uint32_t ab[4], cd[4], U5[5];
-                        bs_sum<3>(wpl[0], wpl[1], ab);
-                        bs_sum<3>(wpl[2], wpl[3], cd);
-                        bs_sum<4>(ab, cd, U5);
-                        bs_add(aU, U5);
-                        const uint32_t x1 = xor3(outw[0], outw[1], outw[2]), y1 = maj3(outw[0], outw[1], outw[2]);
-                        const uint32_t x2 = xor3(outw[3], othw[0], othw[1]), y2 = maj3(outw[3], othw[0], othw[1]);
-                        const uint32_t x3 = xor3(x1, x2, othw[2]), y3 = maj3(x1, x2, othw[2]);
-                        const uint32_t ones = x3 ^ othw[3], y4 = x3 & othw[3];
-                        const uint32_t t1 = xor3(y1, y2, y3), g1 = maj3(y1, y2, y3);
-                        const uint32_t twos = t1 ^ y4, g2 = t1 & y4;
-                        const uint32_t M4[4] = {ones, twos, g1 ^ g2, g1 & g2};
-                        bs_add(aM, M4);
+                        energy_accumulate(wpl, outw, othw, aU, aM);
                     };
-                    const bool pt_due_now = PT && A.use_spw && colour == 1 && A.pt_every > 0 &&
+                    const bool pt_due_now = SPW && colour == 1 && A.pt_every > 0 &&
                                             ((uint64_t)A.sweep0 + (uint64_t)sw + 1) % (uint64_t)A.pt_every == 0;
                     if (pt_due_now) {
                         // ---- colour-1 half sweep + exchange, one WARP per pair of neighbouring slots: the lanes walk the quads
@@ -633,16 +749,12 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                         // registers, and the warp then decides and swaps its own two systems: no pass over the ladder and no
                         // CTA barrier between the half sweep, the decisions and the swaps.
                         const int e1 = (int)(exchange & 1u);
-                        const int npairs = (NT - e1) / 2;
-                        const bool left_lo = e1 == 1, left_hi = ((NT - e1) & 1) != 0;      // slots without a partner this time
-                        const int ntask = npairs + ((left_lo || left_hi) ? 1 : 0);
+                        const int ntask = spw_ntask(e1, NT);
                         const bool last = sw == A.n_sweeps - 1;
                         for (int task = warp_; task < ntask; task += NW) {
-                            const bool paired = task < npairs;
                             int tA, tB;
-                            if (paired) { tA = e1 + 2 * task; tB = tA + 1; }
-                            else if (left_lo && left_hi) { tA = NT - 1; tB = 0; }
-                            else { tA = left_lo ? 0 : NT - 1; tB = tA; }
+                            bool paired;
+                            spw_task(task, e1, NT, tA, tB, paired);
                             const bool two = tB != tA;
                             const int offB = (tB - tA) * N;
                             uint32_t *SaA = S + tA * N + H;
@@ -687,45 +799,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                                     if (two) itemE(tB, SaA + offB, SoA + offB, aU1, aM1);
                                 }
                             }
-                            __syncwarp();
-                            const int U0 = (int)bs_warp_total(aU0, PU, lane_), M0 = 2 * (int)bs_warp_total(aM0, PM, lane_) - N;
-                            const int U1 = (int)bs_warp_total(aU1, PU, lane_), M1 = 2 * (int)bs_warp_total(aM1, PM, lane_) - N;
-                            uint32_t mask = 0u;
-                            if (paired) {
-                                const int smp = w * 32 + lane_;
-                                const double Et = __dsub_rn((double)(2 * U0 - 3 * N), __dmul_rn(A.h, (double)M0));
-                                const double Eu = __dsub_rn((double)(2 * U1 - 3 * N), __dmul_rn(A.h, (double)M1));
-                                const double x = __dmul_rn(__dsub_rn(A.tab[tA].beta, A.tab[tB].beta), __dsub_rn(Et, Eu));
-                                const uint4 r = philox_rk(0u, (uint32_t)exchange, (uint32_t)(smp + d.s_first), ctr3(4, a, tA), A.rk);
-                                const bool accept = (x >= 0.0) || ((uint64_t)r.x < dexp64(A.exp_tab, -x));
-                                mask = __ballot_sync(0xffffffffu, accept && smp < d.n_samples);
-                                if (lane_ == 0) accs[tA] += (uint32_t)__popc(mask);
-                                if (mask != 0u) {                             // masked swap of the warp's own two systems
-                                    for (int k = lane_; k < N / 4; k += 32) {
-                                        uint4 *X = reinterpret_cast<uint4 *>(S + tA * N) + k;
-                                        uint4 *Y = reinterpret_cast<uint4 *>(S + tB * N) + k;
-                                        uint4 xv = *X, yv = *Y;
-                                        uint32_t dd;
-                                        dd = (xv.x ^ yv.x) & mask; xv.x ^= dd; yv.x ^= dd;
-                                        dd = (xv.y ^ yv.y) & mask; xv.y ^= dd; yv.y ^= dd;
-                                        dd = (xv.z ^ yv.z) & mask; xv.z ^= dd; yv.z ^= dd;
-                                        dd = (xv.w ^ yv.w) & mask; xv.w ^= dd; yv.w ^= dd;
-                                        *X = xv;
-                                        *Y = yv;
-                                    }
-                                }
-                            }
-                            if (last) {                                       // publish the energies, permuted like the configurations
-                                const bool swp = (mask >> lane_) & 1u;
-                                const size_t oA = ((size_t)(w * 32 + lane_) * d.R + a) * NT + tA;
-                                A.U[oA] = (int64_t)(swp ? U1 : U0);
-                                A.M[oA] = swp ? M1 : M0;
-                                if (two) {
-                                    const size_t oB = ((size_t)(w * 32 + lane_) * d.R + a) * NT + tB;
-                                    A.U[oB] = (int64_t)(swp ? U0 : U1);
-                                    A.M[oB] = swp ? M0 : M1;
-                                }
-                            }
+                            spw_finish<L>(A, S, accs, aU0, aM0, aU1, aM1, tA, tB, paired, last, lane_, w, a, exchange);
                         }
                     } else {
                     const int i0 = rank * I / NW;
@@ -784,6 +858,75 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
                             ++t;
                         }
                     }
+                    }
+                } else if (SPW && colour == 1 && A.pt_every > 0 &&
+                           ((uint64_t)A.sweep0 + (uint64_t)sw + 1) % (uint64_t)A.pt_every == 0) {
+                    // ---- planar layout: colour-1 half sweep + exchange, one WARP per pair of neighbouring slots (as in the
+                    // pair layout above; neighbour positions and couplings from the tables built at the start of the launch)
+                    constexpr int PU = NB * 24 < 32 ? 5 : NB * 24 < 64 ? 6 : NB * 24 < 128 ? 7 : NB * 24 < 256 ? 8 : 9;
+                    constexpr int PM = NB * 8 < 16 ? 4 : NB * 8 < 32 ? 5 : NB * 8 < 64 ? 6 : 7;
+                    static_assert(NB * 24 < 512 && NB * 8 < 128, "plane counts");
+                    const uint32_t *ixT = reinterpret_cast<const uint32_t *>(spwT), *JgS = ixT + 24 * Q;
+                    const int e1 = (int)(exchange & 1u);
+                    const int ntask = spw_ntask(e1, NT);
+                    const bool last = sw == A.n_sweeps - 1;
+                    for (int task = warp_; task < ntask; task += NW) {
+                        int tA, tB;
+                        bool paired;
+                        spw_task(task, e1, NT, tA, tB, paired);
+                        const bool two = tB != tA;
+                        const int offB = (tB - tA) * N;
+                        uint32_t *SaA = S + tA * N + H;
+                        const uint32_t *SoA = S + tA * N;
+                        uint32_t aU0[PU], aM0[PM], aU1[PU], aM1[PM];
+#pragma unroll
+                        for (int k = 0; k < PU; ++k) aU0[k] = aU1[k] = 0u;
+#pragma unroll
+                        for (int k = 0; k < PM; ++k) aM0[k] = aM1[k] = 0u;
+#pragma unroll 1
+                        for (int kb = 0; kb < NB; ++kb) {
+                            qq = 32 * kb + lane_;
+                            if (qq < Q) {
+                                uint32_t Jq[4][6];                      // (the positions are re-read per system: registers)
+#pragma unroll
+                                for (int e = 0; e < 4; ++e)
+#pragma unroll
+                                    for (int k = 0; k < 6; ++k) Jq[e][k] = JgS[(e * 6 + k) * Q + qq];
+                                auto sys = [&](const int t, uint32_t *__restrict__ Sa, const uint32_t *__restrict__ So, uint32_t (&aU)[PU],
+                                               uint32_t (&aM)[PM]) {
+                                    const uint32_t s4[4] = {Sa[qq], Sa[Q + qq], Sa[2 * Q + qq], Sa[3 * Q + qq]};
+                                    uint32_t v[4][6];
+#pragma unroll
+                                    for (int e = 0; e < 4; ++e)
+#pragma unroll
+                                        for (int k = 0; k < 6; ++k) v[e][k] = So[ixT[(e * 6 + k) * Q + qq]];
+                                    const uint4 r4 = philox_rk((uint32_t)qq, time, wglob, ctr3(3, a, t), A.rk);
+                                    SlotK K;
+                                    {
+                                        const uint4 *k4 = reinterpret_cast<const uint4 *>(thr + t * 8);
+                                        const uint4 k0 = k4[0], k1 = k4[1], k2 = k4[2];
+                                        K.lo[0] = k0.x; K.lo[1] = k0.y; K.lo[2] = k0.z; K.lo[3] = k0.w;
+                                        K.lo[4] = k1.x; K.lo[5] = k1.y; K.lo[6] = k1.z; K.b3c = k1.w;
+                                        K.nc = k2.x; K.ec = k2.y;
+                                    }
+                                    const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
+                                    uint32_t wpl[4][3], outw[4], othw[4];
+#pragma unroll
+                                    for (int e = 0; e < 4; ++e) {
+                                        outw[e] = update_word_energy<BS>(s4[e], amask, xor3(s4[e], v[e][0], Jq[e][0]),
+                                                                         xor3(s4[e], v[e][1], Jq[e][1]), xor3(s4[e], v[e][2], Jq[e][2]),
+                                                                         xor3(s4[e], v[e][3], Jq[e][3]), xor3(s4[e], v[e][4], Jq[e][4]),
+                                                                         xor3(s4[e], v[e][5], Jq[e][5]), rr[e], K, A.one, A.mone, wpl[e]);
+                                        othw[e] = v[e][0];                     // the other colour's word at the same compact index
+                                    }
+                                    Sa[qq] = outw[0]; Sa[Q + qq] = outw[1]; Sa[2 * Q + qq] = outw[2]; Sa[3 * Q + qq] = outw[3];
+                                    energy_accumulate(wpl, outw, othw, aU, aM);
+                                };
+                                sys(tA, SaA, SoA, aU0, aM0);
+                                if (two) sys(tB, SaA + offB, SoA + offB, aU1, aM1);
+                            }
+                        }
+                        spw_finish<L>(A, S, accs, aU0, aM0, aU1, aM1, tA, tB, paired, last, lane_, w, a, exchange);
                     }
                 } else {
                     int bcur = -1;
@@ -857,7 +1000,7 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
         }
         // ---- exchange step (R12), all in shared memory
         const bool pt_due = PT && A.pt_every > 0 && ((uint64_t)A.sweep0 + (uint64_t)sw + 1) % (uint64_t)A.pt_every == 0;
-        if (pt_due && G_::PAIR && A.use_spw) {
+        if (pt_due && SPW) {
             exchange += 1;                                 // done by the warps of the colour-1 half sweep above
         } else if (pt_due) {
             const int lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
@@ -1015,40 +1158,35 @@ bool ladder_supported(const sg_ctx *c)
 template <int L>
 static cudaError_t launch_l(sg_ctx *c, const LadderArgs &A, int threads, size_t smem, cudaStream_t st, int grid)
 {
+    constexpr bool HAS_SPW = Geo<L>::PAIR || Geo<L>::PLANAR;
+    const void *f[6] = {(const void *)k_ladder_pmj<L, false, 0>, (const void *)k_ladder_pmj<L, false, 1>,
+                        (const void *)k_ladder_pmj<L, false, HAS_SPW ? 2 : 1>, (const void *)k_ladder_pmj<L, true, 0>,
+                        (const void *)k_ladder_pmj<L, true, 1>, (const void *)k_ladder_pmj<L, true, HAS_SPW ? 2 : 1>};
     if (attr_needed(c, ATTR_LADDER + L / 2 - 2)) {       // L = 4..16 -> ids 1..7
-        const void *f[4] = {(const void *)k_ladder_pmj<L, false, false>, (const void *)k_ladder_pmj<L, false, true>,
-                            (const void *)k_ladder_pmj<L, true, false>, (const void *)k_ladder_pmj<L, true, true>};
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < 6; ++i) {
             cudaError_t e = cudaFuncSetAttribute(f[i], cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
             if (e != cudaSuccess) return e;
         }
     }
-    const bool pt = A.pt_every > 0;
-    if (pt && A.split) {
+    const int ptm = A.pt_every > 0 ? (A.use_spw && HAS_SPW ? 2 : 1) : 0;
+    const void *kern = f[(A.d.bs_accept ? 3 : 0) + ptm];
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    if (ptm != 0 && A.split) {
         // split ladders with exchanges: the two CTAs of a ladder are a thread-block cluster (distributed shared memory)
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)grid);
-        cfg.blockDim = dim3((unsigned)threads);
-        cfg.dynamicSmemBytes = smem;
-        cfg.stream = st;
-        cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = 2;
         at[0].val.clusterDim.y = 1;
         at[0].val.clusterDim.z = 1;
         cfg.attrs = at;
         cfg.numAttrs = 1;
-        return A.d.bs_accept ? cudaLaunchKernelEx(&cfg, k_ladder_pmj<L, true, true>, A)
-                             : cudaLaunchKernelEx(&cfg, k_ladder_pmj<L, false, true>, A);
     }
-    if (A.d.bs_accept) {
-        if (pt) k_ladder_pmj<L, true, true><<<grid, threads, smem, st>>>(A);
-        else k_ladder_pmj<L, true, false><<<grid, threads, smem, st>>>(A);
-    } else {
-        if (pt) k_ladder_pmj<L, false, true><<<grid, threads, smem, st>>>(A);
-        else k_ladder_pmj<L, false, false><<<grid, threads, smem, st>>>(A);
-    }
-    return cudaGetLastError();
+    void *args[1] = {(void *)&A};
+    return cudaLaunchKernelExC(&cfg, kern, args);
 }
 
 // n_sweeps consecutive sweeps starting at global sweep index `sweep0`, with the exchanges that fall due fused in
@@ -1099,8 +1237,11 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchang
     if (A.split && ((d.N / 4 + maxt - 1) / maxt + 1) * threads < d.N / 4) return -1;   // (cross-pair swap: PER quads per thread)
     size_t smem = ladder_smem_bytes(d.L, d.NT, A.nt_res);
     const bool pair = (d.L / 2) % 4 != 0 && (d.L / 2) % 2 == 0;                 // Geo<L>::PAIR
-    const size_t spw_bytes = 16 + (size_t)Q * 72;                               // 9 offset pairs per quad
-    A.use_spw = pair && !A.split && smem + spw_bytes <= (size_t)227 * 1024 ? 1 : 0;
+    const bool planar = (d.L / 2) % 2 == 1;                                     // Geo<L>::PLANAR
+    // tables of the warp-per-pair exchange half sweep: 9 offset pairs per quad (pair layout), 24 positions + 24 coupling
+    // words per quad (planar layout)
+    const size_t spw_bytes = 16 + (size_t)Q * (pair ? 72 : 192);
+    A.use_spw = (pair || planar) && !A.split && smem + spw_bytes <= (size_t)227 * 1024 ? 1 : 0;
     A.use_tab = !A.use_spw && smem + ladder_tab_bytes(d.L) <= (size_t)227 * 1024 ? 1 : 0;
     if (A.use_spw) smem += spw_bytes;
     if (A.use_tab) smem += ladder_tab_bytes(d.L);
