@@ -12,6 +12,7 @@
 #include "sg_internal.h"
 
 #include <algorithm>
+#include <type_traits>
 
 namespace sg {
 
@@ -106,9 +107,9 @@ struct Geo {
     {
         return PAIR ? ((n >> 1) & 1) * (H / 2) + ((n >> 2) << 1) + (n & 1) : PLANAR ? (n & 3) * Q + (n >> 2) : n;
     }
-    // launch bounds: L=8 runs two 320-thread CTAs per SM (256 ladders of config 2 on 148 SMs)
-    static constexpr int MAXT = L == 8 ? 320 : VEC ? 512 : 384;
-    static constexpr int MINB = L == 8 ? 2 : 1;
+    // (L = 8 has its own kernel, sg_ladder8.cu; this one runs it when that kernel's ladder does not fit: one CTA per SM)
+    static constexpr int MAXT = VEC ? 512 : 384;
+    static constexpr int MINB = 1;
 };
 
 // Per-lane U (unsatisfied bonds) and M (sum of spins) of one system resident in shared memory, by ONE warp:
@@ -561,82 +562,131 @@ __global__ void __launch_bounds__(Geo<L>::MAXT, Geo<L>::MINB) k_ladder_pmj(const
     for (int sw = 0; sw < A.n_sweeps; ++sw) {
 #pragma unroll 1
         for (int colour = 0; colour < 2; ++colour) {
-            if (active) {
+            if constexpr (G_::VEC) {
+                // rows are whole quads: every neighbour of a quad is an aligned 128-bit access, except the one word beyond
+                // each end of the quad (side)
+                constexpr int QR = G_::QR, NBV = Q / 32;
+                constexpr int PU = NBV * 24 < 32 ? 5 : NBV * 24 < 64 ? 6 : NBV * 24 < 128 ? 7 : NBV * 24 < 256 ? 8 : 9;
+                constexpr int PM = NBV * 8 < 16 ? 4 : NBV * 8 < 32 ? 5 : NBV * 8 < 64 ? 6 : NBV * 8 < 128 ? 7 : 8;
+                static_assert(Q % 32 == 0 && NBV * 24 < 512 && NBV * 8 < 256, "plane counts");
                 const uint32_t time = 2u * (A.sweep0 + (uint32_t)sw) + (uint32_t)colour;
                 const uint32_t *Jown = Jsm + (colour * 3) * H;
                 const uint32_t *Joth = Jsm + ((1 - colour) * 3) * H;
-                if constexpr (G_::VEC) {
-                    constexpr int QR = G_::QR;
-                    const int r = q / QR, kq = q % QR;
+                int q_yp = 0, q_ym = 0, q_zp = 0, q_zm = 0, side[4] = {0, 0, 0, 0};
+                uint32_t JA[4], JB[4], Jyp[4], Jym[4], Jzp[4], Jzm[4];
+                // neighbour quads and the 24 coupling words of quad qx (shared by all systems handled with it)
+                auto setup = [&](const int qx) {
+                    const int r = qx / QR, kq = qx % QR;
                     const int y = r % L, z = r / L;
                     const int p = (colour + y + z) & 1;
-                    const int q_yp = (y + 1 == L) ? q - (L - 1) * QR : q + QR;
-                    const int q_ym = (y == 0) ? q + (L - 1) * QR : q - QR;
-                    const int q_zp = (z + 1 == L) ? q - (L - 1) * L * QR : q + L * QR;
-                    const int q_zm = (z == 0) ? q + (L - 1) * L * QR : q - L * QR;
-                    int side[4];
+                    q_yp = (y + 1 == L) ? qx - (L - 1) * QR : qx + QR;
+                    q_ym = (y == 0) ? qx + (L - 1) * QR : qx - QR;
+                    q_zp = (z + 1 == L) ? qx - (L - 1) * L * QR : qx + L * QR;
+                    q_zm = (z == 0) ? qx + (L - 1) * L * QR : qx - L * QR;
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
                         const int m = 4 * kq + e;
                         const int ms = p ? (m + 1 == Lh ? 0 : m + 1) : (m == 0 ? Lh - 1 : m - 1);
                         side[e] = r * Lh + ms;
                     }
-                    // couplings of this quad -> registers (shared by all systems of the group)
-                    uint32_t JA[4], JB[4], Jyp[4], Jym[4], Jzp[4], Jzm[4];
-                    {
-                        const uint4 jx = reinterpret_cast<const uint4 *>(Jown)[q];
-                        const uint4 jox = reinterpret_cast<const uint4 *>(Joth)[q];
-                        const uint4 jy = reinterpret_cast<const uint4 *>(Jown + H)[q];
-                        const uint4 joy = reinterpret_cast<const uint4 *>(Joth + H)[q_ym];
-                        const uint4 jz = reinterpret_cast<const uint4 *>(Jown + 2 * H)[q];
-                        const uint4 joz = reinterpret_cast<const uint4 *>(Joth + 2 * H)[q_zm];
-                        const uint32_t jxv[4] = {jx.x, jx.y, jx.z, jx.w}, joxv[4] = {jox.x, jox.y, jox.z, jox.w};
+                    const uint4 jx = reinterpret_cast<const uint4 *>(Jown)[qx];
+                    const uint4 jox = reinterpret_cast<const uint4 *>(Joth)[qx];
+                    const uint4 jy = reinterpret_cast<const uint4 *>(Jown + H)[qx];
+                    const uint4 joy = reinterpret_cast<const uint4 *>(Joth + H)[q_ym];
+                    const uint4 jz = reinterpret_cast<const uint4 *>(Jown + 2 * H)[qx];
+                    const uint4 joz = reinterpret_cast<const uint4 *>(Joth + 2 * H)[q_zm];
+                    const uint32_t jxv[4] = {jx.x, jx.y, jx.z, jx.w}, joxv[4] = {jox.x, jox.y, jox.z, jox.w};
 #pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            // bond to the neighbour at the same compact index / at the side index
-                            JA[e] = p ? joxv[e] : jxv[e];
-                            JB[e] = p ? jxv[e] : Joth[side[e]];
-                        }
-                        Jyp[0] = jy.x; Jyp[1] = jy.y; Jyp[2] = jy.z; Jyp[3] = jy.w;
-                        Jym[0] = joy.x; Jym[1] = joy.y; Jym[2] = joy.z; Jym[3] = joy.w;
-                        Jzp[0] = jz.x; Jzp[1] = jz.y; Jzp[2] = jz.z; Jzp[3] = jz.w;
-                        Jzm[0] = joz.x; Jzm[1] = joz.y; Jzm[2] = joz.z; Jzm[3] = joz.w;
+                    for (int e = 0; e < 4; ++e) {
+                        // bond to the neighbour at the same compact index / at the side index
+                        JA[e] = p ? joxv[e] : jxv[e];
+                        JB[e] = p ? jxv[e] : Joth[side[e]];
                     }
-#pragma unroll 1
-                    for (int tl = g; tl < ntl; tl += A.G) {
-                        const int t = tlo + tl;
-                        uint32_t *Sa = S + tl * N + colour * H;
-                        const uint32_t *So = S + tl * N + (1 - colour) * H;
-                        const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[q];
-                        const uint4 o0 = reinterpret_cast<const uint4 *>(So)[q];
-                        const uint4 oyp = reinterpret_cast<const uint4 *>(So)[q_yp];
-                        const uint4 oym = reinterpret_cast<const uint4 *>(So)[q_ym];
-                        const uint4 ozp = reinterpret_cast<const uint4 *>(So)[q_zp];
-                        const uint4 ozm = reinterpret_cast<const uint4 *>(So)[q_zm];
-                        const uint32_t os[4] = {So[side[0]], So[side[1]], So[side[2]], So[side[3]]};
-                        const uint4 r4 = philox_rk((uint32_t)q, time, wglob, ctr3(3, a, t), A.rk);
-                        SlotK K;
-                        {
-                            const uint4 *k4 = reinterpret_cast<const uint4 *>(thr + t * 8);
-                            const uint4 k0 = k4[0], k1 = k4[1], k2 = k4[2];
-                            K.lo[0] = k0.x; K.lo[1] = k0.y; K.lo[2] = k0.z; K.lo[3] = k0.w;
-                            K.lo[4] = k1.x; K.lo[5] = k1.y; K.lo[6] = k1.z; K.b3c = k1.w;
-                            K.nc = k2.x; K.ec = k2.y;
-                        }
-                        const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
-                        const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
-                        const uint32_t v0[4] = {o0.x, o0.y, o0.z, o0.w}, vyp[4] = {oyp.x, oyp.y, oyp.z, oyp.w};
-                        const uint32_t vym[4] = {oym.x, oym.y, oym.z, oym.w}, vzp[4] = {ozp.x, ozp.y, ozp.z, ozp.w};
-                        const uint32_t vzm[4] = {ozm.x, ozm.y, ozm.z, ozm.w};
-                        uint32_t out[4];
+                    Jyp[0] = jy.x; Jyp[1] = jy.y; Jyp[2] = jy.z; Jyp[3] = jy.w;
+                    Jym[0] = joy.x; Jym[1] = joy.y; Jym[2] = joy.z; Jym[3] = joy.w;
+                    Jzp[0] = jz.x; Jzp[1] = jz.y; Jzp[2] = jz.z; Jzp[3] = jz.w;
+                    Jzm[0] = joz.x; Jzm[1] = joz.y; Jzm[2] = joz.z; Jzm[3] = joz.w;
+                };
+                // quad qx of slot t (Sa / So = its own / the other colour block); en: with the energy bookkeeping
+                auto vitem = [&](const bool en, const int qx, const int t, uint32_t *__restrict__ Sa, const uint32_t *__restrict__ So,
+                                 uint32_t (&aU)[PU], uint32_t (&aM)[PM]) {
+                    const uint4 sv = reinterpret_cast<const uint4 *>(Sa)[qx];
+                    const uint4 o0 = reinterpret_cast<const uint4 *>(So)[qx];
+                    const uint4 oyp = reinterpret_cast<const uint4 *>(So)[q_yp];
+                    const uint4 oym = reinterpret_cast<const uint4 *>(So)[q_ym];
+                    const uint4 ozp = reinterpret_cast<const uint4 *>(So)[q_zp];
+                    const uint4 ozm = reinterpret_cast<const uint4 *>(So)[q_zm];
+                    const uint32_t os[4] = {So[side[0]], So[side[1]], So[side[2]], So[side[3]]};
+                    const uint4 r4 = philox_rk((uint32_t)qx, time, wglob, ctr3(3, a, t), A.rk);
+                    SlotK K;
+                    {
+                        const uint4 *k4 = reinterpret_cast<const uint4 *>(thr + t * 8);
+                        const uint4 k0 = k4[0], k1 = k4[1], k2 = k4[2];
+                        K.lo[0] = k0.x; K.lo[1] = k0.y; K.lo[2] = k0.z; K.lo[3] = k0.w;
+                        K.lo[4] = k1.x; K.lo[5] = k1.y; K.lo[6] = k1.z; K.b3c = k1.w;
+                        K.nc = k2.x; K.ec = k2.y;
+                    }
+                    const uint32_t s[4] = {sv.x, sv.y, sv.z, sv.w};
+                    const uint32_t rr[4] = {r4.x, r4.y, r4.z, r4.w};
+                    const uint32_t v0[4] = {o0.x, o0.y, o0.z, o0.w}, vyp[4] = {oyp.x, oyp.y, oyp.z, oyp.w};
+                    const uint32_t vym[4] = {oym.x, oym.y, oym.z, oym.w}, vzp[4] = {ozp.x, ozp.y, ozp.z, ozp.w};
+                    const uint32_t vzm[4] = {ozm.x, ozm.y, ozm.z, ozm.w};
+                    uint32_t out[4];
+                    if (en) {                                      // (a literal at both call sites)
+                        uint32_t wpl[4][3];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            out[e] = update_word_energy<BS>(s[e], amask, xor3(s[e], v0[e], JA[e]), xor3(s[e], os[e], JB[e]),
+                                                            xor3(s[e], vyp[e], Jyp[e]), xor3(s[e], vym[e], Jym[e]),
+                                                            xor3(s[e], vzp[e], Jzp[e]), xor3(s[e], vzm[e], Jzm[e]), rr[e], K, A.one,
+                                                            A.mone, wpl[e]);
+                        energy_accumulate(wpl, out, v0, aU, aM);
+                    } else {
 #pragma unroll
                         for (int e = 0; e < 4; ++e)
                             out[e] = flip_word_k<BS>(s[e], amask, xor3(s[e], v0[e], JA[e]), xor3(s[e], os[e], JB[e]),
-                                                 xor3(s[e], vyp[e], Jyp[e]), xor3(s[e], vym[e], Jym[e]),
-                                                 xor3(s[e], vzp[e], Jzp[e]), xor3(s[e], vzm[e], Jzm[e]), rr[e], K, A.one,
-                                                 A.mone);
-                        reinterpret_cast<uint4 *>(Sa)[q] = make_uint4(out[0], out[1], out[2], out[3]);
+                                                     xor3(s[e], vyp[e], Jyp[e]), xor3(s[e], vym[e], Jym[e]),
+                                                     xor3(s[e], vzp[e], Jzp[e]), xor3(s[e], vzm[e], Jzm[e]), rr[e], K, A.one,
+                                                     A.mone);
                     }
+                    reinterpret_cast<uint4 *>(Sa)[qx] = make_uint4(out[0], out[1], out[2], out[3]);
+                };
+                const bool spw_now = SPW && colour == 1 && A.pt_every > 0 &&
+                                     ((uint64_t)A.sweep0 + (uint64_t)sw + 1) % (uint64_t)A.pt_every == 0;
+                if (spw_now) {
+                    // ---- colour-1 half sweep + exchange, one WARP per pair of neighbouring slots (see the pair layout below)
+                    const int lane_ = tid & 31, warp_ = tid >> 5, NW = nthr >> 5;
+                    const int e1 = (int)(exchange & 1u);
+                    const int ntask = spw_ntask(e1, NT);
+                    const bool last = sw == A.n_sweeps - 1;
+                    for (int task = warp_; task < ntask; task += NW) {
+                        int tA, tB;
+                        bool paired;
+                        spw_task(task, e1, NT, tA, tB, paired);
+                        const bool two = tB != tA;
+                        const int offB = (tB - tA) * N;
+                        uint32_t *SaA = S + tA * N + H;
+                        const uint32_t *SoA = S + tA * N;
+                        uint32_t aU0[PU], aM0[PM], aU1[PU], aM1[PM];
+#pragma unroll
+                        for (int k = 0; k < PU; ++k) aU0[k] = aU1[k] = 0u;
+#pragma unroll
+                        for (int k = 0; k < PM; ++k) aM0[k] = aM1[k] = 0u;
+#pragma unroll 1
+                        for (int kb = 0; kb < NBV; ++kb) {
+                            const int qx = 32 * kb + lane_;
+                            setup(qx);
+                            vitem(true, qx, tA, SaA, SoA, aU0, aM0);
+                            if (two) vitem(true, qx, tB, SaA + offB, SoA + offB, aU1, aM1);
+                        }
+                        spw_finish<L>(A, S, accs, aU0, aM0, aU1, aM1, tA, tB, paired, last, lane_, w, a, exchange);
+                    }
+                } else if (active) {
+                    uint32_t dU[PU], dM[PM];                       // (unused by the instantiation without bookkeeping)
+                    setup(q);
+#pragma unroll 1
+                    for (int tl = g; tl < ntl; tl += A.G)
+                        vitem(false, q, tlo + tl, S + tl * N + colour * H, S + tl * N + (1 - colour) * H, dU, dM);
                 }
             }
             if constexpr (!G_::VEC) {
@@ -1158,7 +1208,7 @@ bool ladder_supported(const sg_ctx *c)
 template <int L>
 static cudaError_t launch_l(sg_ctx *c, const LadderArgs &A, int threads, size_t smem, cudaStream_t st, int grid)
 {
-    constexpr bool HAS_SPW = Geo<L>::PAIR || Geo<L>::PLANAR;
+    constexpr bool HAS_SPW = Geo<L>::PAIR || Geo<L>::PLANAR || L == 8;
     const void *f[6] = {(const void *)k_ladder_pmj<L, false, 0>, (const void *)k_ladder_pmj<L, false, 1>,
                         (const void *)k_ladder_pmj<L, false, HAS_SPW ? 2 : 1>, (const void *)k_ladder_pmj<L, true, 0>,
                         (const void *)k_ladder_pmj<L, true, 1>, (const void *)k_ladder_pmj<L, true, HAS_SPW ? 2 : 1>};
@@ -1220,7 +1270,7 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchang
     A.split = ladder_needs_split(d) ? 1 : 0;
     A.nt_res = A.split ? (d.NT + 1) / 2 : d.NT;
     // groups: as many as fit in <= 512 threads, at most the resident slots, preferring a divisor of their number
-    const int maxt = d.L == 8 ? 320 : ((d.L / 2) % 4 == 0 ? 512 : 384);
+    const int maxt = (d.L / 2) % 4 == 0 ? 512 : 384;
     int G = std::max(1, std::min(A.nt_res, maxt / Q));
     for (int gtry = G; gtry >= 1 && gtry * 2 > G; --gtry)
         if (A.nt_res % gtry == 0) { G = gtry; break; }
@@ -1242,8 +1292,9 @@ int launch_ladder_pmj(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchang
     // words per quad (planar layout)
     const size_t spw_bytes = 16 + (size_t)Q * (pair ? 72 : 192);
     A.use_spw = (pair || planar) && !A.split && smem + spw_bytes <= (size_t)227 * 1024 ? 1 : 0;
+    if (d.L == 8 && !A.split) A.use_spw = 1;                                    // rows of whole quads: no table needed
     A.use_tab = !A.use_spw && smem + ladder_tab_bytes(d.L) <= (size_t)227 * 1024 ? 1 : 0;
-    if (A.use_spw) smem += spw_bytes;
+    if (A.use_spw && (pair || planar)) smem += spw_bytes;
     if (A.use_tab) smem += ladder_tab_bytes(d.L);
     int grid = d.W * d.R;
     A.n_full = grid;

@@ -390,9 +390,12 @@ def test_fuzzed_shapes_run_vs_oracle(sg, O, case):
 
 @pytest.mark.parametrize("L,h,NT,R,pt_every,n_samples", [(12, 0.1, 1, 2, 1, 32), (12, -0.2, 2, 2, 1, 33), (12, 0.3, 3, 4, 1, 32),
                                                        (12, 0.1, 6, 2, 2, 64), (12, 0.0, 7, 4, 1, 32), (4, 0.3, 2, 2, 1, 40),
-                                                       (4, -0.3, 9, 4, 1, 32), (4, 0.2, 20, 2, 3, 65)])
+                                                       (4, -0.3, 9, 4, 1, 32), (4, 0.2, 20, 2, 3, 65),
+                                                       (6, 0.2, 9, 4, 1, 33), (6, 0.0, 2, 2, 1, 32), (10, 0.1, 7, 2, 2, 32), (10, -0.3, 12, 4, 1, 33),
+                                                       (8, 0.2, 30, 4, 1, 33), (8, -0.1, 33, 2, 2, 32)])
 def test_pair_layout_ladder_odd_and_tiny_ladders(sg, O, L, h, NT, R, pt_every, n_samples):
-    """k_ladder_pmj<4 | 12> (pair layout; exchange half sweep by one warp per pair of slots): ladders with one slot, an
+    """k_ladder_pmj<4 | 12> (pair layout), <6 | 10> (planar layout), <8> with more slots than the L = 8 kernel takes (whole-quad
+    rows) — exchange half sweep by one warp per pair of slots: ladders with one slot, an
     odd number of slots (a slot without a partner at both parities of the exchange), more pairs than warps, 2 and 4
     replicas, h = 0 (carry-chain compare) — spins, the kernel's own (U, M) after an exchange, accepted-swap counts and
     moments vs the oracle."""
