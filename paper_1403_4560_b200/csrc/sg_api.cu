@@ -22,7 +22,7 @@ constexpr int DEXP64_N = 5761, DEXP32_N = 1441;
 inline size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-    size_t spins, spins_alt, J, Jp, tps, J6, tab, exp64, exp32, tw, U, M, U_alt, M_alt, swap, pt_acc, hashes, acc, hist, rec, stage, total;
+    size_t spins, spins_alt, gbits, J, Jp, tps, J6, tab, exp64, exp32, tw, U, M, U_alt, M_alt, swap, pt_acc, hashes, acc, hist, rec, stage, total;
     int chunk_meas, chunk_stage, S_pad;
 };
 
@@ -84,6 +84,9 @@ Layout make_layout(int L, int n_samples, int R, int NT, int kind)
     lo.chunk_meas = (int)cm;
     lo.hist = take(hist_per * cm);
     lo.rec = take(rec_per * cm);
+    // Gaussian path: bit-packed copy of one measurement chunk (32 samples per word, the +-J layout), so that the
+    // bit-sliced measurement kernel serves both paths
+    lo.gbits = (kind == SG_GAUSS && L <= 16) ? take((cm / 32) * (size_t)R * NT * N * 4) : 0;
     const size_t stage_per = std::max((size_t)R * NT * N, 12 * N);
     size_t cs = std::max<size_t>(1, SCRATCH_CAP / stage_per);
     cs = std::min<size_t>(cs, (size_t)n_samples);
@@ -239,6 +242,12 @@ int do_measure(sg_ctx *c, double *out)
         const int ns = std::min(c->chunk_samples, d.n_samples - s0);
         if (measure_fused_supported(c)) {
             const int k = launch_measure_pmj(c, s0, ns, out != nullptr);
+            if (k < 0) return check_launch(c, "measure kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "measure kernel launch failed");
+            c->launches += k;
+        } else if (measure_fused_gauss_supported(c)) {
+            // Gaussian path: the chunk's spins as bits of 32-sample words, then the same bit-sliced measurement kernel
+            c->launches += launch_bits_gauss(c, s0, ns);
+            const int k = launch_measure_pmj(c, s0, ns, out != nullptr, c->gbits - (size_t)(s0 >> 5) * d.R * d.NT * d.N);
             if (k < 0) return check_launch(c, "measure kernel") ? SG_ECUDA : fail(c, SG_ECUDA, "measure kernel launch failed");
             c->launches += k;
         } else {
@@ -417,6 +426,7 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     c->ev_state = nullptr;
     c->ev_read[0] = c->ev_read[1] = nullptr;
     c->read_pending[0] = c->read_pending[1] = false;
+    c->gbits = (coupling_kind == SG_GAUSS && L <= 16) ? (uint32_t *)(b + lo.gbits) : nullptr;
     c->J = (uint32_t *)(b + lo.J);
     c->Jg = (float *)(b + lo.J);
     c->Jp = (coupling_kind == SG_PMJ && L == 32) ? (uint4 *)(b + lo.Jp) : nullptr;

@@ -272,6 +272,39 @@ k_hist_gauss(Dims d, const int8_t *__restrict__ spins, int s0, uint16_t *__restr
     }
 }
 
+// Byte spins of 32 consecutive samples -> one word per site (bit j = sample s0 + 32 wl + j, 1 <-> S = +1), the +-J layout
+// [wl][R][NT][2][H].  One warp per 128-byte segment of a system: for each of the 32 samples a coalesced 128-byte load
+// (lane l: bytes 4 l .. 4 l + 3), the four sign bits of the lane go to bit j of its four output words.  Samples beyond
+// n_samples read as S = -1 (their lanes are never accumulated).
+__global__ void __launch_bounds__(128)
+k_bits_gauss(Dims d, const int8_t *__restrict__ spins, int s0, int n_words, uint32_t *__restrict__ out)
+{
+    const int lane = threadIdx.x & 31;
+    const int n4 = d.N / 4;                                     // uint32 per system in the byte layout = uint4 per system out
+    const int segs = (n4 + 31) / 32;
+    const long long warp = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
+    if (warp >= (long long)n_words * d.R * d.NT * segs) return;
+    const int seg = (int)(warp % segs);
+    const long long sys = warp / segs;                          // (wl * R + a) * NT + t
+    const int at = (int)(sys % ((long long)d.R * d.NT));
+    const int wl = (int)(sys / ((long long)d.R * d.NT));
+    const int k = seg * 32 + lane;
+    if (k >= n4) return;
+    uint32_t w0 = 0, w1 = 0, w2 = 0, w3 = 0;
+#pragma unroll 4
+    for (int j = 0; j < 32; ++j) {
+        const int s = s0 + 32 * wl + j;
+        uint32_t v = 0xffffffffu;
+        if (s < d.n_samples) v = reinterpret_cast<const uint32_t *>(spins + ((size_t)s * d.R * d.NT + at) * d.N)[k];
+        const uint32_t up = ~v;                                 // sign bit of a byte clear <-> S = +1
+        w0 |= ((up >> 7) & 1u) << j;
+        w1 |= ((up >> 15) & 1u) << j;
+        w2 |= ((up >> 23) & 1u) << j;
+        w3 |= (up >> 31) << j;
+    }
+    reinterpret_cast<uint4 *>(out + (size_t)sys * d.N)[k] = make_uint4(w0, w1, w2, w3);
+}
+
 // -------------------------------------------------------------------- pack / unpack / getters
 __global__ void k_unpack_gauss(Dims d, const int8_t *__restrict__ spins, int s0, int ns, int8_t *__restrict__ out)
 {
@@ -355,6 +388,15 @@ int launch_hist_gauss(sg_ctx *c, int s0, int ns)
     const Dims &d = c->d;
     const size_t sh = (size_t)N_HIST * d.L * 32 * sizeof(uint16_t);
     k_hist_gauss<<<(unsigned)(ns * d.NT * d.P), 32, sh, c->stream>>>(d, c->spins8, s0, c->hist);
+    return 1;
+}
+
+int launch_bits_gauss(sg_ctx *c, int s0, int ns)
+{
+    const Dims &d = c->d;
+    const int n_words = (ns + 31) / 32;
+    const long long warps = (long long)n_words * d.R * d.NT * ((d.N / 4 + 31) / 32);
+    k_bits_gauss<<<(unsigned)((warps + 3) / 4), 128, 0, c->stream>>>(d, c->spins8, s0, n_words, c->gbits);
     return 1;
 }
 

@@ -87,6 +87,7 @@ struct sg_ctx {
     uint4 *Jp;                          // PMJ, L = 32: couplings repacked per warp step for k_res32_pmj (else NULL)
     int8_t *spins8;                     // GAUSS: [S][R][NT][2][H] colour-compacted bytes
     float *Jg;                          // GAUSS: [S][2][3][H]
+    uint32_t *gbits;                    // GAUSS, L <= 16: [chunk / 32][R][NT][2][H] bit-packed copy of a measurement chunk
     sg::SlotTab *tab;                   // [NT]
     double *exp64_tab;                  // [5761]
     float *exp32_tab;                   // [1441]
@@ -139,7 +140,10 @@ int launch_hist_pmj(sg_ctx *c, int s0, int ns);             // samples [s0, s0+n
 int launch_hist_gauss(sg_ctx *c, int s0, int ns);
 int launch_finalize(sg_ctx *c, int s0, int ns, bool want_rec);   // hist -> rec (optional), acc
 bool measure_fused_supported(const sg_ctx *c);             // bit-sliced one-launch measurement usable?
-int launch_measure_pmj(sg_ctx *c, int s0, int ns, bool want_rec);   // spins -> rec (optional), acc; -1 on error
+// spins -> rec (optional), acc; -1 on error.  spins: the packed state to read (nullptr = c->spins), indexed by GLOBAL word
+int launch_measure_pmj(sg_ctx *c, int s0, int ns, bool want_rec, const uint32_t *spins = nullptr);
+bool measure_fused_gauss_supported(const sg_ctx *c);       // Gaussian path: measurement through a bit-packed copy of the chunk?
+int launch_bits_gauss(sg_ctx *c, int s0, int ns);          // byte spins of samples [s0, s0 + ns) -> c->gbits (32 samples per word)
 int launch_unpack_pmj(sg_ctx *c, int s0, int ns);           // spins -> stage8 (canonical bytes)
 int launch_pack_pmj(sg_ctx *c, int s0, int ns);             // stage8 -> spins (lanes of [s0, s0+ns))
 int launch_unpack_gauss(sg_ctx *c, int s0, int ns);

@@ -470,7 +470,7 @@ static size_t measure_smem(int P)
 }
 
 template <int L>
-static int launch_measure_L(sg_ctx *c, int s0, int ns, bool want_rec)
+static int launch_measure_L(sg_ctx *c, int s0, int ns, bool want_rec, const uint32_t *spins)
 {
     const Dims &d = c->d;
     const size_t smem = measure_smem<L>(d.P);
@@ -479,7 +479,7 @@ static int launch_measure_L(sg_ctx *c, int s0, int ns, bool want_rec)
             return -1;
     }
     const int w0 = s0 >> 5, nw = (ns + 31) >> 5;
-    k_measure_pmj<L, false><<<(unsigned)(nw * d.NT), 256, smem, c->stream>>>(d, c->spins, c->twiddle, w0, s0,
+    k_measure_pmj<L, false><<<(unsigned)(nw * d.NT), 256, smem, c->stream>>>(d, spins ? spins : c->spins, c->twiddle, w0, s0,
                                                                              want_rec ? c->rec : nullptr, meas_out(c));
     return 1;
 }
@@ -524,16 +524,23 @@ bool measure_fused_supported(const sg_ctx *c)
     return c->path == SG_PATH_AUTO && is_packed(c) && (L == 4 || L == 6 || L == 8 || L == 10 || L == 12 || L == 16 || L == 32);
 }
 
+bool measure_fused_gauss_supported(const sg_ctx *c)
+{
+    const int L = c->d.L;
+    return c->path == SG_PATH_AUTO && c->kind == SG_GAUSS && c->gbits != nullptr &&
+           (L == 4 || L == 6 || L == 8 || L == 10 || L == 12 || L == 16);
+}
+
 // samples [s0, s0+ns), s0 a multiple of 32: records (optional) and accumulators in one launch
-int launch_measure_pmj(sg_ctx *c, int s0, int ns, bool want_rec)
+int launch_measure_pmj(sg_ctx *c, int s0, int ns, bool want_rec, const uint32_t *spins)
 {
     switch (c->d.L) {
-    case 4: return launch_measure_L<4>(c, s0, ns, want_rec);
-    case 6: return launch_measure_L<6>(c, s0, ns, want_rec);
-    case 8: return launch_measure_L<8>(c, s0, ns, want_rec);
-    case 10: return launch_measure_L<10>(c, s0, ns, want_rec);
-    case 12: return launch_measure_L<12>(c, s0, ns, want_rec);
-    case 16: return launch_measure_L<16>(c, s0, ns, want_rec);
+    case 4: return launch_measure_L<4>(c, s0, ns, want_rec, spins);
+    case 6: return launch_measure_L<6>(c, s0, ns, want_rec, spins);
+    case 8: return launch_measure_L<8>(c, s0, ns, want_rec, spins);
+    case 10: return launch_measure_L<10>(c, s0, ns, want_rec, spins);
+    case 12: return launch_measure_L<12>(c, s0, ns, want_rec, spins);
+    case 16: return launch_measure_L<16>(c, s0, ns, want_rec, spins);
     case 32: return launch_measure_32(c, s0, ns);
     default: return -1;
     }
