@@ -158,7 +158,8 @@ __device__ __forceinline__ void half_sweep_quad(uint32_t *__restrict__ Sa, const
 }
 
 // SPT = systems per thread (NT / G) when it is a compile-time constant (unrolled), 0 = run-time loop
-template <int SPT, bool BS>
+// PT = false: the instantiation for launches without exchanges (all exchange code compiled out)
+template <int SPT, bool BS, bool PT>
 __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ Ladder8Args A)
 {
     constexpr int N = 512, H = 256;
@@ -220,7 +221,7 @@ __global__ void __launch_bounds__(320, 2) k_ladder8_pmj(const __grid_constant__ 
 
     for (int sw = 0; sw < A.n_sweeps; ++sw) {
         const uint64_t sweep = A.sweep0 + (uint64_t)sw;
-        const bool pt_due = A.pt_every > 0 && ((sweep + 1) % (uint64_t)A.pt_every) == 0;
+        const bool pt_due = PT && A.pt_every > 0 && ((sweep + 1) % (uint64_t)A.pt_every) == 0;
 #pragma unroll 1
         for (int colour = 0; colour < 2; ++colour) {
             if (active) {
@@ -382,8 +383,10 @@ int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_swe
     if (attr_needed(c, ATTR_LADDER8)) {
         bool ok = true;
         auto set = [&](auto kern) { ok = ok && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024) == cudaSuccess; };
-        set(k_ladder8_pmj<0, false>); set(k_ladder8_pmj<1, false>); set(k_ladder8_pmj<2, false>); set(k_ladder8_pmj<4, false>);
-        set(k_ladder8_pmj<0, true>); set(k_ladder8_pmj<1, true>); set(k_ladder8_pmj<2, true>); set(k_ladder8_pmj<4, true>);
+        set(k_ladder8_pmj<0, false, false>); set(k_ladder8_pmj<1, false, false>); set(k_ladder8_pmj<2, false, false>); set(k_ladder8_pmj<4, false, false>);
+        set(k_ladder8_pmj<0, true, false>); set(k_ladder8_pmj<1, true, false>); set(k_ladder8_pmj<2, true, false>); set(k_ladder8_pmj<4, true, false>);
+        set(k_ladder8_pmj<0, false, true>); set(k_ladder8_pmj<1, false, true>); set(k_ladder8_pmj<2, false, true>); set(k_ladder8_pmj<4, false, true>);
+        set(k_ladder8_pmj<0, true, true>); set(k_ladder8_pmj<1, true, true>); set(k_ladder8_pmj<2, true, true>); set(k_ladder8_pmj<4, true, true>);
         if (!ok) return -1;
     }
     const Dims &d = c->d;
@@ -417,17 +420,18 @@ int launch_ladder8_pmj(sg_ctx *c, uint64_t sweep0, uint64_t exchange0, int n_swe
     const size_t smem = ladder8_smem(d.NT, pt_every > 0);
     const int spt = d.NT % G == 0 ? d.NT / G : 0;
     const int grid = d.W * d.R;
-    if (d.bs_accept) {
-        if (spt == 4) k_ladder8_pmj<4, true><<<grid, threads, smem, c->stream>>>(A);
-        else if (spt == 2) k_ladder8_pmj<2, true><<<grid, threads, smem, c->stream>>>(A);
-        else if (spt == 1) k_ladder8_pmj<1, true><<<grid, threads, smem, c->stream>>>(A);
-        else k_ladder8_pmj<0, true><<<grid, threads, smem, c->stream>>>(A);
-    } else {
-        if (spt == 4) k_ladder8_pmj<4, false><<<grid, threads, smem, c->stream>>>(A);
-        else if (spt == 2) k_ladder8_pmj<2, false><<<grid, threads, smem, c->stream>>>(A);
-        else if (spt == 1) k_ladder8_pmj<1, false><<<grid, threads, smem, c->stream>>>(A);
-        else k_ladder8_pmj<0, false><<<grid, threads, smem, c->stream>>>(A);
-    }
+    auto go = [&](auto kern) { kern<<<grid, threads, smem, c->stream>>>(A); };
+    const bool pt = pt_every > 0;
+#define SG_L8_PICK(SPTV)                                                                                        \
+    do {                                                                                                        \
+        if (d.bs_accept) { if (pt) go(k_ladder8_pmj<SPTV, true, true>); else go(k_ladder8_pmj<SPTV, true, false>); }   \
+        else { if (pt) go(k_ladder8_pmj<SPTV, false, true>); else go(k_ladder8_pmj<SPTV, false, false>); }            \
+    } while (0)
+    if (spt == 4) SG_L8_PICK(4);
+    else if (spt == 2) SG_L8_PICK(2);
+    else if (spt == 1) SG_L8_PICK(1);
+    else SG_L8_PICK(0);
+#undef SG_L8_PICK
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
