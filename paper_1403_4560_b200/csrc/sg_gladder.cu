@@ -221,9 +221,14 @@ __global__ void __launch_bounds__(512, 1) k_gladder(const __grid_constant__ GLad
                         }
                     long long ev = __double2ll_rz(__dadd_rn(__dadd_rn(ed[0], ed[1]), __dadd_rn(ed[2], ed[3])));
                     int mv = __dp4a((int)sv, 0x01010101, __dp4a((int)o0, 0x01010101, 0));
-                    for (int o = 16; o; o >>= 1) {
-                        ev += __shfl_xor_sync(0xffffffffu, ev, o);
-                        mv += __shfl_xor_sync(0xffffffffu, mv, o);
+                    // warp totals by integer reductions: |ev| < 2^41 (24 bonds of |J_fix| < 2^36), so ev + 2^41 splits into two
+                    // 21-bit chunks whose 32-lane sums fit in 32 bits
+                    {
+                        const unsigned long long evp = (unsigned long long)(ev + (1ll << 41));
+                        const unsigned c0 = __reduce_add_sync(0xffffffffu, (unsigned)(evp & 0x1fffffu));
+                        const unsigned c1 = __reduce_add_sync(0xffffffffu, (unsigned)(evp >> 21));
+                        ev = (long long)c0 + ((long long)c1 << 21) - (32ll << 41);
+                        mv = __reduce_add_sync(0xffffffffu, mv);
                     }
                     if (lane == 0) {
                         atomicAdd(reinterpret_cast<unsigned long long *>(&Efix[t]), (unsigned long long)ev);
