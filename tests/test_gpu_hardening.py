@@ -400,3 +400,33 @@ def test_full_sweep_count_protocol(sg, oracle_full_runs, name):
         + ((w.n_sweeps // w.pt_every) % 2) * (w.n_temps // 2) * w.n_samples * w.n_replicas
     assert np.all(acc <= prop)
     sim.close()
+
+
+@pytest.mark.parametrize("name,n,me", [("C3", 12, 1), ("C2", 24, 2)])
+def test_overlapped_measurements_at_full_pool_size(sg, name, n, me):
+    """Stress of the overlapped measurements (second state buffer, two library streams) at the full pool size, with a
+    measurement after every sweep / every second sweep so that every launch both writes a buffer a measurement still
+    reads from the previous round and is followed by one: moments, state hashes and the kernels' own energies must equal
+    those of the same schedule run serially (sg_run(.., 0) + sg_measure), three times in a row."""
+    w = W.BY_NAME[name]
+    temps = w.temps()
+    a = sg.Simulation(w.L, w.h, w.n_samples, w.n_replicas, temps, w.kind, w.seed)
+    b = sg.Simulation(w.L, w.h, w.n_samples, w.n_replicas, temps, w.kind, w.seed)
+    for k in range(n // me):
+        b.sg_run(me, 1, 0)
+        b.sg_measure(False)
+    mb, nb = b.sg_get_moments()
+    hb = b.sg_get_state_hash()
+    Ub, Mb = b.sg_get_energies_cached()
+    b.close()
+    for rep in range(3):
+        if rep:
+            a.sg_reset()
+        a.sg_run(n, 1, me)
+        ma, na = a.sg_get_moments()
+        assert na == nb == n // me
+        assert np.array_equal(ma, mb), "%s repeat %d: overlapped measurements differ from serial ones" % (name, rep)
+        assert np.array_equal(a.sg_get_state_hash(), hb)
+        Ua, Ma = a.sg_get_energies_cached()
+        assert np.array_equal(Ua, Ub) and np.array_equal(Ma, Mb)
+    a.close()
