@@ -179,12 +179,18 @@ __device__ __forceinline__ void bs_add(uint32_t (&acc)[NA], const uint32_t (&x)[
 // column i (bit j of the result = bit i of lane j's input).  All 32 lanes must participate.
 __device__ __forceinline__ uint32_t transpose32(uint32_t x, int lane)
 {
+    // stage j: exchange j x j bit blocks with lane ^ j.  A lane with bit j clear keeps its low blocks (mask m) and takes
+    // the partner's low blocks shifted up by j; a lane with bit j set keeps its high blocks (m << j) and takes the
+    // partner's high blocks shifted down by j.  Both shifts are ONE rotation (left by j, or by 32 - j) because the bits
+    // that wrap around land under the keep mask: per stage a shuffle, a funnel shift and a LOP3 select.
     uint32_t m = 0x0000FFFFu;
 #pragma unroll
     for (int j = 16; j >= 1; j >>= 1) {
         const uint32_t y = __shfl_xor_sync(0xffffffffu, x, j);
-        if (lane & j) x = (x & (m << j)) | ((y >> j) & m);
-        else          x = (x & m) | ((y & m) << j);
+        const bool up = (lane & j) != 0;
+        const uint32_t keep = up ? (m << j) : m;
+        const uint32_t rot = __funnelshift_l(y, y, up ? 32 - j : j);
+        x = lop3<0xCA>(keep, x, rot);               // keep ? x : rot
         m ^= (m << (j >> 1));      // 0000FFFF -> 00FF00FF -> 0F0F0F0F -> 33333333 -> 55555555
     }
     return x;
