@@ -1,5 +1,7 @@
 // sg_measure.cu — plane histograms -> overlaps q_ab(0), q_ab(K) (Eq. 2) -> records
 // and moment accumulators (R7-R9).  Shared by the packed and the byte path.
+#include <type_traits>
+
 #include "sg_device.cuh"
 #include "sg_internal.h"
 
@@ -262,59 +264,88 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
     for (int i = tid; i < P * C::PLW; i += nthr) PL[i] = 0u;
     __syncthreads();
 
-    // ---- phase 1: one thread per (pair, bin): bit-sliced count of its L^2 words
-    for (int item = tid; item < P * NB; item += nthr) {
-        const int pair = item / NB, bin = item - pair * NB;
-        const int hh = bin / L, b = bin - hh * L;
-        const BinGeom g = bin_geometry<L>(hh, b);
-        const uint32_t *Dp = Dsm + pair * N;
-        uint32_t ones = 0, twos = 0, fours = 0, hi[C::HI];
+    // ---- phase 1: one thread per (pair, bin): bit-sliced count of its L^2 words.  The items are ordered by the stride of the
+    // inner loop (L^2: histograms 0, 1, 3, 4; L: 2, 5, 6; 1: 7, 8), each class padded to whole warps, so that a warp runs ONE
+    // instantiation with that stride as a compile-time constant: the loads of the unrolled inner loop need no index arithmetic
+    {
+        constexpr int L2 = L * L;
+        const int n0 = P * 4 * L, n1 = P * 3 * L, n2 = P * 2 * L;          // items per class
+        const int p0 = (n0 + 31) & ~31, p1 = (n1 + 31) & ~31, p2 = (n2 + 31) & ~31;
+        auto count_bin = [&](auto sv_tag, const int pair, const int hh, const int b) {
+            constexpr int SV = decltype(sv_tag)::value;
+            const int bin = hh * L + b;
+            const BinGeom g = bin_geometry<L>(hh, b);
+            const uint32_t *Dp = Dsm + pair * N;
+            uint32_t ones = 0, twos = 0, fours = 0, hi[C::HI];
 #pragma unroll
-        for (int k = 0; k < C::HI; ++k) hi[k] = 0;
-        // The bins of one histogram (consecutive threads, b = 0 .. L-1) walk their L^2 sites in the same order, and except
-        // for the x histogram their addresses differ by multiples of L words: with the walk as written they would meet in
-        // the same shared-memory bank at every step.  Thread b therefore starts the loop whose stride is one word (the x
-        // direction) at offset b: the sites counted are the same, the banks of a step are all different.
-        const int skew_u = g.su == 1 ? b : 0, skew_v = g.sv == 1 ? b : 0;
+            for (int k = 0; k < C::HI; ++k) hi[k] = 0;
+            // The bins of one histogram (consecutive threads, b = 0 .. L-1) walk their L^2 sites in the same order, and except
+            // for the x histogram their addresses differ by multiples of L words: with the walk as written they would meet in
+            // the same shared-memory bank at every step.  Thread b therefore starts the loop whose stride is one word (the x
+            // direction) at offset b: the sites counted are the same, the banks of a step are all different.
+            const int skew_u = g.su == 1 ? b : 0, skew_v = SV == 1 ? b : 0;
 #pragma unroll 1
-        for (int uu = 0; uu < L; ++uu) {
-            int u = uu + skew_u;
-            if (u >= L) u -= L;
-            int dd = (g.ku * u + g.kb) % L;
-            if (dd < 0) dd += L;
-            const uint32_t *base = Dp + u * g.su + dd * g.sd;
+            for (int uu = 0; uu < L; ++uu) {
+                int u = uu + skew_u;
+                if (u >= L) u -= L;
+                int dd = (g.ku * u + g.kb) % L;
+                if (dd < 0) dd += L;
+                const uint32_t *base = Dp + u * g.su + dd * g.sd;
 #pragma unroll
-            for (int v0 = 0; v0 < L; v0 += 8) {
-                uint32_t x[8];
+                for (int v0 = 0; v0 < L; v0 += 8) {
+                    uint32_t x[8];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    int v = v0 + j + skew_v;
-                    if (v >= L) v -= L;
-                    x[j] = (v0 + j < L) ? base[v * g.sv] : 0u;
+                    for (int j = 0; j < 8; ++j) {
+                        int v = v0 + j + skew_v;
+                        if (v >= L) v -= L;
+                        x[j] = (v0 + j < L) ? base[v * SV] : 0u;
+                    }
+                    uint32_t tA, tB, fA, fB, e;
+                    csa(tA, ones, ones, x[0], x[1]);
+                    csa(tB, ones, ones, x[2], x[3]);
+                    csa(fA, twos, twos, tA, tB);
+                    csa(tA, ones, ones, x[4], x[5]);
+                    csa(tB, ones, ones, x[6], x[7]);
+                    csa(fB, twos, twos, tA, tB);
+                    csa(e, fours, fours, fA, fB);
+                    // ripple the weight-8 carry into the high planes
+#pragma unroll
+                    for (int k = 0; k < C::HI; ++k) {
+                        const uint32_t hk = hi[k];
+                        hi[k] = hk ^ e;
+                        e = hk & e;
+                    }
                 }
-                uint32_t tA, tB, fA, fB, e;
-                csa(tA, ones, ones, x[0], x[1]);
-                csa(tB, ones, ones, x[2], x[3]);
-                csa(fA, twos, twos, tA, tB);
-                csa(tA, ones, ones, x[4], x[5]);
-                csa(tB, ones, ones, x[6], x[7]);
-                csa(fB, twos, twos, tA, tB);
-                csa(e, fours, fours, fA, fB);
-                // ripple the weight-8 carry into the high planes
+            }
+            uint32_t *out = PL + pair * C::PLW + (bin / C::PER) * 32 + (bin % C::PER) * C::BPB;
+            out[0] = ones;
+            out[1] = twos;
+            out[2] = fours;
 #pragma unroll
-                for (int k = 0; k < C::HI; ++k) {
-                    const uint32_t hk = hi[k];
-                    hi[k] = hk ^ e;
-                    e = hk & e;
+            for (int k = 0; k < C::HI; ++k) out[3 + k] = hi[k];
+        };
+        for (int item = tid; item < p0 + p1 + p2; item += nthr) {         // (the class of an item is warp-uniform)
+            if (item < p0) {
+                if (item < n0) {
+                    constexpr int H4[4] = {0, 1, 3, 4};
+                    const int pair = item / (4 * L), rem = item - pair * 4 * L;
+                    count_bin(std::integral_constant<int, L2>{}, pair, H4[rem / L], rem % L);
+                }
+            } else if (item < p0 + p1) {
+                const int i1 = item - p0;
+                if (i1 < n1) {
+                    constexpr int H3[3] = {2, 5, 6};
+                    const int pair = i1 / (3 * L), rem = i1 - pair * 3 * L;
+                    count_bin(std::integral_constant<int, L>{}, pair, H3[rem / L], rem % L);
+                }
+            } else {
+                const int i2 = item - p0 - p1;
+                if (i2 < n2) {
+                    const int pair = i2 / (2 * L), rem = i2 - pair * 2 * L;
+                    count_bin(std::integral_constant<int, 1>{}, pair, 7 + rem / L, rem % L);
                 }
             }
         }
-        uint32_t *out = PL + pair * C::PLW + (bin / C::PER) * 32 + (bin % C::PER) * C::BPB;
-        out[0] = ones;
-        out[1] = twos;
-        out[2] = fours;
-#pragma unroll
-        for (int k = 0; k < C::HI; ++k) out[3 + k] = hi[k];
     }
     __syncthreads();
 
@@ -356,11 +387,12 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
                 if (mo.pq && w * 32 + l < d.n_samples)       // overlap histogram: N - tot sites agree
                     atomicAdd(&mo.pq[((size_t)(w * 32 + l) * d.NT + t) * mo.pq_bins + pq_bin(N - tot, N, mo.pq_bins)], 1u);
             }
+            // (fused multiply-adds: the records are compared to 1e-12, not bit for bit, and -fmad=false would split them)
             double re = 0.0, im = 0.0;
 #pragma unroll
             for (int m = 0; m < L; ++m) {
-                re += v[m] * cosv[m];
-                im += v[m] * sinv[m];
+                re = fma(v[m], cosv[m], re);
+                im = fma(v[m], sinv[m], im);
             }
             const int k1 = hh < 3 ? hh : hh + 3;
             r[(1 + 2 * k1) * 32] = re * invN;
@@ -369,8 +401,8 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
                 double re2 = 0.0, im2 = 0.0;
 #pragma unroll
                 for (int m = 0; m < L; ++m) {
-                    re2 += v[m] * cosv[(2 * m) % L];
-                    im2 += v[m] * sinv[(2 * m) % L];
+                    re2 = fma(v[m], cosv[(2 * m) % L], re2);
+                    im2 = fma(v[m], sinv[(2 * m) % L], im2);
                 }
                 r[(1 + 2 * (hh + 3)) * 32] = re2 * invN;
                 r[(2 + 2 * (hh + 3)) * 32] = im2 * invN;
@@ -447,16 +479,21 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
         }
     }
     __syncthreads();
-    for (int item = tid; item < 32 * SG_NMOM; item += nthr) {
-        const int l = item / SG_NMOM, j = item - l * SG_NMOM;
+    // one addition per address and launch: the reduction instruction gives the same result as load-add-store without
+    // waiting for the load.  A warp takes the samples l = warp, warp + nwarp, ...: 66 consecutive doubles per sample
+    // (coalesced), no division in the index
+    for (int l = warp; l < 32; l += nwarp) {
         const int s = w * 32 + l;
         if (s >= d.n_samples) continue;
-        const size_t o = ((size_t)s * d.NT + t) * SG_NMOM + j;
-        const double v = OUT[l * OUT_LD + j];
-        // one addition per address and launch: the reduction instruction gives the same result as load-add-store
-        // without waiting for the load
-        atomicAdd(&mo.acc[o], v);
-        if (mo.acc_win) atomicAdd(&mo.acc_win[o], v);
+        double *A = mo.acc + ((size_t)s * d.NT + t) * SG_NMOM;
+        double *B = mo.acc_win ? mo.acc_win + ((size_t)s * d.NT + t) * SG_NMOM : nullptr;
+        const double *src = OUT + l * OUT_LD;
+#pragma unroll
+        for (int j = lane; j < SG_NMOM; j += 32) {
+            const double v = src[j];
+            atomicAdd(&A[j], v);
+            if (B) atomicAdd(&B[j], v);
+        }
     }
 }
 
