@@ -197,7 +197,7 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
               double *__restrict__ rec, MeasOut mo)
 {
     using C = MeasureCfg<L>;
-    constexpr int N = C::N, NB = C::NB, Lh = L / 2, H = N / 2;
+    constexpr int N = C::N, Lh = L / 2, H = N / 2;
     extern __shared__ __align__(16) unsigned char sm_raw[];
     const int P = ONEPAIR ? 1 : d.P;                       // pairs handled by this CTA
     const int pair0 = ONEPAIR ? (int)(blockIdx.x % (unsigned)d.P) : 0;
@@ -245,20 +245,27 @@ k_measure_pmj(Dims d, const uint32_t *__restrict__ spins, const double *__restri
             }
         }
     } else
-    for (int k = tid; k < N; k += nthr) {                              // k = colour * H + n
-        const int c = k / H, n = k - c * H;
-        const int row = n / Lh, m = n - row * Lh;
-        const int z = row / L, y = row - z * L;
-        const int x = 2 * m + ((c + y + z) & 1);
-        const int site = x + L * (y + L * z);
-        uint32_t sr[4];
+    for (int k4 = tid; k4 < N / 4; k4 += nthr) {                       // four consecutive compact entries: one 128-bit load per replica
+        uint4 sr4[4];
 #pragma unroll
         for (int a = 0; a < 4; ++a)
-            sr[a] = a < d.R ? spins[(((size_t)w * d.R + a) * d.NT + t) * N + k] : 0u;
+            sr4[a] = a < d.R ? reinterpret_cast<const uint4 *>(spins + (((size_t)w * d.R + a) * d.NT + t) * N)[k4] : make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
-        for (int pair = 0; pair < 6; ++pair) {
-            constexpr int PA[6] = {0, 0, 0, 1, 1, 2}, PB[6] = {1, 2, 3, 2, 3, 3};
-            if (pair < P) Dsm[pair * N + site] = sr[PA[pair]] ^ sr[PB[pair]];
+        for (int e = 0; e < 4; ++e) {
+            const int k = 4 * k4 + e;                                      // k = colour * H + n
+            const int c = k / H, n = k - c * H;
+            const int row = n / Lh, m = n - row * Lh;
+            const int z = row / L, y = row - z * L;
+            const int x = 2 * m + ((c + y + z) & 1);
+            const int site = x + L * (y + L * z);
+            uint32_t sr[4];
+#pragma unroll
+            for (int a = 0; a < 4; ++a) sr[a] = e == 0 ? sr4[a].x : e == 1 ? sr4[a].y : e == 2 ? sr4[a].z : sr4[a].w;
+#pragma unroll
+            for (int pair = 0; pair < 6; ++pair) {
+                constexpr int PA[6] = {0, 0, 0, 1, 1, 2}, PB[6] = {1, 2, 3, 2, 3, 3};
+                if (pair < P) Dsm[pair * N + site] = sr[PA[pair]] ^ sr[PB[pair]];
+            }
         }
     }
     for (int i = tid; i < P * C::PLW; i += nthr) PL[i] = 0u;
