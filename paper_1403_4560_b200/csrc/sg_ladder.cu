@@ -1,12 +1,21 @@
-// sg_ladder.cu — the fast +-J path for lattices whose temperature ladder fits in shared memory.
+// sg_ladder.cu — the fast +-J path for lattices whose temperature ladder fits in shared memory (L = 4 .. 16).
 //
-// One CTA owns one (packed word w, replica a) ladder: its NT systems (NT * N words) and the word's
-// couplings (3 N words) stay in shared memory for `n_sweeps` consecutive checkerboard sweeps, so
-// global memory is touched once per launch.  A thread owns one quad q of 4 consecutive same-colour
-// sites (= one Philox call, R6) for the systems t = g, g+G, ... of its group; the 24 coupling words
-// of its quad live in registers across those systems.  Bit-sliced arithmetic as in sg_pmj.cu:
-// per word-site 6 XOR3 + 8 (count) + 8 (accept/flip) + 5 (Philox share) = 27 ALU-pipe lane-ops; the
-// seven "r < thr" masks and the Philox products are IMAD.WIDE on the FMA pipe.
+// One CTA owns one (packed word w, replica a) ladder: its NT systems (NT * N words) and the word's couplings (3 N words)
+// stay in shared memory for `n_sweeps` consecutive checkerboard sweeps and the exchanges between them, so global memory is
+// touched once per launch.  A ladder larger than one SM is split over a cluster of two CTAs (half of the slots each).
+// The unit of work is a quad: 4 consecutive same-colour sites = one Philox call (R6); its 24 coupling words live in
+// registers across the systems handled with it.  Three shared-memory layouts, by the row length L/2 in words:
+//   * whole quads per row (L = 8, 16): canonical order; thread = (quad, group of slots); 128-bit neighbour accesses;
+//   * even, not whole quads (L = 4, 12): "pair" layout [low 64-bit pairs][high pairs]; items (block of 32 quads, slot)
+//     dealt out evenly over 12 warps; 64-bit neighbour accesses without bank conflicts;
+//   * odd (L = 6, 10): "planar" layout, word e of every quad in array e; same items; 32-bit unit-stride accesses.
+// Three instantiations per (L, compare variant), template parameter PTM: 0 = plain sweeps (no exchange code; the last,
+// half-empty wave of ladders goes to two CTAs each), 1 = exchanges by a one-warp-per-slot recount (+ the cross pair of a
+// split ladder through distributed shared memory), 2 = exchanges by the warp-per-pair colour-1 half sweep (energy counts in
+// registers, decision and swap by the same warp).
+// Bit-sliced arithmetic as in sg_pmj.cu: per word-site 6 XOR3 + 8 (count) + 4 (compare / flip) + 3 carries + 5 (Philox
+// share) = 26 ALU-pipe lane-ops with the binary-search compare; the Philox products and the threshold selection are IMADs on
+// the FMA pipe.
 #include "sg_accept.cuh"
 #include "sg_device.cuh"
 #include "sg_internal.h"
