@@ -533,10 +533,9 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
             cudaDeviceGetStreamPriorityRange(&lo_pri, &hi_pri);
             if ((rc = check_cuda(c, cudaStreamCreateWithPriority(&c->stream_hi, cudaStreamNonBlocking, hi_pri), "stream_hi"))) return rc;
             if ((rc = check_cuda(c, cudaStreamCreateWithPriority(&c->stream2, cudaStreamNonBlocking, lo_pri), "stream2"))) return rc;
-            cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming);
-            cudaEventCreateWithFlags(&c->ev_state, cudaEventDisableTiming);
-            cudaEventCreateWithFlags(&c->ev_read[0], cudaEventDisableTiming);
-            cudaEventCreateWithFlags(&c->ev_read[1], cudaEventDisableTiming);
+            cudaEvent_t *evs[4] = {&c->ev_join, &c->ev_state, &c->ev_read[0], &c->ev_read[1]};
+            for (cudaEvent_t *e : evs)
+                if ((rc = check_cuda(c, cudaEventCreateWithFlags(e, cudaEventDisableTiming), "event"))) return rc;
         }
         auto buf_id = [&](const uint32_t *p) { return p == std::min(c->spins, c->spins_alt) ? 0 : 1; };
         // An overlapped measurement is SUBMITTED after the next ladder launch, so that the ladder CTAs are placed first
