@@ -163,6 +163,27 @@ int sg_set_kernel_path(sg_ctx *ctx, int path);
  * SG_GAUSS.  Synchronous. */
 int sg_get_state_hash(sg_ctx *ctx, uint64_t *out);
 
+/* sg_get_state_hash for callers that cannot allocate device memory.  Same hashes, same layout of `out` (HOST ptr), same
+ * synchronous behaviour, but the per-system hashes are staged in one fixed 512 KiB array that is part of the library image
+ * (a file-scope __device__ array in csrc/sg_noalloc.cu) instead of a buffer that grows with the pool.  The call and
+ * everything under it make no cudaMalloc / cudaFree / cudaMallocAsync call and create no stream or event, so it is safe
+ * where those are off limits: inside a host program that has given all device memory to its own pool allocator (a raw
+ * cudaMalloc would fail or eat into that pool), in a hook that fires inside a running simulation loop (cudaMalloc and
+ * cudaFree stall every stream of the device), or for a caller that was handed a context built on somebody else's
+ * workspace and has no allocator at all.  (Create such a context with a caller-owned `workspace`; sg_create with
+ * workspace = NULL does allocate.)
+ *   limit     n_words * n_replicas * n_temps <= SG_NOALLOC_MAX_SYSTEMS (n_words as for sg_get_state_hash); beyond it
+ *             SG_EINVAL, nothing is launched, `out` is untouched and sg_last_error names the limit
+ *   cost      the array takes 512 KiB on every GPU that loads this library, until the process exits
+ *   first use the first call on each device looks the array's device address up (cudaGetSymbolAddress; this also makes
+ *             the runtime load the library's device code there).  Make that first call with the context's device current,
+ *             like every other call, and before starting any stream capture; later calls only launch, copy and wait
+ *   sharing   all calls on one GPU use the same array and it keeps the previous call's contents.  Nothing needs
+ *             clearing (a call reads back only the entries it has just written), but two calls whose GPU work may
+ *             overlap, e.g. two contexts driven from two host threads, race on it: serialise them. */
+#define SG_NOALLOC_MAX_SYSTEMS 65536
+int sg_get_state_hash_noalloc(sg_ctx *ctx, uint64_t *out);
+
 /* The energies the sweep / exchange kernels computed for themselves (what the swap decisions of R12
  * actually used), permuted like the configurations by the exchanges since: same layout as
  * sg_get_energies, which always recounts with a separate kernel.  SG_ESTATE if the kernels' own

@@ -776,6 +776,25 @@ int sg_get_state_hash(sg_ctx *c, uint64_t *out)
     return check_cuda(c, cudaStreamSynchronize(c->stream), "sync hashes");
 }
 
+// sg_get_state_hash without any allocation: per-system hashes staged in the static device array of sg_noalloc.cu.
+// flush_pending only launches kernels into the caller's workspace, so the whole call stays allocation-free.
+int sg_get_state_hash_noalloc(sg_ctx *c, uint64_t *out)
+{
+    if (!c || !out) return SG_EINVAL;
+    const long long n_sys = (long long)c->d.W * c->d.R * c->d.NT;
+    if (n_sys > (long long)SG_NOALLOC_MAX_SYSTEMS)
+        return fail(c, SG_EINVAL, "sg_get_state_hash_noalloc: " + std::to_string(n_sys) + " systems exceed the static scratch of " +
+                                      std::to_string((long long)SG_NOALLOC_MAX_SYSTEMS) + " (SG_NOALLOC_MAX_SYSTEMS); use sg_get_state_hash");
+    int rc;
+    if ((rc = flush_pending(c))) return rc;
+    bool too_large = false;
+    int launches = 0;
+    const cudaError_t e = hash_noalloc(c, out, &too_large, &launches);
+    c->launches += (uint64_t)launches;
+    if (too_large) return fail(c, SG_EINVAL, "sg_get_state_hash_noalloc: pool exceeds SG_NOALLOC_MAX_SYSTEMS");
+    return check_cuda(c, e, "sg_get_state_hash_noalloc");
+}
+
 int sg_get_pt_stats(sg_ctx *c, uint64_t *proposed, uint64_t *accepted)
 {
     if (!c) return SG_EINVAL;

@@ -158,6 +158,8 @@ int launch_tp_to_std(sg_ctx *c);                           // tps -> spins
 int launch_tp_run(sg_ctx *c, uint64_t sweep0, int n_sweeps, uint64_t exchange0, int pt_every);   // 1 launch (-1 on error)
 inline bool is_packed(const sg_ctx *c) { return c->kind != SG_GAUSS; }   // sample-packed +-J state in c->spins
 int launch_hash(sg_ctx *c, uint64_t *dev_out);             // one 64-bit hash per system -> dev_out
+// sg_noalloc.cu: hashes of the current state -> out_host through the library's static scratch array (no allocation)
+cudaError_t hash_noalloc(sg_ctx *c, uint64_t *out_host, bool *too_large, int *launches);
 sg::MeasOut meas_out(const sg_ctx *c);                     // where the measurement kernels add (window from the sweep counter)
 
 // kernel families for sg_ctx::attr_done

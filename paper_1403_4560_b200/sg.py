@@ -13,6 +13,7 @@ PMJ, GAUSS, PMJ_TPACK = 0, 1, 2
 NK, REC, NMOM = 12, 25, 66
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ESTATE = 0, -1, -2, -3, -4, -5
 PATH_AUTO, PATH_GENERIC = 0, 1
+NOALLOC_MAX_SYSTEMS = 65536
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "csrc", "libsg_b200.so")
@@ -44,6 +45,7 @@ EXPORTS = {
     "sg_last_error": (C.c_char_p, [C.c_void_p]),
     "sg_set_kernel_path": (C.c_int, [C.c_void_p, C.c_int]),
     "sg_get_state_hash": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "sg_get_state_hash_noalloc": (C.c_int, [C.c_void_p, C.c_void_p]),
     "sg_get_energies_cached": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "sg_get_pt_stats": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "sg_enable_pq": (C.c_int, [C.c_void_p, C.c_int]),
@@ -199,6 +201,14 @@ class Simulation:
         nw = (self.n_samples + 31) // 32 if self.kind != GAUSS else self.n_samples
         out = np.empty((nw, self.R, self.NT), dtype=np.uint64)
         self._check(_lib.sg_get_state_hash(self._h, _p(out)))
+        return out
+
+    def sg_get_state_hash_noalloc(self):
+        """sg_get_state_hash for callers that must not allocate device memory (include/sg.h): same values, staged in the
+        library's fixed 512 KiB device array; raises SgError(EINVAL) beyond NOALLOC_MAX_SYSTEMS systems."""
+        nw = (self.n_samples + 31) // 32 if self.kind != GAUSS else self.n_samples
+        out = np.empty((nw, self.R, self.NT), dtype=np.uint64)
+        self._check(_lib.sg_get_state_hash_noalloc(self._h, _p(out)))
         return out
 
     def sg_get_pt_stats(self):
