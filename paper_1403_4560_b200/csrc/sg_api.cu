@@ -226,9 +226,10 @@ int do_exchange(sg_ctx *c)
     if (!c->um_fresh) c->launches += is_packed(c) ? launch_energy_pmj(c) : launch_energy_gauss(c);
     c->um_fresh = true;
     c->launches += is_packed(c) ? launch_pt_pmj(c, c->exchanges) : launch_pt_gauss(c, c->exchanges);
+    if ((rc = check_launch(c, "pt kernels"))) return rc;    // the exchange counter only moves once both kernels are enqueued
     if (c->kind == SG_PMJ_TPACK) c->tp_state = 2;           // the swap ran on the sample-packed copy
     c->exchanges += 1;
-    return check_launch(c, "pt kernels");
+    return SG_OK;
 }
 
 int do_measure(sg_ctx *c, double *out)

@@ -194,13 +194,13 @@ k_pt_decide_gauss(Dims d, const int64_t *__restrict__ U, const int32_t *__restri
     if (accept) atomicAdd(&pt_acc[t], 1ULL);
 }
 
-// One CTA per (pair, replica, sample): leaves at once if the pair does not swap; otherwise trades the two
-// configurations and their E_fix, M.
+// One CTA per (sample, replica, pair): leaves at once if the pair does not swap; otherwise trades the two
+// configurations and their E_fix, M.  The sample index is gridDim.x (limit 2^31 - 1; y and z stop at 65535).
 __global__ void __launch_bounds__(256)
 k_pt_swap_gauss(Dims d, int8_t *__restrict__ spins, const uint32_t *__restrict__ swapmask,
                 uint32_t exchange, int npairs, int64_t *__restrict__ U, int32_t *__restrict__ M)
 {
-    const int pair = blockIdx.x, a = blockIdx.y, s = blockIdx.z;
+    const int s = blockIdx.x, a = blockIdx.y, pair = blockIdx.z;
     if (!swapmask[((size_t)s * d.R + a) * (d.NT / 2) + pair]) return;
     const int t = (int)(exchange & 1u) + 2 * pair;
     const size_t sys = ((size_t)s * d.R + a) * d.NT + t;
@@ -378,7 +378,7 @@ int launch_pt_gauss(sg_ctx *c, uint64_t exchange)
     if (npairs <= 0) return 0;
     k_pt_decide_gauss<<<blocks_for((long long)d.n_samples * d.R * npairs, 128), 128, 0, c->stream>>>(
         d, c->U, c->M, c->tab, c->exp64_tab, c->h, (uint32_t)exchange, npairs, c->swapmask, c->pt_acc);
-    k_pt_swap_gauss<<<dim3(npairs, d.R, d.n_samples), 256, 0, c->stream>>>(d, c->spins8, c->swapmask, (uint32_t)exchange,
+    k_pt_swap_gauss<<<dim3(d.n_samples, d.R, npairs), 256, 0, c->stream>>>(d, c->spins8, c->swapmask, (uint32_t)exchange,
                                                                            npairs, c->U, c->M);
     return 2;
 }

@@ -264,13 +264,13 @@ k_pt_decide_pmj(Dims d, const int64_t *__restrict__ U, const int32_t *__restrict
     }
 }
 
-// One CTA per (pair, replica, word): reads the pair's mask once and leaves if no lane swaps (the common
+// One CTA per (word, replica, pair) - the word index is gridDim.x (limit 2^31 - 1; y and z stop at 65535): reads the pair's mask once and leaves if no lane swaps (the common
 // case on a wide ladder); otherwise trades the selected lanes of the two configurations and of their U, M.
 __global__ void __launch_bounds__(256)
 k_pt_swap_pmj(Dims d, uint32_t *__restrict__ spins, const uint32_t *__restrict__ swapmask,
               uint32_t exchange, int npairs, int64_t *__restrict__ U, int32_t *__restrict__ M)
 {
-    const int pair = blockIdx.x, a = blockIdx.y, w = blockIdx.z;
+    const int w = blockIdx.x, a = blockIdx.y, pair = blockIdx.z;
     const uint32_t mask = swapmask[(size_t)(w * d.R + a) * (d.NT / 2) + pair];
     if (mask == 0) return;
     const int t = (int)(exchange & 1u) + 2 * pair;
@@ -466,7 +466,7 @@ int launch_pt_pmj(sg_ctx *c, uint64_t exchange)
     if (npairs <= 0) return 0;
     k_pt_decide_pmj<<<blocks_for((long long)d.W * d.R * npairs, 4), 128, 0, c->stream>>>(
         d, c->U, c->M, c->tab, c->exp64_tab, c->h, (uint32_t)exchange, npairs, c->swapmask, c->pt_acc);
-    k_pt_swap_pmj<<<dim3(npairs, d.R, d.W), 256, 0, c->stream>>>(d, c->spins, c->swapmask, (uint32_t)exchange, npairs,
+    k_pt_swap_pmj<<<dim3(d.W, d.R, npairs), 256, 0, c->stream>>>(d, c->spins, c->swapmask, (uint32_t)exchange, npairs,
                                                                  c->U, c->M);
     return 2;
 }

@@ -430,3 +430,26 @@ def test_overlapped_measurements_at_full_pool_size(sg, name, n, me):
         Ua, Ma = a.sg_get_energies_cached()
         assert np.array_equal(Ua, Ub) and np.array_equal(Ma, Mb)
     a.close()
+
+
+def test_exchange_with_more_than_65535_gaussian_samples(sg, O):
+    """the stand-alone swap kernels index the sample / word by gridDim.x (limit 2^31 - 1), not by
+    gridDim.z (65535), so a Gaussian pool of more than 65535 samples on the generic exchange path (L = 4 has no ladder
+    kernel) runs; first, middle and last sample against the oracle, counters consistent with the state."""
+    L, h, R, NT, seed, ns = 4, 0.2, 2, 3, 21, 65600
+    temps = W.ladder(0.7, 1.1, NT)
+    sim = sg.Simulation(L, h, ns, R, temps, sg.GAUSS, seed)
+    try:
+        for _ in range(4):
+            sim.sg_sweep(1)
+            sim.sg_pt_exchange()
+        assert sim.sg_get_counters() == (4, 4)
+        U, M = sim.sg_get_energies()
+        prop, acc = sim.sg_get_pt_stats()
+        assert prop[0] == 2 * ns * R and prop[1] == 2 * ns * R and 0 < acc[0] <= prop[0]
+        for s in (0, 40000, 65535, 65536, ns - 1):
+            want = oracle_job(O, L, h, R, temps, O.GAUSS, seed, s, [(4, 1, 0)])
+            assert np.array_equal(sim.sg_get_spins(s, 1)[0], want["spins"]), s
+            assert np.array_equal(U[s], want["U"]) and np.array_equal(M[s], want["M"]), s
+    finally:
+        sim.close()
