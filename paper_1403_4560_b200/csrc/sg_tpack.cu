@@ -388,7 +388,10 @@ cudaError_t launch_tp(sg_ctx *c, const TpArgs &A, size_t smem, int grid)
         e = cudaFuncSetAttribute(k_tp_run<L, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
     }
-    if (grid >= 148 * 6) k_tp_run<L, 32><<<grid, TP_THREADS, smem, c->stream>>>(A);      // enough lattices to fill every SM
+    int dev = 0, n_sm = 0;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm <= 0) n_sm = 148;
+    if (grid >= n_sm * 6) k_tp_run<L, 32><<<grid, TP_THREADS, smem, c->stream>>>(A);     // enough lattices to fill every SM
     else k_tp_run<L, 8><<<grid, TP_THREADS, smem, c->stream>>>(A);
     return cudaGetLastError();
 }

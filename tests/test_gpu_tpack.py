@@ -124,3 +124,49 @@ def test_tpack_unsupported_shapes(sg):
         sim.sg_set_first_sample(5)          # must be a multiple of 32: the sweep draws are keyed by the packed word
     sim.sg_set_first_sample(64)
     sim.close()
+
+
+BIG = [
+    # name, L, h, n_samples, R, NT, (T_lo, T_hi): n_samples * R >= 6 lattices per SM (888 on a B200) selects k_tp_run<L, 32>
+    ("L4-1024-lattices", 4, 0.3, 512, 2, 8, (0.5, 2.0)),
+    ("L6-960-lattices-40-slots", 6, 0.1, 480, 2, 40, (0.7, 2.5)),
+]
+
+
+@pytest.mark.parametrize("case", BIG, ids=[c[0] for c in BIG])
+def test_tpack_many_lattices_kernel(sg, O, case):
+    """with at least 6 lattices per SM the launch takes the instantiation that keeps 32 slots per work
+    item (k_tp_run<L, 32>); the cases above never reach it.  Whole pool against the sample-packed SG_PMJ path, three
+    samples (first word, a middle lane, last) against the oracle."""
+    import torch
+    _, L, h, ns, R, NT, (Tlo, Thi) = case
+    assert ns * R >= 6 * torch.cuda.get_device_properties(0).multi_processor_count
+    temps = W.ladder(Tlo, Thi, NT)
+    tp = sg.Simulation(L, h, ns, R, temps, sg.PMJ_TPACK, 77)
+    std = sg.Simulation(L, h, ns, R, temps, sg.PMJ, 77)
+    try:
+        for sim in (tp, std):
+            sim.sg_run(6, 1, 0)
+            sim.sg_run(6, 2, 3)
+        assert np.array_equal(tp.sg_get_spins(), std.sg_get_spins())
+        assert np.array_equal(tp.sg_get_state_hash(), std.sg_get_state_hash())
+        pt_tp, pt_std = tp.sg_get_pt_stats(), std.sg_get_pt_stats()
+        assert np.array_equal(pt_tp[0], pt_std[0]) and np.array_equal(pt_tp[1], pt_std[1]) and pt_tp[1].sum() > 0
+        Uc, Mc = tp.sg_get_energies_cached()
+        U, M = std.sg_get_energies()
+        assert np.array_equal(Uc, U) and np.array_equal(Mc, M)
+        mom, n = tp.sg_get_moments()
+        mom2, nn = std.sg_get_moments()
+        assert n == nn == 2 and close(mom, mom2)
+        for s in (0, ns // 2 + 13, ns - 1):
+            o = O.Oracle(L, h, R, temps, seed=77, sample=s)
+            o.run(6, 1, 0)
+            o.run(6, 2, 3)
+            assert np.array_equal(tp.sg_get_spins(s, 1)[0], o.spins()), "sample %d" % s
+            Uo, Mo = o.energies()
+            assert np.array_equal(Uc[s], Uo) and np.array_equal(Mc[s], Mo)
+            want, no = o.moments()
+            assert no == n and close(mom[s], want)
+            o.close()
+    finally:
+        tp.close(); std.close()
