@@ -217,6 +217,11 @@ int sg_enable_log_binning(sg_ctx *ctx, int n_windows);
  * (may be NULL).  SG_ESTATE if not enabled, SG_EINVAL if k is out of range.  Synchronous. */
 int sg_get_window_moments(sg_ctx *ctx, int k, double *out, int64_t *n_meas);
 
+/* Fault injection for tests of the error paths: the `countdown`-th resident-ladder launch that sg_run would enqueue from
+ * now on (L <= 16 paths) is not enqueued and sg_run returns SG_ECUDA instead; countdown = 0 disarms.  Everything enqueued
+ * before it is complete and counted: the context stays usable and a further sg_run continues the same trajectory. */
+int sg_debug_fail_launch(sg_ctx *ctx, int countdown);
+
 /* Description of the last error of this context (or of the last failed sg_create if ctx is NULL).
  * The string is owned by the library and valid until the next call on the same context. */
 const char *sg_last_error(sg_ctx *ctx);

@@ -396,6 +396,7 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     c->um_fresh = false;
     c->pending_exchange = false;
     c->attr_done = 0;
+    c->fail_countdown = 0;
     Dims &d = c->d;
     d.L = L; d.Lh = L / 2; d.N = L * L * L; d.H = d.N / 2;
     d.R = n_replicas; d.NT = n_temps; d.P = n_replicas * (n_replicas - 1) / 2;
@@ -530,13 +531,28 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
         if (overlap && !c->stream2) {
             // the ladder launches of an overlapped run go to a HIGH-priority stream of the library, the measurements to a
             // low-priority one: the block scheduler then places a measurement CTA only where no ladder CTA fits
+            // All six objects are created into locals and handed to the context together: a failure half way leaves the
+            // context as it was (nothing leaks, the next call tries again) instead of a stream without its events.
             int lo_pri = 0, hi_pri = 0;
             cudaDeviceGetStreamPriorityRange(&lo_pri, &hi_pri);
-            if ((rc = check_cuda(c, cudaStreamCreateWithPriority(&c->stream_hi, cudaStreamNonBlocking, hi_pri), "stream_hi"))) return rc;
-            if ((rc = check_cuda(c, cudaStreamCreateWithPriority(&c->stream2, cudaStreamNonBlocking, lo_pri), "stream2"))) return rc;
-            cudaEvent_t *evs[4] = {&c->ev_join, &c->ev_state, &c->ev_read[0], &c->ev_read[1]};
-            for (cudaEvent_t *e : evs)
-                if ((rc = check_cuda(c, cudaEventCreateWithFlags(e, cudaEventDisableTiming), "event"))) return rc;
+            cudaStream_t s_hi = nullptr, s_lo = nullptr;
+            cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+            cudaError_t e = cudaStreamCreateWithPriority(&s_hi, cudaStreamNonBlocking, hi_pri);
+            if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&s_lo, cudaStreamNonBlocking, lo_pri);
+            for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming);
+            if (e != cudaSuccess) {
+                for (cudaEvent_t x : ev)
+                    if (x) cudaEventDestroy(x);
+                if (s_lo) cudaStreamDestroy(s_lo);
+                if (s_hi) cudaStreamDestroy(s_hi);
+                return check_cuda(c, e, "sg_run: streams / events of the overlapped measurements");
+            }
+            c->stream_hi = s_hi;
+            c->stream2 = s_lo;
+            c->ev_join = ev[0];
+            c->ev_state = ev[1];
+            c->ev_read[0] = ev[2];
+            c->ev_read[1] = ev[3];
         }
         auto buf_id = [&](const uint32_t *p) { return p == std::min(c->spins, c->spins_alt) ? 0 : 1; };
         // An overlapped measurement is SUBMITTED after the next ladder launch, so that the ladder CTAs are placed first
@@ -581,6 +597,8 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
                 if ((rc = check_cuda(c, cudaStreamWaitEvent(c->stream, c->ev_read[buf_id(out)], 0), "wait measurement"))) return rc;
                 c->read_pending[buf_id(out)] = false;
             }
+            if (c->fail_countdown > 0 && --c->fail_countdown == 0)   // sg_debug_fail_launch: this launch "fails" before it is enqueued
+                return fail(c, SG_ECUDA, "sg_run: injected launch failure (sg_debug_fail_launch)");
             const int k = ladder8_supported(c) ? launch_ladder8_pmj(c, c->sweeps, c->exchanges, (int)run, pt_every, out)
                           : gladder_supported(c) ? launch_gladder(c, c->sweeps, (int)run, c->exchanges, pt_every)
                                                  : launch_ladder_pmj(c, c->sweeps, (int)run, c->exchanges, pt_every, out);
@@ -612,6 +630,22 @@ int sg_run(sg_ctx *c, int n_sweeps, int pt_every, int meas_every)
         return SG_OK;
         };
         rc = run_loop();
+        if (overlap && rc) {
+            // Error exit: the caller's stream must still come after everything the two library streams were given, or a
+            // later sg_get_moments / sg_destroy could race a measurement that is still running.  The measurement of the
+            // last completed launch is still submitted, so that the counters (sweeps, n_meas) describe the state that
+            // is there; then both streams are joined and no read is left marked pending.  The first error is the one
+            // reported.
+            const std::string first_err = c->err;
+            submit_deferred();
+            c->stream = user_stream;
+            cudaStream_t lib_streams[2] = {c->stream_hi, c->stream2};
+            for (cudaStream_t ls : lib_streams)
+                if (cudaEventRecord(c->ev_join, ls) == cudaSuccess) cudaStreamWaitEvent(user_stream, c->ev_join, 0);
+            c->read_pending[0] = c->read_pending[1] = false;
+            c->err = first_err;
+            return rc;
+        }
         if (overlap) {                                              // ... and the caller's stream continues after both
             c->stream = user_stream;
             if (!rc) rc = check_cuda(c, cudaEventRecord(c->ev_join, c->stream_hi), "record exit");
@@ -904,6 +938,14 @@ int sg_get_launch_count(sg_ctx *c, uint64_t *launches)
 {
     if (!c || !launches) return SG_EINVAL;
     *launches = c->launches;
+    return SG_OK;
+}
+
+int sg_debug_fail_launch(sg_ctx *c, int countdown)
+{
+    if (!c) return SG_EINVAL;
+    if (countdown < 0) return fail(c, SG_EINVAL, "sg_debug_fail_launch: countdown < 0");
+    c->fail_countdown = countdown;
     return SG_OK;
 }
 

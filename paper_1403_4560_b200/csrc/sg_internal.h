@@ -71,6 +71,7 @@ struct sg_ctx {
     bool um_fresh;                      // U, M below are the kernels' own energies of the CURRENT state
     bool pending_exchange;              // L = 32 resident path: exchange `exchanges - 1` is decided and applied by the
                                         // next k_res32_pmj launch on load (or by flush_pending), from U, M below
+    int fail_countdown;                 // sg_debug_fail_launch: > 0 = the fail_countdown-th ladder launch of sg_run from now reports a failure
     uint32_t attr_done;                 // bit k: cudaFuncSetAttribute done for kernel family k on this context's device
     // device memory
     void *ws;                           // base of the workspace

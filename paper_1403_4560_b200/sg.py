@@ -43,6 +43,7 @@ EXPORTS = {
     "sg_get_counters": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "sg_get_launch_count": (C.c_int, [C.c_void_p, C.c_void_p]),
     "sg_last_error": (C.c_char_p, [C.c_void_p]),
+    "sg_debug_fail_launch": (C.c_int, [C.c_void_p, C.c_int]),
     "sg_set_kernel_path": (C.c_int, [C.c_void_p, C.c_int]),
     "sg_get_state_hash": (C.c_int, [C.c_void_p, C.c_void_p]),
     "sg_get_state_hash_noalloc": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -258,6 +259,9 @@ class Simulation:
         self._check(_lib.sg_get_moments(self._h, C.c_void_p(out.ctypes.data if hasattr(out, "ctypes") else out.data_ptr()),
                                         C.byref(n)))
         return n.value
+
+    def sg_debug_fail_launch(self, countdown):
+        self._check(_lib.sg_debug_fail_launch(self._h, int(countdown)))
 
     def sg_get_counters(self):
         a, b = C.c_uint64(), C.c_uint64()
