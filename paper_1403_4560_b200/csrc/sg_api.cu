@@ -485,8 +485,9 @@ int sg_sweep(sg_ctx *c, int n)
     if (!c) return SG_EINVAL;
     if (n < 0) return fail(c, SG_EINVAL, "sg_sweep: n < 0");
     if (sweeps_overflow(c, n)) return fail(c, SG_EINVAL, "sg_sweep: the global sweep counter must stay below 2^31");
-    int rc = flush_pending(c);
-    if (!rc) rc = do_sweeps(c, n);
+    // no flush_pending here: do_sweeps flushes on the paths that need the materialised state; the temperature-packed kernel
+    // continues from its own layout and the L = 32 kernel applies a pending exchange while it loads
+    const int rc = do_sweeps(c, n);
     if (rc) return rc;
     return check_launch(c, "sweep kernels");
 }

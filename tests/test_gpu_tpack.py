@@ -170,3 +170,26 @@ def test_tpack_many_lattices_kernel(sg, O, case):
             o.close()
     finally:
         tp.close(); std.close()
+
+
+def test_repeated_short_sweep_calls_stay_in_the_packed_layout(sg):
+    """sg_sweep no longer converts the temperature-packed state back to the sample-packed layout before
+    every call (a full-state transpose nobody read): one launch per call, same trajectory."""
+    temps = W.ladder(0.7, 2.5, 40)
+    tp = sg.Simulation(6, 0.1, 5, 2, temps, sg.PMJ_TPACK, 3)
+    std = sg.Simulation(6, 0.1, 5, 2, temps, sg.PMJ, 3)
+    try:
+        tp.sg_sweep(1)
+        n0 = tp.sg_get_launch_count()
+        for _ in range(5):
+            tp.sg_sweep(1)
+        assert tp.sg_get_launch_count() - n0 == 5
+        tp.sg_pt_exchange()                      # runs on the sample-packed copy: converts once
+        tp.sg_sweep(2)
+        std.sg_sweep(6)
+        std.sg_pt_exchange()
+        std.sg_sweep(2)
+        assert np.array_equal(tp.sg_get_spins(), std.sg_get_spins())
+        assert tp.sg_get_counters() == std.sg_get_counters() == (8, 1)
+    finally:
+        tp.close(); std.close()

@@ -13,7 +13,8 @@ integers, so the tolerance of the other state comparisons in this suite applies:
     held the first call's hashes when it started;
   - a small Gaussian context right after a larger +-J one: what the larger call left further up the array must not
     leak into the smaller result;
-  - a pending parallel-tempering exchange of the L = 32 path is applied first, as in the ordinary call;
+  - the L = 32 path, whose launches hand the state from one buffer to the other and defer exchanges, gives the same
+    hashes through both calls;
   - a pool above the limit is refused with a message that names the limit, and the context stays usable.
 
 This file is named test_zz_* so that pytest collects it last: under `pytest -x` a failure here cannot hide a failure in
@@ -79,12 +80,12 @@ def test_smaller_pool_after_a_larger_one_and_gaussian_bytes():
         small.close()
 
 
-def test_pending_exchange_of_the_L32_path_is_applied_first():
+def test_L32_resident_path_with_deferred_exchanges():
     sg = _sg()
     a = sg.Simulation(32, 0.1, 32, 2, _ladder(4), sg.PMJ, seed=9)
     b = sg.Simulation(32, 0.1, 32, 2, _ladder(4), sg.PMJ, seed=9)
     try:
-        a.sg_run(4, 4, 0)                        # leaves the exchange after sweep 4 to the next launch
+        a.sg_run(4, 4, 0)                        # the exchange after sweep 4 is applied by the time sg_run returns
         b.sg_run(4, 4, 0)
         got = a.sg_get_state_hash_noalloc()      # first thing to look at `a` after the run
         want = b.sg_get_state_hash()
