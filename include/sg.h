@@ -82,7 +82,7 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
 /* Multi-GPU sharding: declare that local sample 0 is global sample `first_sample`
  * of a larger disorder pool, so that every Philox stream is keyed by the GLOBAL sample / word index
  * and results do not depend on how the pool is split over GPUs.  first_sample >= 0, a multiple of
- * 32 for SG_PMJ.  Takes effect at the next sg_reset (call both right after sg_create). */
+ * 32 for SG_PMJ and SG_PMJ_TPACK.  Takes effect at the next sg_reset (call both right after sg_create). */
 int sg_set_first_sample(sg_ctx *ctx, int64_t first_sample);
 
 /* Regenerate couplings and initial spins from the seed, zero the counters and the accumulators:

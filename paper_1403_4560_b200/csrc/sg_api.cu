@@ -368,7 +368,7 @@ int sg_create(sg_ctx **out, int L, double h, int n_samples, int n_replicas, cons
     if (!out) return fail(nullptr, SG_EINVAL, "sg_create: out is NULL");
     if (!temps) return fail(nullptr, SG_EINVAL, "sg_create: temps is NULL");
     if (!valid_args(L, n_samples, n_replicas, n_temps, coupling_kind))
-        return fail(nullptr, SG_EINVAL, "sg_create: need even 4<=L<=64, n_samples>=1, n_replicas in {2,4}, 1<=n_temps<=64, kind in {0,1}");
+        return fail(nullptr, SG_EINVAL, "sg_create: need even 4<=L<=64, 1<=n_samples<=2^24, n_replicas in {2,4}, 1<=n_temps<=64, coupling_kind in {0 (SG_PMJ), 1 (SG_GAUSS), 2 (SG_PMJ_TPACK)}");
     if (!(h == h) || fabs(h) > 1e300) return fail(nullptr, SG_EINVAL, "sg_create: h must be finite");
     for (int t = 0; t < n_temps; ++t) {
         if (!(temps[t] > 0.0) || !(temps[t] < 1e308)) return fail(nullptr, SG_EINVAL, "sg_create: temperatures must be finite and > 0");
@@ -469,7 +469,7 @@ int sg_set_first_sample(sg_ctx *c, int64_t first_sample)
 {
     if (!c) return SG_EINVAL;
     if (first_sample < 0 || first_sample > 0x7fffffff - c->d.n_samples - 32 || (c->kind != SG_GAUSS && (first_sample & 31)))
-        return fail(c, SG_EINVAL, "sg_set_first_sample: need 0 <= first_sample < 2^31, a multiple of 32 for SG_PMJ");
+        return fail(c, SG_EINVAL, "sg_set_first_sample: need 0 <= first_sample < 2^31, a multiple of 32 for SG_PMJ / SG_PMJ_TPACK");
     c->d.s_first = (int)first_sample;
     return SG_OK;
 }

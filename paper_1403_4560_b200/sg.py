@@ -220,8 +220,9 @@ class Simulation:
         return prop, acc
 
     def sg_enable_pq(self, n_bins=None):
-        self.pq_bins = self.N + 1 if n_bins is None else int(n_bins)
-        self._check(_lib.sg_enable_pq(self._h, self.pq_bins))
+        n_bins = self.N + 1 if n_bins is None else int(n_bins)
+        self._check(_lib.sg_enable_pq(self._h, n_bins))
+        self.pq_bins = n_bins                   # only once the library has accepted it
 
     def sg_get_pq(self):
         out = np.empty((self.n_samples, self.NT, self.pq_bins), dtype=np.uint32)
@@ -229,8 +230,8 @@ class Simulation:
         return out
 
     def sg_enable_log_binning(self, n_windows):
-        self.n_windows = int(n_windows)
-        self._check(_lib.sg_enable_log_binning(self._h, self.n_windows))
+        self._check(_lib.sg_enable_log_binning(self._h, int(n_windows)))
+        self.n_windows = int(n_windows)         # only once the library has accepted it
 
     def sg_get_window_moments(self, k):
         out = np.empty((self.n_samples, self.NT, NMOM), dtype=np.float64)

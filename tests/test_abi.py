@@ -65,3 +65,9 @@ def test_workspace_bytes_and_validation_without_gpu():
     assert rc == -1 and not out.value
     lib.sg_last_error.restype = ctypes.c_char_p
     assert b"non-decreasing" in lib.sg_last_error(None)
+    # the message for a bad coupling_kind names all three kinds (SG_PMJ_TPACK = 2 exists)
+    temps = (ctypes.c_double * 2)(1.0, 2.0)
+    rc = lib.sg_create(ctypes.byref(out), 4, ctypes.c_double(0.1), 1, 4, temps, 2, 3, ctypes.c_uint64(1), None,
+                       ctypes.c_size_t(0), None)
+    assert rc == -1 and not out.value
+    assert b"SG_PMJ_TPACK" in lib.sg_last_error(None)

@@ -95,8 +95,14 @@ def test_diagnostics_error_paths_and_estimators(sg):
         sim.sg_enable_pq(8 ** 3 + 2)
     with pytest.raises(sg.SgError):
         sim.sg_enable_log_binning(0)
+    assert (sim.pq_bins, sim.n_windows) == (1, 0)          # a refused enable leaves the binding's sizes alone
     sim.sg_enable_pq(33)
     sim.sg_enable_log_binning(7)
+    with pytest.raises(sg.SgError):
+        sim.sg_enable_pq(0)
+    with pytest.raises(sg.SgError):
+        sim.sg_enable_log_binning(41)
+    assert (sim.pq_bins, sim.n_windows) == (33, 7) and sim.sg_get_pq().shape == (256, 2, 33)
     sim.sg_run(96, 1, 2)
     with pytest.raises(sg.SgError):
         sim.sg_get_window_moments(7)
