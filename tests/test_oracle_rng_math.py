@@ -86,6 +86,31 @@ def test_keyed_draw_layout(golden_dir):
         -1.0 if (v >> 5) & 1 else 1.0 for v in (0x9F3F38EF, 0x8C470732, 0x7E8A14F8))
 
 
+def test_initial_spin_bit_to_lane_mapping_from_bigint_philox():
+    """R6, initial spins: word 0 of philox(c0 = i, c1 = 0, c2, (2 << 24) | (a << 16) | t); +-J: c2 = packed word s >> 5 and
+    lane s & 31 reads bit s & 31 (1 <-> S = +1); Gaussian: c2 = s and bit 0 decides.  Expected values from the big-integer
+    restatement of Philox above, for lanes other than 0, a second word, every replica / slot and a 64-bit seed."""
+    seed = (0x9E3779B9 << 32) | 0x00C0FFEE
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    L, R, temps = 4, 4, list(W.ladder(0.5, 2.0, 5))
+    N = L ** 3
+    for kind, samples in ((O.PMJ, (5, 31, 32, 77)), (O.GAUSS, (0, 3, 33))):
+        for s in samples:
+            o = O.Oracle(L, 0.2, R, temps, kind=kind, seed=seed, sample=s)
+            S = o.spins()                                   # [a][t][i], before any sweep
+            o.close()
+            n_up = 0
+            for a in range(R):
+                for t in range(len(temps)):
+                    for i in range(N):
+                        c2, bit = (s >> 5, s & 31) if kind == O.PMJ else (s, 0)
+                        r0 = _philox_bigint([i, 0, c2, (2 << 24) | (a << 16) | t], key)[0]
+                        want = 1 if (r0 >> bit) & 1 else -1
+                        assert S[a, t, i] == want, (kind, s, a, t, i)
+                        n_up += want == 1
+            assert 0.4 < n_up / (R * len(temps) * N) < 0.6
+
+
 def test_thresholds_worked_example(golden_dir):
     o = O.Oracle(4, 0.3, 1, [0.5, 2.0])
     thr = o.thresholds()
