@@ -143,6 +143,17 @@ int sg_get_thresholds(sg_ctx *ctx, uint64_t *out);
 int sg_get_moments(sg_ctx *ctx, double *out, int64_t *n_meas);
 /* global sweep / exchange counters (either may be NULL) */
 int sg_get_counters(sg_ctx *ctx, uint64_t *sweeps_done, uint64_t *exchanges_done);
+/* Checkpoint / resume: every random draw is keyed by the global sweep / exchange counters, so a run continues
+ * on the same Philox streams from (spins, counters[, moment accumulators]).  Save with sg_get_spins, sg_get_counters,
+ * sg_get_moments; restore into a context created with the SAME parameters and seed (the couplings come from the seed) with
+ * sg_set_spins, sg_set_counters and, if measurements are to continue, sg_set_moments.  The continued run is bit-identical to
+ * an uninterrupted one.  Not restored: the parallel-tempering statistics (sg_get_pt_stats) and the diagnostics
+ * accumulators (P(q), logarithmic-binning windows), which restart from what the new context holds.
+ *   sg_set_counters  sweeps_done < 2^31 (SG_EINVAL beyond)
+ *   sg_set_moments   in: HOST ptr, [n_samples][n_temps][SG_NMOM] doubles as written by sg_get_moments; n_meas >= 0.
+ *                    Synchronous. */
+int sg_set_counters(sg_ctx *ctx, uint64_t sweeps_done, uint64_t exchanges_done);
+int sg_set_moments(sg_ctx *ctx, const double *in, int64_t n_meas);
 /* number of kernels this context has launched so far (for bench.py's gpu_launches) */
 int sg_get_launch_count(sg_ctx *ctx, uint64_t *launches);
 
@@ -216,6 +227,15 @@ int sg_enable_log_binning(sg_ctx *ctx, int n_windows);
 /* Window k: out HOST ptr [n_samples][n_temps][SG_NMOM] (may be NULL), n_meas = measurements that fell into the window
  * (may be NULL).  SG_ESTATE if not enabled, SG_EINVAL if k is out of range.  Synchronous. */
 int sg_get_window_moments(sg_ctx *ctx, int k, double *out, int64_t *n_meas);
+
+/* Which Metropolis comparison the +-J sweep kernels of this context run (it follows from h and the temperatures, DESIGN.md
+ * section 5), so that a benchmark can count the arithmetic of the code that actually ran:
+ *   SG_ACCEPT_BINARY_SEARCH  h != 0, |h| <= 1: three threshold compares per word-site (26 ALU-pipe lane-ops per word-site)
+ *   SG_ACCEPT_CARRY_CHAIN    h == 0: seven compares (30)
+ *   SG_ACCEPT_GENERAL        |h| > 1 or a non-monotone table: 14-mask select (no op-count model)
+ * SG_EUNSUPPORTED for SG_GAUSS. */
+enum { SG_ACCEPT_GENERAL = 0, SG_ACCEPT_CARRY_CHAIN = 1, SG_ACCEPT_BINARY_SEARCH = 2 };
+int sg_get_accept_variant(sg_ctx *ctx, int *variant);
 
 /* Fault injection for tests of the error paths: the `countdown`-th resident-ladder launch that sg_run would enqueue from
  * now on (L <= 16 paths) is not enqueued and sg_run returns SG_ECUDA instead; countdown = 0 disarms.  Everything enqueued

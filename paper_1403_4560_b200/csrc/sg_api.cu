@@ -935,10 +935,42 @@ int sg_get_counters(sg_ctx *c, uint64_t *sweeps_done, uint64_t *exchanges_done)
     return SG_OK;
 }
 
+int sg_set_counters(sg_ctx *c, uint64_t sweeps_done, uint64_t exchanges_done)
+{
+    if (!c) return SG_EINVAL;
+    if (sweeps_done >= (1ull << 31)) return fail(c, SG_EINVAL, "sg_set_counters: the global sweep counter must stay below 2^31");
+    const int rc = flush_pending(c);                        // an exchange still pending belongs to the OLD counters
+    if (rc) return rc;
+    c->sweeps = sweeps_done;
+    c->exchanges = exchanges_done;
+    c->um_fresh = false;
+    return SG_OK;
+}
+
+int sg_set_moments(sg_ctx *c, const double *in, int64_t n_meas)
+{
+    if (!c || !in) return SG_EINVAL;
+    if (n_meas < 0) return fail(c, SG_EINVAL, "sg_set_moments: n_meas < 0");
+    const size_t n = (size_t)c->d.n_samples * c->d.NT * SG_NMOM;
+    int rc;
+    if ((rc = check_cuda(c, cudaMemcpyAsync(c->acc, in, sizeof(double) * n, cudaMemcpyHostToDevice, c->stream), "copy moments"))) return rc;
+    if ((rc = check_cuda(c, cudaStreamSynchronize(c->stream), "sync moments"))) return rc;
+    c->n_meas = n_meas;
+    return SG_OK;
+}
+
 int sg_get_launch_count(sg_ctx *c, uint64_t *launches)
 {
     if (!c || !launches) return SG_EINVAL;
     *launches = c->launches;
+    return SG_OK;
+}
+
+int sg_get_accept_variant(sg_ctx *c, int *variant)
+{
+    if (!c || !variant) return SG_EINVAL;
+    if (c->kind == SG_GAUSS) return fail(c, SG_EUNSUPPORTED, "sg_get_accept_variant: +-J kinds only");
+    *variant = c->d.bs_accept ? SG_ACCEPT_BINARY_SEARCH : c->d.fast_accept ? SG_ACCEPT_CARRY_CHAIN : SG_ACCEPT_GENERAL;
     return SG_OK;
 }
 

@@ -14,6 +14,7 @@ NK, REC, NMOM = 12, 25, 66
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ESTATE = 0, -1, -2, -3, -4, -5
 PATH_AUTO, PATH_GENERIC = 0, 1
 NOALLOC_MAX_SYSTEMS = 65536
+ACCEPT_GENERAL, ACCEPT_CARRY_CHAIN, ACCEPT_BINARY_SEARCH = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "csrc", "libsg_b200.so")
@@ -42,8 +43,11 @@ EXPORTS = {
     "sg_get_moments": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "sg_get_counters": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "sg_get_launch_count": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "sg_set_counters": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint64]),
+    "sg_set_moments": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64]),
     "sg_last_error": (C.c_char_p, [C.c_void_p]),
     "sg_debug_fail_launch": (C.c_int, [C.c_void_p, C.c_int]),
+    "sg_get_accept_variant": (C.c_int, [C.c_void_p, C.c_void_p]),
     "sg_set_kernel_path": (C.c_int, [C.c_void_p, C.c_int]),
     "sg_get_state_hash": (C.c_int, [C.c_void_p, C.c_void_p]),
     "sg_get_state_hash_noalloc": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -261,6 +265,11 @@ class Simulation:
                                         C.byref(n)))
         return n.value
 
+    def sg_get_accept_variant(self):
+        v = C.c_int()
+        self._check(_lib.sg_get_accept_variant(self._h, C.byref(v)))
+        return v.value
+
     def sg_debug_fail_launch(self, countdown):
         self._check(_lib.sg_debug_fail_launch(self._h, int(countdown)))
 
@@ -268,6 +277,15 @@ class Simulation:
         a, b = C.c_uint64(), C.c_uint64()
         self._check(_lib.sg_get_counters(self._h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    def sg_set_counters(self, sweeps_done, exchanges_done):
+        self._check(_lib.sg_set_counters(self._h, int(sweeps_done), int(exchanges_done)))
+
+    def sg_set_moments(self, moments, n_meas):
+        m = np.ascontiguousarray(moments, dtype=np.float64)
+        if m.shape != (self.n_samples, self.NT, NMOM):
+            raise ValueError("sg_set_moments: expected shape %r" % ((self.n_samples, self.NT, NMOM),))
+        self._check(_lib.sg_set_moments(self._h, _p(m), int(n_meas)))
 
     def sg_get_launch_count(self):
         a = C.c_uint64()
