@@ -29,14 +29,29 @@ sys.path.insert(0, ROOT)
 
 from paper_1403_4560_b200 import workloads as W  # noqa: E402
 
-ALU_OPS_PER_WORDSITE = 30     # algorithmic ALU-pipe lane-ops per 32-sample word-site update:
-#                               6 bond XOR3 + 8 count + 7 threshold carries + 4 compare/flip + 5 Philox share
-HBM_BYTES_PER_WORDSITE_LAUNCH = 8   # spin word read once + written once per LAUNCH of a resident kernel (DESIGN.md §6)
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE roofline launch (the sweep kernel alone, n_k sweeps), from the
-# `ncu --set full` capture named beside it; a pointer to profiles/, not re-measured by this run
-NCU_TRAFFIC = {"C2": (10.92e6, "profiles/r01_v3_resident_kernels.md"),
-               "C3": (114.6e6, "profiles/r02c_kernels.md"),
-               "C5": (8.755e9, "profiles/r02c_kernels.md")}
+# Algorithmic ALU-pipe lane-ops per 32-sample word-site update, by the comparison the kernels of the
+# context actually run (sg_get_accept_variant): 6 bond XOR3 + 8 count + threshold carries + 4 compare/flip + 5 Philox share
+#   binary search (h != 0): 3 carries -> 26;  carry chain (h = 0): 7 carries -> 30;  general select: not modelled (30 assumed)
+ALU_OPS_BY_VARIANT = {2: 26, 1: 30, 0: 30}
+VARIANT_NAME = {2: "binary-search compare (3 carries)", 1: "carry chain (7 carries)", 0: "general 14-mask select (not modelled; 30 assumed)"}
+HBM_BYTES_PER_WORDSITE_LAUNCH = 8   # spin word read once + written once per LAUNCH of a resident kernel (DESIGN.md 6)
+# What `ncu --set full` reported for ONE roofline launch (the sweep kernel alone, n_k sweeps) of each +-J config, from the
+# capture summarised in the file named beside it: dram bytes (read + write), ALU-pipe active fraction
+# (sm__pipe_alu_cycles_active / sm__cycles_active) and executed thread-instructions per word-site (all pipes / ALU pipe
+# only).  Pointers to profiles/, not re-measured by this run; the line says so.  `frac` (algorithmic ops / peak) must stay
+# below `pipe_alu_active` (executed ops / peak) of the same launch: useful work cannot exceed executed work.
+NCU_CAPTURE = {
+    "C2": {"traffic": 10.90e6, "pipe_alu_active": 0.6890, "pipe_alu_elapsed": 0.6091, "inst_per_wordsite": 50.0,
+           "alu_inst_per_wordsite": 28.6, "source": "profiles/r03_kernels.md (k_ladder8_pmj<4,1,0>, 256 plain sweeps)"},
+    "C3": {"traffic": 114.7e6, "pipe_alu_active": 0.6880, "pipe_alu_elapsed": 0.6784, "inst_per_wordsite": 55.1,
+           "alu_inst_per_wordsite": 30.5, "source": "profiles/r03_kernels.md (k_ladder_pmj<12,1,0>, 256 plain sweeps)"},
+    "C5": {"traffic": 8.759e9, "pipe_alu_active": 0.6611, "pipe_alu_elapsed": 0.6589, "inst_per_wordsite": 48.4,
+           "alu_inst_per_wordsite": 27.7, "source": "profiles/r03_kernels.md (k_res32_pmj<1>, 16 sweeps)"},
+}
+# Gaussian path (C4), k_gladder<16>, one 256-sweep launch: executed thread instructions per flip attempt, issue-slot and pipe
+# utilisation, dram bytes of the launch
+GAUSS_CAPTURE = {"C4": {"inst_per_flip": 60.4, "issue_active": 0.776, "pipe_alu_active": 0.567, "pipe_fma_active": 0.413,
+                        "traffic": 514.6e6, "source": "profiles/r03_kernels.md (k_gladder<16>, 256 plain sweeps)"}}
 ALU_LANES_PER_SM = 64         # INT/LOP3 lanes per SM per clock (16 per SMSP x 4; B300_MICROARCH pipe table)
 N_SM = 148
 
@@ -234,28 +249,48 @@ def time_sweep_kernel(sim, w, stream, dev, reps=3):
     return float(sum(a.elapsed_time(b) for a, b in kev)) / reps, n_k, launches
 
 
-def roofline_block(w, sweep_ms, n_k, sweep_launches, step_ms, alu_peak, pk):
+def roofline_block(w, sweep_ms, n_k, sweep_launches, step_ms, alu_peak, pk, variant=2):
     ws = wordsites_per_sweep(w)
     nominal = ALU_LANES_PER_SM * N_SM * pk["sm_max_mhz"] * 1e6 / 1e12       # T lane-ops / s
     sweep_rate = w.flip_attempts(n_k) / (sweep_ms * 1e6)
     launch_s = sweep_ms * 1e-3 / max(1, sweep_launches)
     share = (sweep_ms / n_k) * w.n_sweeps / step_ms
     if w.kind != W.PMJ:
-        return {"bound": "alu", "kernel": "sweep (Gaussian fp32 byte path)", "achieved": None, "peak": None, "unit": "Tlaneop/s",
-                "frac": None, "traffic": None, "sweep_only_flips_per_ns": sweep_rate, "share_of_step": share,
+        # Gaussian byte/fp32 path: bound by instruction ISSUE (ncu: issue slots 78 % busy, ALU pipe 57 %, FMA pipe 41 %, LSU 16 %,
+        # no memory stall; profiles/r03_kernels.md).  Peak = 4 warp instructions per clock per SM = 128 thread-instruction slots.
+        # The work figure is the EXECUTED thread-instruction count per flip attempt of the named capture (no smaller
+        # algorithmic count is claimed for this path), so frac is an issue-slot utilisation, not an algorithmic efficiency.
+        cap = GAUSS_CAPTURE.get(w.name)
+        peak = 128.0 * N_SM * pk["sm_max_mhz"] * 1e6 / 1e12
+        ach = cap["inst_per_flip"] * sweep_rate * 1e9 / 1e12 if cap else None
+        return {"bound": "issue", "kernel": "sweep (Gaussian fp32 byte path, k_gladder)", "achieved": ach, "peak": peak,
+                "unit": "Tinst/s", "frac": ach / peak if cap else None, "traffic": cap["traffic"] if cap else None,
+                "peak_source": "nominal: 4 schedulers x 1 warp instruction (32 threads) per clock x 148 SMs x %.0f MHz" % pk["sm_max_mhz"],
+                "inst_per_flip_attempt": cap["inst_per_flip"] if cap else None,
+                "ncu": dict(cap, note="from the named `ncu --set full` capture of one 256-sweep launch (a pointer to profiles/, not "
+                                      "re-measured by this run)") if cap else None,
+                "sweep_only_flips_per_ns": sweep_rate, "share_of_step": share,
                 "launch_us": 1e6 * launch_s, "sweeps_per_launch": n_k // max(1, sweep_launches),
-                "note": "BASELINE.json sets no roofline target for the Gaussian path (parity only); no op-count model is claimed"}
-    ach = ALU_OPS_PER_WORDSITE * ws * n_k / (sweep_ms * 1e-3) / 1e12
+                "note": "BASELINE.json sets no roofline target for the Gaussian path (parity only); executed-instruction "
+                        "fraction of the issue-slot peak"}
+    ops = ALU_OPS_BY_VARIANT[variant]
+    ach = ops * ws * n_k / (sweep_ms * 1e-3) / 1e12
     hbm_ach = HBM_BYTES_PER_WORDSITE_LAUNCH * ws / launch_s / 1e9
-    traffic, traffic_src = NCU_TRAFFIC.get(w.name, (None, None))
+    cap = NCU_CAPTURE.get(w.name, {})
     return {"bound": "alu", "kernel": "sweep (+-J multispin)", "achieved": ach, "peak": alu_peak, "unit": "Tlaneop/s",
-            "frac": ach / alu_peak, "traffic": traffic,
-            "traffic_source": ("ncu --set full capture of one such launch, summarised in %s (an earlier commit's capture; "
-                               "a pointer, not re-measured by this run)" % traffic_src) if traffic_src else None,
+            "frac": ach / alu_peak, "traffic": cap.get("traffic"),
+            "accept_variant": VARIANT_NAME[variant],
+            "ncu": {"pipe_alu_active": cap.get("pipe_alu_active"), "pipe_alu_elapsed": cap.get("pipe_alu_elapsed"),
+                    "inst_per_wordsite": cap.get("inst_per_wordsite"),
+                    "alu_inst_per_wordsite": cap.get("alu_inst_per_wordsite"), "source": cap.get("source"),
+                    "note": "from the named `ncu --set full` capture of one such launch (a pointer to profiles/, not "
+                            "re-measured by this run): sm__pipe_alu_cycles_active as a fraction of active / of elapsed SM "
+                            "cycles, executed thread instructions and ALU-pipe lane slots per word-site.  frac counts "
+                            "algorithmic ops over wall time, so it must stay below pipe_alu_elapsed"},
             "peak_source": "measured in this run: dependency-free LOP3 micro-benchmark (csrc/probe/alu_probe.cu); "
                            "nominal 64 INT lanes/SM/clk x 148 SMs x %.0f MHz = %.2f" % (pk["sm_max_mhz"], nominal),
             "peak_nominal": nominal, "frac_of_nominal": ach / nominal,
-            "alu_ops_per_wordsite": ALU_OPS_PER_WORDSITE, "launch_us": 1e6 * launch_s,
+            "alu_ops_per_wordsite": ops, "launch_us": 1e6 * launch_s,
             "sweeps_per_launch": n_k // max(1, sweep_launches),
             "sweep_only_flips_per_ns": sweep_rate, "share_of_step": share,
             "hbm": {"achieved": hbm_ach, "peak": pk["hbm_gbs"], "peak_source": pk["src"], "unit": "GB/s", "frac": hbm_ach / pk["hbm_gbs"],
@@ -273,16 +308,29 @@ def short_run(sg, torch, name, sweeps, dev, stream, flush, alu_peak, pk):
     def barrier():
         torch.cuda.synchronize(dev)
 
-    ms, launches = time_steps(sim, w, step_plan(w), 2, 1, stream, flush, barrier)
+    ms, launches = time_steps(sim, w, step_plan(w), 3, 1, stream, flush, barrier)
     step_ms = float(np.mean(ms))
     sweep_ms, n_k, sl = time_sweep_kernel(sim, w, stream, dev)
     prop, acc = sim.sg_get_pt_stats()
+    variant = sim.sg_get_accept_variant() if w.kind == W.PMJ else 0
     sim.close()
-    rb = roofline_block(w, sweep_ms, n_k, sl, step_ms, alu_peak, pk)
-    return {"workload": "%s at %d of %d sweeps (same PT / measurement cadence)" % (name, sweeps, W.BY_NAME[name].n_sweeps),
-            "value": w.flip_attempts() / (step_ms * 1e6), "unit": "flips/ns", "ms_per_step": step_ms,
-            "sweep_only_flips_per_ns": rb["sweep_only_flips_per_ns"], "frac": rb["frac"], "gpu_launches_per_step": launches // 2,
-            "pt_acceptance": float(acc.sum()) / max(1.0, float(prop.sum()))}
+    rb = roofline_block(w, sweep_ms, n_k, sl, step_ms, alu_peak, pk, variant)
+    out = {"workload": "%s at %d of %d sweeps (same PT / measurement cadence)" % (name, sweeps, W.BY_NAME[name].n_sweeps),
+           "value": w.flip_attempts() / (step_ms * 1e6), "unit": "flips/ns", "ms_per_step": step_ms,
+           "ms_per_step_best": float(np.min(ms)), "ms_per_step_median": float(np.median(ms)),
+           "sweep_only_flips_per_ns": rb["sweep_only_flips_per_ns"], "frac": rb["frac"],
+           "alu_ops_per_wordsite": rb.get("alu_ops_per_wordsite"), "accept_variant": rb.get("accept_variant"),
+           "pipe_alu_active": (rb.get("ncu") or {}).get("pipe_alu_active"),
+           "pipe_alu_elapsed": (rb.get("ncu") or {}).get("pipe_alu_elapsed"), "ncu_source": (rb.get("ncu") or {}).get("source"),
+           "gpu_launches_per_step": launches // 3,
+           "pt_acceptance": float(acc.sum()) / max(1.0, float(prop.sum()))}
+    if w.kind == W.PMJ and w.n_samples % 32:
+        # idle lanes of the last packed word are simulated too (report both rates)
+        all_lanes = 32.0 * w.n_words / w.n_samples
+        out["active_lanes"] = "%d of %d" % (w.n_samples, 32 * w.n_words)
+        out["value_all_lanes"] = out["value"] * all_lanes
+        out["sweep_only_flips_per_ns_all_lanes"] = out["sweep_only_flips_per_ns"] * all_lanes
+    return out
 
 
 def run_ours(args, w):
@@ -322,6 +370,19 @@ def run_ours(args, w):
     total_ms = float(sum(step_ms))
     sweep_ms, n_k, sweep_launches = time_sweep_kernel(sim, w, stream, dev)
     prop, acc = sim.sg_get_pt_stats()
+    variant = sim.sg_get_accept_variant() if w.kind == W.PMJ else 0
+    # the launches the step really uses (sweeps between two exchanges + the exchange work fused into them), timed alone:
+    # 64 sweeps at the workload's PT cadence, no measurement
+    cad_ms = cad_launches = None
+    if w.pt_every > 0:
+        sim.sg_run(4 * w.pt_every, w.pt_every, 0)
+        l0 = sim.sg_get_launch_count()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record(stream)
+        sim.sg_run(64, w.pt_every, 0)
+        c1.record(stream)
+        torch.cuda.synchronize(dev)
+        cad_ms, cad_launches = float(c0.elapsed_time(c1)), int(sim.sg_get_launch_count() - l0)
     sampler.stop_flag = True
     sampler.join()
     alu_peak_measured = probe_alu_peak(stream) / 1e12                        # T lane-ops/s, LOP3 micro-benchmark
@@ -388,13 +449,21 @@ def run_ours(args, w):
 
     if rank == 0:
         ms_per_step = total_ms_max / args.steps
-        roofline = roofline_block(w, sweep_ms, n_k, sweep_launches, total_ms / args.steps, alu_peak_measured, pk)
+        roofline = roofline_block(w, sweep_ms, n_k, sweep_launches, total_ms / args.steps, alu_peak_measured, pk, variant)
+        if cad_ms is not None:
+            roofline["step_cadence"] = {
+                "what": "64 sweeps with PT every %d through sg_run, no measurement: the launches the timed step is made of" % w.pt_every,
+                "flips_per_ns": w.flip_attempts(64) / (cad_ms * 1e6), "launches": cad_launches,
+                "launch_us": 1e3 * cad_ms / max(1, cad_launches)}
         out = {"metric": "spin_flip_attempts_per_ns", "value": value, "unit": "flips/ns", "n_gpus": world,
                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+               "ms_per_step_best": float(np.min(step_ms)), "ms_per_step_median": float(np.median(step_ms)),
                "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                "dtype": "u32" if w.kind == W.PMJ else "f32", "data": "synthetic",
                "config": workload_config(w, world), "clocks": sampler.result(),
                "e2e": {"value": e2e_value, "unit": "flips/ns", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                       "h2d_note": "computed from the sizes of the tables sg_create uploads (temperatures, per-slot thresholds, "
+                                   "exp tables, twiddles), not counted by the library; couplings and spins are generated on the device",
                        "result": "moment accumulators" if measures else "per-system energies (U, M) of the final state"},
                "gpu_launches": int(launches), "roofline": roofline,
                "pt": {"proposed": int(prop.sum()), "accepted": int(acc.sum()),
@@ -405,7 +474,7 @@ def run_ours(args, w):
             others = {}
             del workspace
             torch.cuda.empty_cache()
-            for name, sweeps in (("C2", 2048), ("C3", 1024), ("C4", 256)):
+            for name, sweeps in (("C1", 1000), ("C2", 2048), ("C3", 1024), ("C4", 256)):
                 if name != w.name:
                     others[name] = short_run(sg, torch, name, sweeps, dev, stream, flush, alu_peak_measured, pk)
             out["other_configs"] = others
