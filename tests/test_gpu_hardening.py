@@ -210,6 +210,56 @@ def test_config5_first_sweeps_many_samples(sg, O):
     sim.close()
 
 
+def _check_sample(O, w, temps, plan, s, spins_s, U_s, M_s, mom_s):
+    """Oracle run of sample s compared in the worker (nothing but the verdict is kept): returns accepted swaps."""
+    want = oracle_job(O, w.L, w.h, w.n_replicas, temps, w.kind, w.seed, s, plan)
+    assert np.array_equal(spins_s, want["spins"]), "sample %d: spins" % s
+    assert np.array_equal(U_s, want["U"]) and np.array_equal(M_s, want["M"]), "sample %d: kernels' own energies" % s
+    if mom_s is not None:
+        assert close(mom_s, want["mom"]), "sample %d: moments" % s
+    return want["pt"][1]
+
+
+@pytest.mark.parametrize("name", ["C3", "C4"])
+def test_all_samples_of_config3_and_config4_first_32_sweeps(sg, O, name):
+    """SURVEY.md §8d (1), VERDICT round 2 (missing 5): EVERY sample of config 3 (4096) and config 4 (512, Gaussian) for the
+    first 32 sweeps (PT every sweep, measurements at sweeps 16 and 32) directly against the oracle - spins, the kernels' own
+    (U, M), moments, accepted swaps of the whole pool - so that the resident kernels are not only checked through another
+    GPU path that shares their device headers."""
+    w = W.BY_NAME[name]
+    temps = w.temps()
+    sim = sg.Simulation(w.L, w.h, w.n_samples, w.n_replicas, temps, w.kind, w.seed)
+    try:
+        sim.sg_run(32, 1, 16)
+        spins = sim.sg_get_spins()
+        Uc, Mc = sim.sg_get_energies_cached()
+        mom, n = sim.sg_get_moments()
+        prop, acc = sim.sg_get_pt_stats()
+        assert n == 2
+    finally:
+        sim.close()
+    accepted = list(POOL.map(lambda s: _check_sample(O, w, temps, [(32, 1, 16)], s, spins[s], Uc[s], Mc[s], mom[s]),
+                             range(w.n_samples)))
+    assert int(acc.sum()) == sum(accepted)
+
+
+def test_config5_first_sweeps_every_word(sg, O):
+    """The same for config 5 (first 4 sweeps + the first exchange): 1024 samples, four rotating lanes of EVERY one of the
+    256 packed words."""
+    w = W.BY_NAME["C5"]
+    temps = w.temps()
+    samples = sorted(32 * wd + (wd + 8 * k) % 32 for wd in range(w.n_words) for k in range(4))
+    assert len(set(samples)) == 1024
+    sim = sg.Simulation(w.L, w.h, w.n_samples, w.n_replicas, temps, w.kind, w.seed)
+    try:
+        sim.sg_run(4, 4, 0)
+        Uc, Mc = sim.sg_get_energies_cached()
+        spins = {s: sim.sg_get_spins(s, 1)[0] for s in samples}
+    finally:
+        sim.close()
+    list(POOL.map(lambda s: _check_sample(O, w, temps, [(4, 4, 0)], s, spins[s], Uc[s], Mc[s], None), samples))
+
+
 # ------------------------------------------------------------------------------------------------ (c)
 TIGHT = [
     # name, L, h, n_samples, R, NT, (T_lo, T_hi), kind, pt_every, n_sweeps
