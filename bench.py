@@ -57,11 +57,11 @@ N_SM = 148
 
 
 def probe_alu_peak(stream):
-    """Measured ALU-pipe (LOP3) peak in lane-ops/s: bench-only micro-benchmark (csrc/probe/alu_probe.cu),
-    a library of its own, not part of the product ABI."""
+    """Measured ALU-pipe (LOP3) peak in lane-ops/s: bench-only micro-benchmark (bench_probe/alu_probe.cu),
+    a library of its own beside bench.py, not part of the product package or its ABI."""
     import ctypes as C
-    from paper_1403_4560_b200 import build
-    lib = C.CDLL(build.build_probe())
+    from bench_probe import build as probe_build
+    lib = C.CDLL(probe_build.build_probe())
     lib.sgprobe_alu_peak.restype = C.c_int
     lib.sgprobe_alu_peak.argtypes = [C.c_void_p, C.c_void_p]
     v = C.c_double()
@@ -287,7 +287,7 @@ def roofline_block(w, sweep_ms, n_k, sweep_launches, step_ms, alu_peak, pk, vari
                             "re-measured by this run): sm__pipe_alu_cycles_active as a fraction of active / of elapsed SM "
                             "cycles, executed thread instructions and ALU-pipe lane slots per word-site.  frac counts "
                             "algorithmic ops over wall time, so it must stay below pipe_alu_elapsed"},
-            "peak_source": "measured in this run: dependency-free LOP3 micro-benchmark (csrc/probe/alu_probe.cu); "
+            "peak_source": "measured in this run: dependency-free LOP3 micro-benchmark (bench_probe/alu_probe.cu); "
                            "nominal 64 INT lanes/SM/clk x 148 SMs x %.0f MHz = %.2f" % (pk["sm_max_mhz"], nominal),
             "peak_nominal": nominal, "frac_of_nominal": ach / nominal,
             "alu_ops_per_wordsite": ops, "launch_us": 1e6 * launch_s,

@@ -11,8 +11,6 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libsg_b200.so")
-PROBE_SRC = os.path.join(CSRC, "probe", "alu_probe.cu")
-PROBE_LIB = os.path.join(CSRC, "probe", "libsg_probe.so")     # bench-only micro-benchmark, not the product ABI
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",
          "-Xcompiler", "-fPIC,-O2,-Wall", "-shared"]
@@ -30,18 +28,9 @@ def headers():
         [os.path.join(HERE, "..", "include", "sg.h")]
 
 
-def build_probe(force=False):
-    if force or not os.path.exists(PROBE_LIB) or os.path.getmtime(PROBE_LIB) < os.path.getmtime(PROBE_SRC):
-        tmp = PROBE_LIB + ".tmp.%d" % os.getpid()
-        subprocess.run([NVCC, *FLAGS, "-o", tmp, PROBE_SRC], check=True)
-        os.replace(tmp, PROBE_LIB)
-    return PROBE_LIB
-
-
 def build(force=False, verbose=False, extra=()):
     """Compile every csrc/*.cu to an object (in parallel, only the stale ones) and link libsg_b200.so."""
     from concurrent.futures import ThreadPoolExecutor
-    build_probe(force)
     os.makedirs(OBJ_DIR, exist_ok=True)
     hdr_t = max(os.path.getmtime(p) for p in headers())
     compile_flags = [f for f in FLAGS if f != "-shared"]
